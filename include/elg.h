@@ -1,0 +1,185 @@
+/* elg.h -- C ABI of libelg: B200-native (sm_100a) tracking of a 6-D fp64 macroparticle bunch through a
+ * lumped-element beamline -- the data-parallel hot path of arXiv:1710.07350 ("GPU acceleration and
+ * performance of the particle-beam-dynamics code Elegant").
+ *
+ * Citations: "PAPER.md:NN" = line of the paper text; "Gk" = reading k in DESIGN.md ("Readings").
+ *
+ * Problem statement: a bunch of particles traverses a succession of elements.  Per-particle
+ * element maps, particle loss, a longitudinal wake built from a
+ * histogram and an array convolution and beam-moment reductions (PAPER.md:123-131,
+ * 145) are all computed by CUDA kernels of this library; nothing is computed on the host and there is no
+ * CPU fallback: every compute call fails with ELG_ECUDA when no device is usable.
+ *
+ * Conventions
+ *  - Every call returns an int32 status: ELG_OK = 0, negative = error.  No exceptions or aborts cross the
+ *    ABI; elg_last_error() returns a thread-local message for the last failing call.
+ *  - "d_" arguments are DEVICE pointers, "h_" arguments are HOST pointers.  The library allocates no
+ *    device memory: the caller (PyTorch in this repo) allocates the particle store and one workspace and
+ *    lends them to the bunch handle for its lifetime.  While a bunch handle exists the caller must not
+ *    write those buffers (the paper nulls the host pointer while the device owns the data).
+ *  - Calls are asynchronous on the stream given to elg_bunch_create, except those that return host data
+ *    (elg_moments, elg_lost, elg_n_alive, elg_bunch_read, and elg_track when it has host outputs), which
+ *    synchronise that stream (the paper's finishReductionStreams moment).
+ *  - Coordinates (G1): 0 x [m], 1 x' [rad], 2 y [m], 3 y' [rad], 4 s [m] (total path length,
+ *    PAPER.md:75-77), 5 delta = (p-p0)/p0; plus an int64 particle ID.
+ *
+ * Particle store layout (struct of arrays): seven arrays, each elg_soa_stride(n0)
+ * elements of 8 bytes apart, in the order x, x', y, y', s, delta (fp64) and ID (int64); the buffer is
+ * 7 * stride * 8 bytes and must be 256-byte aligned.  The live particles are the prefix [0, n_alive) of
+ * every array, in their original relative order (stable compaction, G18/G19).
+ */
+#ifndef ELG_H
+#define ELG_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ELG_OK = 0, ELG_EINVAL = -1, ELG_ENOMEM = -2, ELG_ECUDA = -3, ELG_ESTATE = -4, ELG_ECAPACITY = -5 };
+
+/* element types (glossary PAPER.md:175; Table I rows PAPER.md:143-165) */
+enum { ELG_DRIFT = 1, ELG_MATRIX = 2, ELG_RFKICK = 3, ELG_RCOL = 4, ELG_ECOL = 5, ELG_WAKE = 6, ELG_HISTO = 7 };
+/* histogram window modes (G10) */
+enum { ELG_WIN_EXPLICIT = 0, ELG_WIN_AUTO_MINMAX = 1, ELG_WIN_AUTO_TABLE = 2 };
+/* wake kinds (G12) */
+enum { ELG_WAKE_RESONATOR = 0, ELG_WAKE_TABLE = 1 };
+/* when elg_track records moments (G26) */
+enum { ELG_MOM_NONE = 0, ELG_MOM_TURN = 1, ELG_MOM_ELEMENT = 2 };
+
+/* One beamline element; all pointers are HOST pointers, copied by elg_beamline_load.
+ *   DRIFT  (Listing 1): L.   x += x'L; y += y'L; s += L sqrt(1 + x'^2 + y'^2)
+ *   MATRIX (G3): R (36 doubles, row-major R[6r+c]), C (6 doubles or NULL = 0).
+ *                                   v <- C + R v, each row accumulated from C[r] over c = 0..5 with FMAs
+ *   RFKICK (G8): V [V], f [Hz], phi [rad].
+ *                                   delta += V/(beta0 p0c) sin(phi + 2 pi f (s - s_ref)/(beta0 c)),
+ *                                   s_ref = design path length in front of the element on this turn
+ *   RCOL   (G17): ax, ay [m].  survive iff |x| <= ax and |y| <= ay
+ *   ECOL   (G17): ax, ay [m] semi-axes.  survive iff (x/ax)^2 + (y/ay)^2 <= 1
+ *   WAKE   (G9-G16): nb bins, window mode (+ t_lo_rel, dt if EXPLICIT), wake kind with
+ *                                   (f, Q, Rs) or (table, n_table, dt_table), interp (1 = linear between
+ *                                   bin centres, 0 = own bin)
+ *   HISTO: nb, window, t_lo_rel, dt: time histogram only (diagnostic), no kick
+ */
+typedef struct {
+    int32_t type;
+    int32_t nb;
+    int32_t window;
+    int32_t wake;
+    int32_t interp;
+    int32_t reserved;
+    double L;
+    double V, f, phi;
+    double ax, ay;
+    double Q, Rs;
+    double t_lo_rel, dt, dt_table;
+    const double* R;
+    const double* C;
+    const double* table;
+    int64_t n_table;
+} elg_element;
+
+typedef struct elg_bunch elg_bunch;
+typedef struct elg_beamline elg_beamline;
+
+/* Options of elg_track.  All pointers are HOST pointers (nullable); when any is non-NULL the call
+ * synchronises the stream before returning.
+ *   records : capacity_records x 43 doubles, one record = n_alive, centroid[6], Sigma[36] row-major
+ *             (population central moments over live particles, G20); taken after every turn
+ *             (ELG_MOM_TURN) or after every element (ELG_MOM_ELEMENT, G26).  n_records returns the number
+ *             of records taken (may exceed the capacity; the excess is dropped).
+ *   hist_out / V_out / window_out : per-stage outputs of the successive WAKE/HISTO executions (counts
+ *             uint32[nb]; V double[nb] for WAKE only; window = t_lo, dt, 1/dt), used by the stage-by-stage
+ *             parity protocol; *_written return the totals (in entries / triples).
+ */
+typedef struct {
+    int32_t moments_every;
+    int32_t reserved;
+    double* records;
+    int64_t capacity_records;
+    int64_t n_records;
+    uint32_t* hist_out;
+    int64_t hist_capacity;
+    int64_t hist_written;
+    double* V_out;
+    int64_t V_capacity;
+    int64_t V_written;
+    double* window_out;
+    int64_t window_capacity;
+    int64_t window_written;
+} elg_track_opts;
+
+/* ---- library ---------------------------------------------------------------------------------- */
+const char* elg_version(void);
+const char* elg_last_error(void);
+/* number of kernels this library has launched in this process (for bench.py's gpu_launches) */
+int64_t elg_launch_count(void);
+
+/* ---- particle store geometry ------------------------------------------------------------------ */
+/* elements between successive arrays of the store: n0 rounded up to a multiple of 32 (256 bytes) */
+int64_t elg_soa_stride(int64_t n0);
+/* 7 * stride * 8 */
+int64_t elg_soa_bytes(int64_t n0);
+
+/* ---- beamline (host only; needs no device) ----------------------------------------------------- */
+/* Validates and copies n_elems elements (L finite, apertures > 0, nb >= 2, Q > 1/2, ...).  On a bad
+ * element returns ELG_EINVAL and elg_last_error() names its index.  ring = 1: the line closes on itself,
+ * RF phase references and EXPLICIT windows advance by the line length every turn (G8).  The design path
+ * length is the sequential fp64 sum of L (DRIFT) and C[4] (MATRIX) of the preceding elements. */
+int32_t elg_beamline_load(elg_beamline** out, const elg_element* h_elems, int64_t n_elems, int32_t ring);
+void    elg_beamline_destroy(elg_beamline*);
+int64_t elg_beamline_n_elements(const elg_beamline*);
+double  elg_beamline_length(const elg_beamline*);
+/* design path length in front of element k (0 <= k <= n_elems) on turn 0 */
+double  elg_beamline_s_design(const elg_beamline*, int64_t k);
+/* number of kernel launches one turn takes under the given moments mode (fused runs, north_star part 1) */
+int64_t elg_beamline_launches_per_turn(const elg_beamline*, int32_t moments_every);
+
+/* ---- bunch ------------------------------------------------------------------------------------- */
+/* Workspace size for a bunch of n0 particles tracked through bl (nullable: sized for nb <= 65536 and
+ * tables <= 65536 points), with room for lost_capacity lost-particle records (0 = none kept). */
+int32_t elg_workspace_bytes(int64_t n0, const elg_beamline* bl, int64_t lost_capacity, int64_t* bytes);
+/* Borrow d_soa (layout above; already filled by the caller, or to be filled by elg_bunch_upload) and
+ * d_work (256-byte aligned, work_bytes >= elg_workspace_bytes(n0, sized_for, lost_capacity); sized_for is
+ * only read during this call).  p0c_eV, mc2_eV: reference momentum and
+ * rest energy (G7); charge_C: bunch charge, macro-charge q = charge / n0 for the whole run (G15).
+ * stream: a cudaStream_t (NULL = default stream).  n_alive = n0, turn = 0, lost log empty. */
+int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, void* d_work, int64_t work_bytes,
+                         const elg_beamline* sized_for, int64_t lost_capacity, double p0c_eV, double mc2_eV, double charge_C, void* stream);
+void    elg_bunch_destroy(elg_bunch*);
+/* Copy n0 particles from host arrays (pinned or pageable) into the store and rewind the bunch.
+ * h_ids NULL: ID = index (G27). */
+int32_t elg_bunch_upload(elg_bunch*, const double* const h_coords[6], const int64_t* h_ids);
+/* The caller has rewritten d_soa with n0 fresh particles: n_alive = n0, turn = 0, lost log empty. */
+int32_t elg_bunch_rewind(elg_bunch*);
+
+/* Track n_turns passes through the beamline.  opts nullable. */
+int32_t elg_track(elg_bunch*, const elg_beamline*, int64_t n_turns, elg_track_opts* opts);
+
+/* Moments of the live particles now (north_star part 4).  n_alive == 0: ELG_ESTATE, outputs untouched. */
+int32_t elg_moments(elg_bunch*, int64_t* n_alive, double h_centroid[6], double h_sigma[36]);
+/* Lost-particle log in canonical order (G18): chronological (turn, element index), then original array
+ * position.  coords6 is cap x 6 row-major (the coordinates at the aperture; its s is the loss position),
+ * nullable.  cap < n_lost: fills cap records and returns ELG_ECAPACITY with the true n_lost. */
+int32_t elg_lost(elg_bunch*, int64_t* n_lost, int64_t cap, int64_t* h_ids, int32_t* h_turn, int32_t* h_elem,
+                 double* h_coords6);
+int32_t elg_n_alive(elg_bunch*, int64_t* n_alive);
+/* Copy the live particles to host arrays of capacity cap each (any pointer nullable). */
+int32_t elg_bunch_read(elg_bunch*, double* const h_coords[6], int64_t* h_ids, int64_t cap);
+/* Device pointer of coordinate c (0..5) or of the IDs (c = 6) in the CURRENT store (compaction ping-pongs
+ * between d_soa and a copy in the workspace). */
+int32_t elg_bunch_device_array(elg_bunch*, int32_t c, void** d_ptr);
+
+/* ---- single-stage test hooks (same kernels as elg_track; device arrays supplied by the caller) ----- */
+int32_t elg_dbg_histogram(const double* d_s, int64_t n, double inv_bc, double t_lo, double inv_dt, int32_t nb,
+                          uint32_t* d_counts, void* stream);
+int32_t elg_dbg_wake_samples(int32_t kind, int32_t nb, double dt, double f, double Q, double Rs,
+                             const double* d_table, int64_t n_table, double dt_table, double* d_W, void* stream);
+int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W, int32_t nb, double q, double* d_V,
+                         void* stream);
+int32_t elg_dbg_kick(const double* d_s, double* d_delta, int64_t n, double inv_bc, double t_lo, double inv_dt,
+                     int32_t nb, const double* d_V, double inv_E, int32_t interp, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

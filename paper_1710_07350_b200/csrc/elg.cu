@@ -1,0 +1,767 @@
+// elg.cu -- C ABI of libelg (include/elg.h): host-side planning and kernel launches.
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -fmad=false -shared -Xcompiler -fPIC
+// The host code holds no particle arithmetic: it cuts the beamline into fused runs, fills kernel
+// parameter blocks and launches the kernels of elg_kernels.cuh.  There is no CPU fallback.
+#include "../../include/elg.h"
+#include "elg_kernels.cuh"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace elg;
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<long long> g_launches{0};
+
+int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
+
+#define ELG_CK(call)                                                                           \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(ELG_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
+    } while (0)
+
+constexpr double kCLight = 299792458.0;                 // m/s
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+constexpr int kMaxOpsSmall = 8;
+constexpr int kMaxOpsLarge = 80;                        // 80 x 42 x 8 B = 26.9 KB of kernel parameters
+constexpr int kMaxGrid = 4096;
+constexpr long long kRecCap = 2048;                     // device ring of moment records
+constexpr int kNbDefault = 65536;
+
+inline long long align_up(long long x, long long a) { return (x + a - 1) / a * a; }
+
+struct HostOp {
+    uint8_t type;
+    double coef[42];
+};
+
+struct ResConst { double kloss, alpha, wbar, ratio; };
+
+}  // namespace
+
+struct elg_beamline {
+    std::vector<elg_element> e;
+    std::vector<std::vector<double>> R, C, table;
+    std::vector<ResConst> res;
+    std::vector<double> s_design;
+    double length = 0.0;
+    int32_t ring = 0;
+    int32_t nb_max = 0;
+    long long table_total = 0;
+    std::vector<long long> table_off;                   // offset of element k's table in the device copy
+    unsigned long long serial = 0;
+};
+
+struct elg_bunch {
+    long long n0 = 0, stride = 0, lost_cap = 0, work_bytes = 0;
+    char* d_soa = nullptr;
+    char* d_work = nullptr;
+    cudaStream_t stream = nullptr;
+    double p0c = 0, mc2 = 0, charge = 0, beta0 = 0, inv_bc = 0, inv_E = 0, q_macro = 0;
+    // workspace carve-up
+    DevState* st = nullptr;
+    char* soaB = nullptr;
+    unsigned long long* tile_status = nullptr;
+    double* mm_partial = nullptr;
+    double* mom_partial = nullptr;
+    double* records = nullptr;
+    unsigned int* counts = nullptr;
+    double* W = nullptr;
+    double* V = nullptr;
+    double* table = nullptr;
+    long long nb_cap = 0, table_cap = 0;
+    long long* lost_id = nullptr;
+    long long* lost_te = nullptr;
+    double* lost_v = nullptr;
+    // dynamic state mirrored on the host without any device read
+    int cur_buf = 0;                                    // 0: d_soa, 1: workspace copy
+    int cur_slot = 0;
+    unsigned int epoch = 0;
+    long long turn = 0;
+    unsigned long long table_serial = 0;
+    long long rec_count = 0;                            // records in the device ring
+    // launch geometry
+    int sms = 0;
+    int grid_chain[2][2] = {{0, 0}, {0, 0}};            // [large][compact]
+    int grid_hist = 0, grid_mom = 0;
+    int hist_aggregate = 0;
+
+    double* coord(int buf, int c) const { return reinterpret_cast<double*>((buf ? soaB : d_soa) + (long long)c * stride * 8); }
+    long long* ids(int buf) const { return reinterpret_cast<long long*>((buf ? soaB : d_soa) + 6LL * stride * 8); }
+};
+
+namespace {
+
+unsigned long long g_bl_serial = 0;
+
+// ------------------------------------------------------------------------------------- workspace
+struct WorkLayout {
+    long long off_state, off_soaB, off_status, off_mm, off_mom, off_rec, off_counts, off_W, off_V, off_table,
+        off_lost_id, off_lost_te, off_lost_v, total;
+};
+
+WorkLayout layout(long long n0, long long nb_cap, long long table_cap, long long lost_cap) {
+    WorkLayout L{};
+    const long long stride = elg_soa_stride(n0);
+    long long o = 0;
+    L.off_state = o; o = align_up(o + (long long)sizeof(DevState), 256);
+    L.off_soaB = o; o = align_up(o + 7 * stride * 8, 256);
+    L.off_status = o; o = align_up(o + (stride / kTile + 2) * 8, 256);
+    L.off_mm = o; o = align_up(o + 2LL * kMaxGrid * 8, 256);
+    L.off_mom = o; o = align_up(o + (long long)kNMom * kMaxGrid * 8, 256);
+    L.off_rec = o; o = align_up(o + (kRecCap + 1) * 43 * 8, 256);   // + 1: elg_moments' own slot
+    L.off_counts = o; o = align_up(o + nb_cap * 4, 256);
+    L.off_W = o; o = align_up(o + nb_cap * 8, 256);
+    L.off_V = o; o = align_up(o + nb_cap * 8, 256);
+    L.off_table = o; o = align_up(o + table_cap * 8, 256);
+    L.off_lost_id = o; o = align_up(o + lost_cap * 8, 256);
+    L.off_lost_te = o; o = align_up(o + lost_cap * 8, 256);
+    L.off_lost_v = o; o = align_up(o + 6 * lost_cap * 8, 256);
+    L.total = o;
+    return L;
+}
+
+void caps_for(const elg_beamline* bl, long long* nb_cap, long long* table_cap) {
+    *nb_cap = bl ? (bl->nb_max > 2 ? bl->nb_max : 2) : kNbDefault;
+    *table_cap = bl ? (bl->table_total > 1 ? bl->table_total : 1) : kNbDefault;
+}
+
+template <class K>
+int32_t grid_for(K kernel, int sms, int smem, int* out) {
+    int occ = 0;
+    ELG_CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kBlock, smem));
+    if (occ < 1) return fail(ELG_ECUDA, "kernel does not fit on an SM");
+    long long g = (long long)occ * sms;
+    if (g > kMaxGrid) g = kMaxGrid / sms * sms;
+    *out = (int)g;
+    return ELG_OK;
+}
+
+int32_t device_sms(int* sms) {
+    int dev = 0;
+    ELG_CK(cudaGetDevice(&dev));
+    ELG_CK(cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, dev));
+    return ELG_OK;
+}
+
+int32_t hist_setup_once() {
+    static bool done = false;
+    if (!done) {
+        ELG_CK(cudaFuncSetAttribute(hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kHistSmemBins * 4));
+        done = true;
+    }
+    return ELG_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+extern "C" const char* elg_version(void) { return "elg 0.1 (sm_100a)"; }
+extern "C" const char* elg_last_error(void) { return g_err.c_str(); }
+extern "C" int64_t elg_launch_count(void) { return g_launches.load(); }
+extern "C" int64_t elg_soa_stride(int64_t n0) { return n0 <= 0 ? 32 : align_up(n0, 32); }
+extern "C" int64_t elg_soa_bytes(int64_t n0) { return 7 * elg_soa_stride(n0) * 8; }
+
+// ------------------------------------------------------------------------------------- beamline
+extern "C" int32_t elg_beamline_load(elg_beamline** out, const elg_element* elems, int64_t n_elems, int32_t ring) {
+    if (!out || n_elems < 0 || (n_elems > 0 && !elems)) return fail(ELG_EINVAL, "elg_beamline_load: bad arguments");
+    elg_beamline* bl = new (std::nothrow) elg_beamline;
+    if (!bl) return fail(ELG_ENOMEM, "elg_beamline_load: out of host memory");
+    bl->ring = ring;
+    bl->e.assign(elems, elems + n_elems);
+    bl->R.resize(n_elems); bl->C.resize(n_elems); bl->table.resize(n_elems);
+    bl->res.resize(n_elems); bl->table_off.assign(n_elems, 0);
+    bl->s_design.resize(n_elems + 1);
+    bl->serial = ++g_bl_serial;
+    double s = 0.0;                                         // G8: sequential ascending fp64 sum
+    for (int64_t k = 0; k < n_elems; k++) {
+        elg_element& e = bl->e[k];
+        bl->s_design[k] = s;
+        const char* why = nullptr;
+        switch (e.type) {
+            case ELG_DRIFT:
+                if (!std::isfinite(e.L)) why = "DRIFT: L not finite"; else s = s + e.L;
+                break;
+            case ELG_MATRIX:
+                if (!e.R) { why = "MATRIX: R is NULL"; break; }
+                bl->R[k].assign(e.R, e.R + 36); e.R = bl->R[k].data();
+                if (e.C) { bl->C[k].assign(e.C, e.C + 6); e.C = bl->C[k].data(); s = s + e.C[4]; }
+                break;
+            case ELG_RFKICK:
+                if (!std::isfinite(e.V) || !std::isfinite(e.f) || !std::isfinite(e.phi)) why = "RFKICK: V, f, phi must be finite";
+                break;
+            case ELG_RCOL: case ELG_ECOL:
+                if (!(e.ax > 0.0) || !(e.ay > 0.0)) why = "aperture: ax, ay must be > 0";
+                break;
+            case ELG_WAKE: case ELG_HISTO:
+                if (e.nb < 2) { why = "WAKE/HISTO: nb < 2"; break; }
+                if (e.nb > (1 << 24)) { why = "WAKE/HISTO: nb > 2^24"; break; }
+                if (e.window < ELG_WIN_EXPLICIT || e.window > ELG_WIN_AUTO_TABLE) { why = "WAKE/HISTO: bad window mode"; break; }
+                if (e.window == ELG_WIN_EXPLICIT && (!(e.dt > 0.0) || !std::isfinite(e.t_lo_rel))) { why = "EXPLICIT window: dt > 0 and finite t_lo_rel required"; break; }
+                if (e.nb > bl->nb_max) bl->nb_max = e.nb;
+                if (e.type == ELG_WAKE) {
+                    if (e.wake == ELG_WAKE_RESONATOR) {
+                        if (!(e.Q > 0.5) || !(e.f > 0.0) || !std::isfinite(e.Rs)) { why = "resonator: Q > 1/2, f > 0, finite Rs required"; break; }
+                        // G12, same expressions as the definition, evaluated once here
+                        const double wr = kTwoPi * e.f;
+                        ResConst rc;
+                        rc.kloss = wr * e.Rs / (2.0 * e.Q);
+                        rc.alpha = wr / (2.0 * e.Q);
+                        rc.wbar = std::sqrt(wr * wr - rc.alpha * rc.alpha);
+                        rc.ratio = rc.alpha / rc.wbar;
+                        bl->res[k] = rc;
+                    } else if (e.wake == ELG_WAKE_TABLE) {
+                        if (!e.table || e.n_table < 1 || !(e.dt_table > 0.0)) { why = "table wake: table, n_table >= 1, dt_table > 0 required"; break; }
+                        bl->table[k].assign(e.table, e.table + e.n_table); e.table = bl->table[k].data();
+                        bl->table_off[k] = bl->table_total;
+                        bl->table_total += e.n_table;
+                    } else { why = "WAKE: bad wake kind"; break; }
+                    if (e.window == ELG_WIN_AUTO_TABLE && e.wake != ELG_WAKE_TABLE) why = "AUTO_TABLE window needs a table wake";
+                }
+                break;
+            default: why = "unknown element type";
+        }
+        if (why) {
+            char buf[160];
+            std::snprintf(buf, sizeof buf, "elg_beamline_load: element %lld: %s", (long long)k, why);
+            delete bl;
+            return fail(ELG_EINVAL, buf);
+        }
+    }
+    bl->s_design[n_elems] = s;
+    bl->length = s;
+    *out = bl;
+    return ELG_OK;
+}
+extern "C" void elg_beamline_destroy(elg_beamline* bl) { delete bl; }
+extern "C" int64_t elg_beamline_n_elements(const elg_beamline* bl) { return bl ? (int64_t)bl->e.size() : 0; }
+extern "C" double elg_beamline_length(const elg_beamline* bl) { return bl ? bl->length : 0.0; }
+extern "C" double elg_beamline_s_design(const elg_beamline* bl, int64_t k) {
+    if (!bl || k < 0 || k > (int64_t)bl->e.size()) return NAN;
+    return bl->s_design[k];
+}
+
+// ------------------------------------------------------------------------------------- bunch
+extern "C" int32_t elg_workspace_bytes(int64_t n0, const elg_beamline* bl, int64_t lost_capacity, int64_t* bytes) {
+    if (n0 < 0 || lost_capacity < 0 || !bytes) return fail(ELG_EINVAL, "elg_workspace_bytes: bad arguments");
+    long long nb_cap, table_cap;
+    caps_for(bl, &nb_cap, &table_cap);
+    *bytes = layout(n0, nb_cap, table_cap, lost_capacity).total;
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_bunch_rewind(elg_bunch* b) {
+    if (!b) return fail(ELG_EINVAL, "elg_bunch_rewind: NULL bunch");
+    init_state_kernel<<<1, 1, 0, b->stream>>>(b->st, b->n0);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    b->cur_buf = 0; b->cur_slot = 0; b->turn = 0; b->rec_count = 0;
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, void* d_work, int64_t work_bytes,
+                                    const elg_beamline* sized_for, int64_t lost_capacity, double p0c, double mc2, double charge, void* stream) {
+    if (!out || n0 < 0 || n0 >= (1LL << 31) || !d_soa || !d_work || lost_capacity < 0 || !(p0c > 0.0) || !(mc2 > 0.0))
+        return fail(ELG_EINVAL, "elg_bunch_create: bad arguments (0 <= n0 < 2^31, non-NULL buffers, p0c, mc2 > 0)");
+    if (((uintptr_t)d_soa & 255) || ((uintptr_t)d_work & 255))
+        return fail(ELG_EINVAL, "elg_bunch_create: d_soa and d_work must be 256-byte aligned");
+    long long nb_cap, table_cap;
+    caps_for(sized_for, &nb_cap, &table_cap);
+    const WorkLayout L = layout(n0, nb_cap, table_cap, lost_capacity);
+    if (work_bytes < L.total) return fail(ELG_ECAPACITY, "elg_bunch_create: workspace smaller than elg_workspace_bytes");
+    int sms = 0;
+    { int32_t rc = device_sms(&sms); if (rc != ELG_OK) return rc; }
+    elg_bunch* b = new (std::nothrow) elg_bunch;
+    if (!b) return fail(ELG_ENOMEM, "elg_bunch_create: out of host memory");
+    b->n0 = n0; b->stride = elg_soa_stride(n0); b->lost_cap = lost_capacity; b->work_bytes = work_bytes;
+    b->d_soa = (char*)d_soa; b->d_work = (char*)d_work; b->stream = (cudaStream_t)stream;
+    b->p0c = p0c; b->mc2 = mc2; b->charge = charge;
+    {   // G7, G9, G30: unfused, in this order
+        const double e2 = p0c * p0c + mc2 * mc2;
+        b->beta0 = p0c / std::sqrt(e2);
+        b->inv_bc = 1.0 / (b->beta0 * kCLight);
+        b->inv_E = 1.0 / (b->beta0 * p0c);
+        b->q_macro = (n0 > 0) ? charge / (double)n0 : 0.0;     // G15
+    }
+    b->nb_cap = nb_cap; b->table_cap = table_cap;
+    char* w = b->d_work;
+    b->st = (DevState*)(w + L.off_state);
+    b->soaB = w + L.off_soaB;
+    b->tile_status = (unsigned long long*)(w + L.off_status);
+    b->mm_partial = (double*)(w + L.off_mm);
+    b->mom_partial = (double*)(w + L.off_mom);
+    b->records = (double*)(w + L.off_rec);
+    b->counts = (unsigned int*)(w + L.off_counts);
+    b->W = (double*)(w + L.off_W);
+    b->V = (double*)(w + L.off_V);
+    b->table = (double*)(w + L.off_table);
+    b->lost_id = (long long*)(w + L.off_lost_id);
+    b->lost_te = (long long*)(w + L.off_lost_te);
+    b->lost_v = (double*)(w + L.off_lost_v);
+    b->sms = sms;
+    int32_t rc = ELG_OK;
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, false>, sms, 0, &b->grid_chain[0][0]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, true>, sms, 0, &b->grid_chain[0][1]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsLarge, false>, sms, 0, &b->grid_chain[1][0]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsLarge, true>, sms, 0, &b->grid_chain[1][1]);
+    if (rc == ELG_OK) rc = hist_setup_once();
+    if (rc == ELG_OK) rc = grid_for(hist_kernel, sms, kHistSmemBins * 4, &b->grid_hist);
+    if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, &b->grid_mom);
+    if (rc != ELG_OK) { delete b; return rc; }
+    const char* agg = std::getenv("ELG_HIST_AGGREGATE");
+    b->hist_aggregate = agg ? std::atoi(agg) : -1;                 // -1: automatic
+    cudaError_t ce = cudaMemsetAsync(b->tile_status, 0, (b->stride / kTile + 2) * 8, b->stream);
+    if (ce != cudaSuccess) { delete b; return fail(ELG_ECUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(ce)); }
+    rc = elg_bunch_rewind(b);
+    if (rc != ELG_OK) { delete b; return rc; }
+    *out = b;
+    return ELG_OK;
+}
+extern "C" void elg_bunch_destroy(elg_bunch* b) {
+    if (b) cudaStreamSynchronize(b->stream);
+    delete b;
+}
+
+extern "C" int32_t elg_bunch_upload(elg_bunch* b, const double* const h_coords[6], const int64_t* h_ids) {
+    if (!b || !h_coords) return fail(ELG_EINVAL, "elg_bunch_upload: bad arguments");
+    for (int c = 0; c < 6; c++) {
+        if (!h_coords[c]) return fail(ELG_EINVAL, "elg_bunch_upload: NULL coordinate array");
+        ELG_CK(cudaMemcpyAsync(b->coord(0, c), h_coords[c], b->n0 * 8, cudaMemcpyHostToDevice, b->stream));
+    }
+    if (h_ids) ELG_CK(cudaMemcpyAsync(b->ids(0), h_ids, b->n0 * 8, cudaMemcpyHostToDevice, b->stream));
+    else if (b->n0 > 0) {
+        iota_kernel<<<b->sms * 4, kBlock, 0, b->stream>>>(b->ids(0), b->n0);
+        g_launches++;
+        ELG_CK(cudaGetLastError());
+    }
+    return elg_bunch_rewind(b);
+}
+
+// =====================================================================================================
+// Tracking: the beamline is cut into fused runs (north_star part 1).  Maps accumulate in a pending list
+// and are launched as ONE chain kernel when something needs the particles in memory: an aperture (which
+// becomes the run's terminator and compacts), a WAKE/HISTO (needs min/max of s: fused epilogue), a
+// moments record, more ops than one parameter block holds, or the end of the call.  The wake kick is
+// not a pass of its own: it is queued as the first op of the next run.
+// With b == nullptr the planner only counts launches (elg_beamline_launches_per_turn; CPU-testable).
+// =====================================================================================================
+namespace {
+
+struct Tracker {
+    elg_bunch* b;
+    const elg_beamline* bl;
+    elg_track_opts* o;
+    std::vector<HostOp> pending;
+    int kick_nb = 0, kick_interp = 0;
+    bool mm_valid = false;
+    long long launches = 0;
+    int32_t rc = ELG_OK;
+    long long rec_total = 0;       // records taken in this call
+    long long rec_flushed = 0;     // of which already copied to the host
+    int mm_grid = 0;               // blocks of the launch that produced the current min/max partials
+
+    bool ok() const { return rc == ELG_OK; }
+    void count() { launches++; if (b) g_launches++; }
+    void check(cudaError_t e, const char* what) {
+        if (e != cudaSuccess && rc == ELG_OK) rc = fail(ELG_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    }
+
+    template <int MAXOPS, bool COMPACT>
+    void launch_chain(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm, unsigned rmask, unsigned wmask) {
+        count();
+        if (!b) return;
+        ChainArgs<MAXOPS> a;
+        ChainCommon& c = a.c;
+        const int src = b->cur_buf, dst = COMPACT ? (b->cur_buf ^ 1) : b->cur_buf;
+        for (int k = 0; k < 6; k++) { c.src[k] = b->coord(src, k); c.dst[k] = b->coord(dst, k); }
+        c.id_src = b->ids(src); c.id_dst = b->ids(dst);
+        c.st = b->st; c.cur = b->cur_slot; c.n_ops = (int)pending.size();
+        c.rmask = rmask; c.wmask = wmask;
+        c.ap_type = ap_type; c.ap_x = ap_x; c.ap_y = ap_y;
+        c.lost_id = b->lost_id; c.lost_te = b->lost_te; c.lost_v = b->lost_v; c.lost_cap = b->lost_cap; c.te_code = te_code;
+        c.tile_status = b->tile_status;
+        if (COMPACT) b->epoch = (b->epoch + 1) & 0x3fffffffu;
+        if (COMPACT && b->epoch == 0) {                               // epoch wrapped: stale tags could alias
+            check(cudaMemsetAsync(b->tile_status, 0, (b->stride / kTile + 2) * 8, b->stream), "cudaMemsetAsync");
+            b->epoch = 1;
+        }
+        c.epoch = b->epoch;
+        c.want_minmax = want_mm ? 1 : 0; c.mm_partial = b->mm_partial;
+        c.V = b->V; c.nb = kick_nb; c.interp = kick_interp;
+        for (size_t k = 0; k < pending.size(); k++) {
+            a.type[k] = pending[k].type;
+            std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
+        }
+        const int grid = b->grid_chain[MAXOPS == kMaxOpsLarge ? 1 : 0][COMPACT ? 1 : 0];
+        if (want_mm) mm_grid = grid;
+        chain_kernel<MAXOPS, COMPACT><<<grid, kBlock, 0, b->stream>>>(a);
+        check(cudaGetLastError(), "chain_kernel launch");
+        if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
+    }
+
+    // launch the pending maps (+ aperture terminator, + min/max epilogue)
+    void flush(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm) {
+        if (!ok()) return;
+        if (ap_type == AP_NONE && pending.empty() && !want_mm) return;
+        unsigned rmask = 0, wmask = 0;
+        for (const HostOp& op : pending) {
+            switch (op.type) {
+                case OP_DRIFT: rmask |= 0x1F; wmask |= 0x15; break;           // reads x x' y y' s, writes x y s
+                case OP_MATRIX: rmask |= 0x3F; wmask |= 0x3F; break;
+                case OP_RFKICK: case OP_KICK: rmask |= 0x30; wmask |= 0x20; break;   // reads s delta, writes delta
+            }
+        }
+        if (want_mm) rmask |= 0x10;
+        const bool large = pending.size() > (size_t)kMaxOpsSmall;
+        const bool compact = ap_type != AP_NONE;
+        if (large) { if (compact) launch_chain<kMaxOpsLarge, true>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask);
+                     else launch_chain<kMaxOpsLarge, false>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask); }
+        else       { if (compact) launch_chain<kMaxOpsSmall, true>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask);
+                     else launch_chain<kMaxOpsSmall, false>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask); }
+        if (compact || (wmask & 0x10)) mm_valid = want_mm;
+        else mm_valid = mm_valid || want_mm;
+        pending.clear();
+    }
+
+    void push(const HostOp& op) {
+        if (pending.size() == (size_t)kMaxOpsLarge) flush(AP_NONE, 0, 0, 0, false);
+        pending.push_back(op);
+    }
+
+    void moments_record() {
+        flush(AP_NONE, 0, 0, 0, false);
+        if (!ok()) return;
+        count();
+        rec_total++;
+        if (!b) return;
+        if (b->rec_count == kRecCap) flush_records();
+        MomArgs m;
+        for (int k = 0; k < 6; k++) m.src[k] = b->coord(b->cur_buf, k);
+        m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial;
+        m.record = b->records + 43 * b->rec_count;
+        moments_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(m);
+        check(cudaGetLastError(), "moments_kernel launch");
+        b->rec_count++;
+    }
+
+    void flush_records() {             // device ring -> host (drops what does not fit)
+        if (!b || b->rec_count == 0) return;
+        if (o && o->records) {
+            long long room = o->capacity_records - rec_flushed;
+            long long m = b->rec_count < room ? b->rec_count : room;
+            if (m > 0) check(cudaMemcpyAsync(o->records + 43 * rec_flushed, b->records, m * 43 * 8, cudaMemcpyDeviceToHost, b->stream), "records D2H");
+            check(cudaStreamSynchronize(b->stream), "cudaStreamSynchronize");
+        }
+        rec_flushed += b->rec_count;
+        b->rec_count = 0;
+    }
+
+    void wake_or_histo(long long k, double s_here) {
+        const elg_element& e = bl->e[k];
+        bool writes_s = false;
+        for (const HostOp& op : pending) writes_s = writes_s || op.type == OP_DRIFT || op.type == OP_MATRIX;
+        const bool need_mm = !mm_valid || writes_s;
+        if (!pending.empty() || need_mm) flush(AP_NONE, 0, 0, 0, need_mm);
+        if (!ok()) return;
+        count();                                                      // window
+        count();                                                      // histogram
+        if (b) {
+            if (e.nb > b->nb_cap) { rc = fail(ELG_ECAPACITY, "elg_track: workspace was sized for fewer bins than this beamline needs"); return; }
+            WindowArgs w;
+            w.st = b->st; w.cur = b->cur_slot; w.mm_partial = b->mm_partial; w.n_partial = mm_grid;
+            w.mode = e.window; w.nb = e.nb; w.t_lo_rel = e.t_lo_rel;
+            w.dt_in = (e.window == ELG_WIN_AUTO_TABLE) ? e.dt_table : e.dt;
+            w.t_design = s_here * b->inv_bc; w.inv_bc = b->inv_bc; w.counts = b->counts;
+            window_kernel<<<1, kBlock, 0, b->stream>>>(w);
+            check(cudaGetLastError(), "window_kernel launch");
+            HistArgs h;
+            h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1;
+            h.inv_bc = b->inv_bc; h.t_lo = 0; h.inv_dt = 0; h.nb = e.nb; h.counts = b->counts;
+            h.aggregate = b->hist_aggregate < 0 ? 0 : b->hist_aggregate;
+            hist_kernel<<<b->grid_hist, kBlock, kHistSmemBins * 4, b->stream>>>(h);
+            check(cudaGetLastError(), "hist_kernel launch");
+            stage_out_hist(e.nb);
+        } else if (o) { o->window_written++; o->hist_written += e.nb; }
+        if (e.type != ELG_WAKE) return;
+        count();                                                      // wake samples
+        count();                                                      // convolution
+        if (b) {
+            WakeArgs wa;
+            wa.st = b->st; wa.dt_fixed = 0.0; wa.kind = e.wake; wa.nb = e.nb;
+            const ResConst& r = bl->res[k];
+            wa.kloss = r.kloss; wa.alpha = r.alpha; wa.wbar = r.wbar; wa.ratio = r.ratio;
+            wa.table = b->table + bl->table_off[k]; wa.n_table = e.n_table; wa.dt_table = e.dt_table; wa.W = b->W;
+            wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
+            check(cudaGetLastError(), "wake_samples_kernel launch");
+            ConvArgs cv;
+            cv.counts = b->counts; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro; cv.V = b->V;
+            conv_kernel<<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
+            check(cudaGetLastError(), "conv_kernel launch");
+            if (o && o->V_out && o->V_written + e.nb <= o->V_capacity)
+                check(cudaMemcpyAsync(o->V_out + o->V_written, b->V, (size_t)e.nb * 8, cudaMemcpyDeviceToHost, b->stream), "V D2H");
+        }
+        if (o) o->V_written += e.nb;
+        HostOp op{};
+        op.type = OP_KICK;
+        op.coef[0] = b ? b->inv_bc : 0.0; op.coef[1] = b ? b->inv_E : 0.0;
+        pending.push_back(op);
+        kick_nb = e.nb; kick_interp = e.interp;
+    }
+
+    void stage_out_hist(int nb) {
+        if (!o) return;
+        if (o->window_out && o->window_written < o->window_capacity)
+            check(cudaMemcpyAsync(o->window_out + 3 * o->window_written, b->st->win, 24, cudaMemcpyDeviceToHost, b->stream), "window D2H");
+        o->window_written++;
+        if (o->hist_out && o->hist_written + nb <= o->hist_capacity)
+            check(cudaMemcpyAsync(o->hist_out + o->hist_written, b->counts, (size_t)nb * 4, cudaMemcpyDeviceToHost, b->stream), "hist D2H");
+        o->hist_written += nb;
+    }
+
+    void run_turn(long long turn) {
+        const long long ne = (long long)bl->e.size();
+        const int mom = o ? o->moments_every : ELG_MOM_NONE;
+        for (long long k = 0; k < ne && ok(); k++) {
+            const elg_element& e = bl->e[k];
+            const double s_here = std::fma((double)turn, bl->length, bl->s_design[k]);      // G8
+            HostOp op{};
+            switch (e.type) {
+                case ELG_DRIFT: op.type = OP_DRIFT; op.coef[0] = e.L; push(op); break;
+                case ELG_MATRIX:
+                    op.type = OP_MATRIX;
+                    std::memcpy(op.coef, e.R, 36 * sizeof(double));
+                    if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
+                    push(op);
+                    break;
+                case ELG_RFKICK:
+                    op.type = OP_RFKICK;
+                    op.coef[0] = e.V * (b ? b->inv_E : 0.0); op.coef[1] = kTwoPi * e.f; op.coef[2] = e.phi;
+                    op.coef[3] = s_here; op.coef[4] = b ? b->inv_bc : 0.0;
+                    push(op);
+                    break;
+                case ELG_RCOL: case ELG_ECOL: {
+                    const bool rect = e.type == ELG_RCOL;                    // ECOL carries 1/a, 1/b (G17)
+                    flush(rect ? AP_RCOL : AP_ECOL, rect ? e.ax : 1.0 / e.ax, rect ? e.ay : 1.0 / e.ay,
+                          (turn << 32) | k, next_is_hist(k, ne));
+                    break;
+                }
+                case ELG_WAKE: case ELG_HISTO: wake_or_histo(k, s_here); break;
+            }
+            if (mom == ELG_MOM_ELEMENT) moments_record();                                    // G26
+        }
+        if (mom == ELG_MOM_TURN) moments_record();
+    }
+    bool next_is_hist(long long k, long long ne) const {
+        return (k + 1 < ne) && (bl->e[k + 1].type == ELG_WAKE || bl->e[k + 1].type == ELG_HISTO);
+    }
+};
+
+int32_t upload_tables(elg_bunch* b, const elg_beamline* bl) {
+    if (b->table_serial == bl->serial) return ELG_OK;
+    if (bl->table_total > b->table_cap) return fail(ELG_ECAPACITY, "elg_track: workspace was sized for smaller wake tables");
+    for (size_t k = 0; k < bl->e.size(); k++)
+        if (!bl->table[k].empty())
+            ELG_CK(cudaMemcpyAsync(b->table + bl->table_off[k], bl->table[k].data(), bl->table[k].size() * 8,
+                                   cudaMemcpyHostToDevice, b->stream));
+    b->table_serial = bl->serial;
+    return ELG_OK;
+}
+
+}  // namespace
+
+extern "C" int64_t elg_beamline_launches_per_turn(const elg_beamline* bl, int32_t moments_every) {
+    if (!bl) return -1;
+    elg_track_opts o{};
+    o.moments_every = moments_every;
+    Tracker t{nullptr, bl, &o};
+    t.run_turn(0);
+    t.flush(AP_NONE, 0, 0, 0, false);
+    return t.launches;
+}
+
+extern "C" int32_t elg_track(elg_bunch* b, const elg_beamline* bl, int64_t n_turns, elg_track_opts* o) {
+    if (!b || !bl || n_turns < 0) return fail(ELG_EINVAL, "elg_track: bad arguments");
+    if (o) { o->n_records = 0; o->hist_written = 0; o->V_written = 0; o->window_written = 0; }
+    { int32_t rc = upload_tables(b, bl); if (rc != ELG_OK) return rc; }
+    Tracker t{b, bl, o};
+    b->rec_count = 0;
+    for (int64_t it = 0; it < n_turns && t.ok(); it++) {
+        t.run_turn(b->turn);
+        b->turn++;
+    }
+    t.flush(AP_NONE, 0, 0, 0, false);
+    if (t.ok()) t.flush_records();
+    if (o) o->n_records = t.rec_total;
+    if (t.ok() && o && (o->records || o->hist_out || o->V_out || o->window_out)) {
+        cudaError_t e = cudaStreamSynchronize(b->stream);
+        if (e != cudaSuccess) return fail(ELG_ECUDA, std::string("cudaStreamSynchronize: ") + cudaGetErrorString(e));
+    }
+    return t.rc;
+}
+
+// ------------------------------------------------------------------------------------- host readbacks
+extern "C" int32_t elg_n_alive(elg_bunch* b, int64_t* n_alive) {
+    if (!b || !n_alive) return fail(ELG_EINVAL, "elg_n_alive: bad arguments");
+    long long n = 0;
+    ELG_CK(cudaMemcpyAsync(&n, &b->st->n_alive[b->cur_slot], 8, cudaMemcpyDeviceToHost, b->stream));
+    ELG_CK(cudaStreamSynchronize(b->stream));
+    *n_alive = n;
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_moments(elg_bunch* b, int64_t* n_alive, double h_centroid[6], double h_sigma[36]) {
+    if (!b) return fail(ELG_EINVAL, "elg_moments: NULL bunch");
+    MomArgs m;
+    for (int k = 0; k < 6; k++) m.src[k] = b->coord(b->cur_buf, k);
+    m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial;
+    m.record = b->records + 43 * kRecCap;
+    moments_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(m);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    double rec[43];
+    ELG_CK(cudaMemcpyAsync(rec, m.record, sizeof rec, cudaMemcpyDeviceToHost, b->stream));
+    ELG_CK(cudaStreamSynchronize(b->stream));
+    if (n_alive) *n_alive = (int64_t)rec[0];
+    if (rec[0] <= 0.0) return fail(ELG_ESTATE, "elg_moments: no live particles");
+    if (h_centroid) std::memcpy(h_centroid, rec + 1, 6 * sizeof(double));
+    if (h_sigma) std::memcpy(h_sigma, rec + 7, 36 * sizeof(double));
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_bunch_read(elg_bunch* b, double* const h_coords[6], int64_t* h_ids, int64_t cap) {
+    if (!b) return fail(ELG_EINVAL, "elg_bunch_read: NULL bunch");
+    int64_t n = 0;
+    { int32_t rc = elg_n_alive(b, &n); if (rc != ELG_OK) return rc; }
+    if (cap < n) return fail(ELG_ECAPACITY, "elg_bunch_read: capacity smaller than n_alive");
+    if (n > 0) {
+        for (int c = 0; c < 6; c++)
+            if (h_coords && h_coords[c])
+                ELG_CK(cudaMemcpyAsync(h_coords[c], b->coord(b->cur_buf, c), n * 8, cudaMemcpyDeviceToHost, b->stream));
+        if (h_ids) ELG_CK(cudaMemcpyAsync(h_ids, b->ids(b->cur_buf), n * 8, cudaMemcpyDeviceToHost, b->stream));
+        ELG_CK(cudaStreamSynchronize(b->stream));
+    }
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_lost(elg_bunch* b, int64_t* n_lost, int64_t cap, int64_t* h_ids, int32_t* h_turn, int32_t* h_elem,
+                            double* h_coords6) {
+    if (!b || cap < 0) return fail(ELG_EINVAL, "elg_lost: bad arguments");
+    long long nl = 0;
+    ELG_CK(cudaMemcpyAsync(&nl, &b->st->n_lost[b->cur_slot], 8, cudaMemcpyDeviceToHost, b->stream));
+    ELG_CK(cudaStreamSynchronize(b->stream));
+    if (n_lost) *n_lost = nl;
+    long long have = nl < b->lost_cap ? nl : b->lost_cap;           // records kept on the device
+    long long m = have < cap ? have : cap;
+    if (m > 0) {
+        if (h_ids) ELG_CK(cudaMemcpyAsync(h_ids, b->lost_id, m * 8, cudaMemcpyDeviceToHost, b->stream));
+        std::vector<long long> te;
+        if (h_turn || h_elem) {
+            te.resize(m);
+            ELG_CK(cudaMemcpyAsync(te.data(), b->lost_te, m * 8, cudaMemcpyDeviceToHost, b->stream));
+        }
+        std::vector<double> tmp;
+        if (h_coords6) {
+            tmp.resize(6 * m);
+            for (int c = 0; c < 6; c++)
+                ELG_CK(cudaMemcpyAsync(tmp.data() + c * m, b->lost_v + c * b->lost_cap, m * 8, cudaMemcpyDeviceToHost, b->stream));
+        }
+        ELG_CK(cudaStreamSynchronize(b->stream));
+        for (long long j = 0; j < m; j++) {
+            if (h_turn) h_turn[j] = (int32_t)(te[j] >> 32);
+            if (h_elem) h_elem[j] = (int32_t)(te[j] & 0xffffffffLL);
+            if (h_coords6) for (int c = 0; c < 6; c++) h_coords6[6 * j + c] = tmp[c * m + j];   // layout only
+        }
+    }
+    if (cap < nl) return fail(ELG_ECAPACITY, "elg_lost: more lost particles than capacity");
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_bunch_device_array(elg_bunch* b, int32_t c, void** d_ptr) {
+    if (!b || !d_ptr || c < 0 || c > 6) return fail(ELG_EINVAL, "elg_bunch_device_array: bad arguments");
+    *d_ptr = (c < 6) ? (void*)b->coord(b->cur_buf, c) : (void*)b->ids(b->cur_buf);
+    return ELG_OK;
+}
+
+// ------------------------------------------------------------------------------------- test hooks
+namespace {
+int32_t hook_grid(int* grid, int per_sm) {
+    int sms = 0;
+    int32_t rc = device_sms(&sms);
+    if (rc != ELG_OK) return rc;
+    *grid = sms * per_sm;
+    return ELG_OK;
+}
+}  // namespace
+
+extern "C" int32_t elg_dbg_histogram(const double* d_s, int64_t n, double inv_bc, double t_lo, double inv_dt, int32_t nb,
+                                     uint32_t* d_counts, void* stream) {
+    if (n < 0 || nb < 1 || !d_counts || (n > 0 && !d_s)) return fail(ELG_EINVAL, "elg_dbg_histogram: bad arguments");
+    int grid = 0;
+    { int32_t rc = hist_setup_once(); if (rc != ELG_OK) return rc; }
+    { int32_t rc = grid_for(hist_kernel, 1, kHistSmemBins * 4, &grid); if (rc != ELG_OK) return rc; }
+    int sms = 0;
+    { int32_t rc = device_sms(&sms); if (rc != ELG_OK) return rc; }
+    ELG_CK(cudaMemsetAsync(d_counts, 0, (size_t)nb * 4, (cudaStream_t)stream));
+    HistArgs h;
+    h.s = d_s; h.st = nullptr; h.cur = 0; h.n_fixed = n; h.inv_bc = inv_bc; h.t_lo = t_lo; h.inv_dt = inv_dt; h.nb = nb;
+    const char* agg = std::getenv("ELG_HIST_AGGREGATE");
+    h.aggregate = agg ? std::atoi(agg) : 0;
+    h.counts = d_counts;
+    hist_kernel<<<grid * sms, kBlock, kHistSmemBins * 4, (cudaStream_t)stream>>>(h);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_dbg_wake_samples(int32_t kind, int32_t nb, double dt, double f, double Q, double Rs,
+                                        const double* d_table, int64_t n_table, double dt_table, double* d_W, void* stream) {
+    if (nb < 1 || !d_W || !(dt > 0.0)) return fail(ELG_EINVAL, "elg_dbg_wake_samples: bad arguments");
+    WakeArgs wa{};
+    wa.st = nullptr; wa.dt_fixed = dt; wa.kind = kind; wa.nb = nb;
+    if (kind == ELG_WAKE_RESONATOR) {
+        if (!(Q > 0.5)) return fail(ELG_EINVAL, "elg_dbg_wake_samples: Q <= 1/2");
+        const double wr = kTwoPi * f;
+        wa.kloss = wr * Rs / (2.0 * Q);
+        wa.alpha = wr / (2.0 * Q);
+        wa.wbar = std::sqrt(wr * wr - wa.alpha * wa.alpha);
+        wa.ratio = wa.alpha / wa.wbar;
+    } else if (kind == ELG_WAKE_TABLE) {
+        if (!d_table || n_table < 1 || !(dt_table > 0.0)) return fail(ELG_EINVAL, "elg_dbg_wake_samples: bad table");
+    } else return fail(ELG_EINVAL, "elg_dbg_wake_samples: bad kind");
+    wa.table = d_table; wa.n_table = n_table; wa.dt_table = dt_table; wa.W = d_W;
+    wake_samples_kernel<<<(nb + kBlock - 1) / kBlock, kBlock, 0, (cudaStream_t)stream>>>(wa);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W, int32_t nb, double q, double* d_V,
+                                    void* stream) {
+    if (nb < 1 || !d_counts || !d_W || !d_V) return fail(ELG_EINVAL, "elg_dbg_convolve: bad arguments");
+    ConvArgs cv;
+    cv.counts = d_counts; cv.W = d_W; cv.st = nullptr; cv.nb = nb; cv.q = q; cv.V = d_V;
+    conv_kernel<<<(nb + kWarps - 1) / kWarps, kBlock, 0, (cudaStream_t)stream>>>(cv);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_dbg_kick(const double* d_s, double* d_delta, int64_t n, double inv_bc, double t_lo, double inv_dt,
+                                int32_t nb, const double* d_V, double inv_E, int32_t interp, void* stream) {
+    if (n < 0 || nb < 1 || !d_V || (n > 0 && (!d_s || !d_delta))) return fail(ELG_EINVAL, "elg_dbg_kick: bad arguments");
+    int grid = 0;
+    { int32_t rc = hook_grid(&grid, 8); if (rc != ELG_OK) return rc; }
+    kick_kernel<<<grid, kBlock, 0, (cudaStream_t)stream>>>(d_s, d_delta, n, inv_bc, t_lo, inv_dt, nb, d_V, inv_E, interp);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    return ELG_OK;
+}

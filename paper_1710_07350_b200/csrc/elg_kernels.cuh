@@ -1,0 +1,743 @@
+// elg_kernels.cuh -- device code of libelg (sm_100a).  Hand-written CUDA; no code shared with oracle/.
+//
+// Arithmetic specification: every per-particle map is written with explicit
+// fma() in a fixed order and the file is compiled with -fmad=false, so nothing else is contracted.
+// IEEE fma / sqrt / div are correctly rounded on the device, hence DRIFT, MATRIX, aperture predicates,
+// window and bin indices are bit-reproducible; only sin/cos/exp (<= 2 ulp) and summation order differ
+// from a sequential CPU evaluation.
+//
+// Kernels (one section each):
+//   chain_kernel<MAXOPS, COMPACT>  fused run of element maps; COMPACT ends in an aperture and a stable
+//                                  single-pass (decoupled look-back) stream compaction
+//   window_kernel                  min/max partials -> histogram window + occupied bin range, zero counts
+//   hist_kernel                    shared-memory privatised time histogram
+//   wake_samples_kernel, conv_kernel   wake function samples and causal convolution
+//   moments_kernel                 shifted one-pass deterministic fp64 tree reduction (27 sums)
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace elg {
+
+constexpr int kBlock = 256;            // threads per block
+constexpr int kWarps = kBlock / 32;
+constexpr int kP = 2;                  // particles per thread = one 128-bit access per coordinate
+constexpr int kTile = kBlock * kP;     // particles per tile
+constexpr int kHistSmemBins = 16384;   // 64 KB of privatised bins per block
+constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
+
+enum : uint8_t { OP_DRIFT = 1, OP_MATRIX = 2, OP_RFKICK = 3, OP_KICK = 4 };
+enum { AP_NONE = 0, AP_RCOL = 1, AP_ECOL = 2 };
+
+// Device-resident tracking state (first bytes of the workspace).  Nothing here is read by the host
+// during elg_track: n_alive never crosses PCIe on the hot path (the paper syncs per lossy element,
+// PAPER.md:141 step 2).
+struct DevState {
+    long long n_alive[2];      // ping-pong: a compaction reads slot cur, writes slot cur^1
+    long long n_lost[2];
+    double win[4];             // t_lo, dt, inv_dt, -
+    double smin, smax;         // exact min / max of s over live particles
+    long long bin_lo, bin_hi;  // occupied bin range (clamped to [0, nb-1]); bin_lo > bin_hi: nothing binned
+    unsigned int tile_counter; // dynamic tile ids for the look-back scan
+    unsigned int done_counter;
+    unsigned int mom_done;
+    unsigned int pad;
+};
+
+struct ChainCommon {
+    double* src[6];
+    double* dst[6];
+    long long* id_src;
+    long long* id_dst;
+    DevState* st;
+    int cur;                   // n_alive / n_lost slot to read
+    int n_ops;
+    unsigned int rmask, wmask; // coordinates loaded / stored (accessor rule)
+    int ap_type;               // AP_*
+    double ap_x, ap_y;         // RCOL: ax, ay.  ECOL: 1/a, 1/b
+    long long* lost_id;        // lost log (SoA, capacity lost_cap)
+    long long* lost_te;        // turn << 32 | element
+    double* lost_v;            // 6 arrays at stride lost_cap
+    long long lost_cap;
+    long long te_code;
+    unsigned long long* tile_status;
+    unsigned int epoch;
+    int want_minmax;
+    double* mm_partial;        // [2 * gridDim.x]
+    const double* V;           // OP_KICK operands
+    int nb;
+    int interp;
+};
+
+template <int MAXOPS>
+struct ChainArgs {
+    ChainCommon c;
+    uint8_t type[MAXOPS];
+    double coef[MAXOPS][42];   // MATRIX: R[36], C[6].  DRIFT: L.  RFKICK: A, omega, phi0, s_ref, inv_bc.
+                               // KICK: inv_bc, inv_E
+};
+
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// streaming 128-bit accesses: every particle is touched once per launch, keep L1 for the tables
+__device__ __forceinline__ double2 ld_stream2(const double* p) {
+    double2 r;
+    asm volatile("ld.global.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ double ld_stream1(const double* p) {
+    double r;
+    asm volatile("ld.global.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
+    return r;
+}
+
+// bin of a time coordinate (G10): floor((s*inv_bc - t_lo)*inv_dt) in [0, nb) else -1
+__device__ __forceinline__ int bin_of(double s, double inv_bc, double t_lo, double inv_dt, int nb, double* u_out) {
+    const double t = s * inv_bc;
+    const double u = (t - t_lo) * inv_dt;
+    const double fl = floor(u);
+    *u_out = u;
+    if (!(fl >= 0.0) || !(fl < (double)nb)) return -1;
+    return (int)fl;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Element maps on kP particles held in registers.  Coefficients come straight from the kernel parameter
+// constant bank (uniform operands of DFMA), so a MATRIX costs 42 DFMA per particle and no LSU traffic.
+// ---------------------------------------------------------------------------------------------------
+template <int MAXOPS>
+__device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v)[kP][6]) {
+    for (int op = 0; op < a.c.n_ops; op++) {
+        const double* c = a.coef[op];
+        const int ty = a.type[op];
+        if (ty == OP_MATRIX) {                                   // G3
+            double w[kP][6];
+#pragma unroll
+            for (int r = 0; r < 6; r++) {
+#pragma unroll
+                for (int p = 0; p < kP; p++) {
+                    double acc = c[36 + r];
+#pragma unroll
+                    for (int cc = 0; cc < 6; cc++) acc = fma(c[6 * r + cc], v[p][cc], acc);
+                    w[p][r] = acc;
+                }
+            }
+#pragma unroll
+            for (int p = 0; p < kP; p++)
+#pragma unroll
+                for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+        } else if (ty == OP_DRIFT) {                             // PAPER.md:75-77, G2
+            const double L = c[0];
+#pragma unroll
+            for (int p = 0; p < kP; p++) {
+                v[p][0] = fma(v[p][1], L, v[p][0]);
+                v[p][2] = fma(v[p][3], L, v[p][2]);
+                double u = fma(v[p][1], v[p][1], 1.0);
+                u = fma(v[p][3], v[p][3], u);
+                v[p][4] = fma(L, sqrt(u), v[p][4]);
+            }
+        } else if (ty == OP_RFKICK) {                            // G8
+            const double A = c[0], omega = c[1], phi0 = c[2], s_ref = c[3], inv_bc = c[4];
+#pragma unroll
+            for (int p = 0; p < kP; p++) {
+                const double tau = (v[p][4] - s_ref) * inv_bc;
+                const double arg = fma(omega, tau, phi0);
+                v[p][5] = fma(A, sin(arg), v[p][5]);
+            }
+        } else if (ty == OP_KICK) {                              // G14: wake kick of the preceding WAKE
+            const double inv_bc = c[0], inv_E = c[1];
+            const double t_lo = a.c.st->win[0], inv_dt = a.c.st->win[2];
+            const int nb = a.c.nb;
+#pragma unroll
+            for (int p = 0; p < kP; p++) {
+                double u0;
+                const int b = bin_of(v[p][4], inv_bc, t_lo, inv_dt, nb, &u0);
+                if (b < 0) continue;
+                double Vt;
+                if (!a.c.interp || nb < 2) {
+                    Vt = __ldg(a.c.V + b);
+                } else {
+                    const double u = u0 - 0.5;
+                    double k = floor(u);
+                    if (k < 0.0) k = 0.0;
+                    if (k > (double)(nb - 2)) k = (double)(nb - 2);
+                    double fr = u - k;
+                    if (fr < 0.0) fr = 0.0;
+                    if (fr > 1.0) fr = 1.0;
+                    const int ki = (int)k;
+                    const double V0 = __ldg(a.c.V + ki), V1 = __ldg(a.c.V + ki + 1);
+                    Vt = fma(fr, V1 - V0, V0);
+                }
+                v[p][5] = fma(-Vt, inv_E, v[p][5]);
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ bool survives(int ap_type, double ax, double ay, double x, double y) {
+    if (ap_type == AP_RCOL) return (fabs(x) <= ax) && (fabs(y) <= ay);        // NaN -> false (G17)
+    const double xa = x * ax, yb = y * ay;                                    // ECOL: ax, ay hold 1/a, 1/b
+    const double r2 = fma(xa, xa, yb * yb);
+    return r2 <= 1.0;
+}
+
+constexpr unsigned long long kFlagA = 1ull, kFlagP = 2ull;    // aggregate / inclusive prefix available
+__device__ __forceinline__ unsigned long long pack_status(unsigned int epoch, unsigned long long flag,
+                                                          unsigned long long value) {
+    return ((unsigned long long)epoch << 34) | (flag << 32) | value;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// chain_kernel: one launch applies a RUN of consecutive elements to every live particle: each
+// coordinate is loaded once (128-bit), carried in registers through all maps and stored once
+// (north_star part 1; the paper launches one kernel per element).
+// COMPACT: the run ends in an aperture; survivors are written out of place in their original order and
+// the lost particles are appended to the lost log in position order (north_star part 2), with the
+// survivor ranks from a single-pass decoupled look-back scan over tiles.  Persistent grid.
+// ---------------------------------------------------------------------------------------------------
+template <int MAXOPS, bool COMPACT>
+__global__ void __launch_bounds__(kBlock) chain_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+    const ChainCommon& c = a.c;
+    const long long n = c.st->n_alive[c.cur];
+    const long long n_tiles = (n + kTile - 1) / kTile;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double mn = INFINITY, mx = -INFINITY;
+
+    __shared__ int s_warp[kWarps];
+    __shared__ long long s_base;
+    __shared__ long long s_tile;
+
+    long long tile = blockIdx.x;
+    while (true) {
+        if (COMPACT) {                          // dynamic tile order: predecessors are always running
+            if (threadIdx.x == 0) s_tile = (long long)atomicAdd(&c.st->tile_counter, 1u);
+            __syncthreads();
+            tile = s_tile;
+        }
+        if (tile >= n_tiles) break;
+        const long long i0 = tile * kTile + (long long)threadIdx.x * kP;
+        double v[kP][6];
+        long long id[kP];
+        const bool full = (i0 + kP <= n);
+        const unsigned int rmask = COMPACT ? 0x3Fu : c.rmask;
+#pragma unroll
+        for (int cc = 0; cc < 6; cc++) {
+            v[0][cc] = 0.0; v[1][cc] = 0.0;
+            if (rmask & (1u << cc)) {
+                if (full) {
+                    const double2 t = ld_stream2(c.src[cc] + i0);
+                    v[0][cc] = t.x; v[1][cc] = t.y;
+                } else if (i0 < n) {
+                    v[0][cc] = ld_stream1(c.src[cc] + i0);
+                }
+            }
+        }
+        if (COMPACT) {
+            id[0] = 0; id[1] = 0;
+            if (full) {
+                const longlong2 t = *reinterpret_cast<const longlong2*>(c.id_src + i0);
+                id[0] = t.x; id[1] = t.y;
+            } else if (i0 < n) {
+                id[0] = c.id_src[i0];
+            }
+        }
+
+        apply_ops(a, v);
+
+        if (!COMPACT) {
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) {
+                if (c.wmask & (1u << cc)) {
+                    if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[0][cc], v[1][cc]);
+                    else if (i0 < n) c.dst[cc][i0] = v[0][cc];
+                }
+            }
+            if (c.want_minmax) {
+                if (i0 < n) { mn = fmin(mn, v[0][4]); mx = fmax(mx, v[0][4]); }
+                if (full) { mn = fmin(mn, v[1][4]); mx = fmax(mx, v[1][4]); }
+            }
+            tile += gridDim.x;
+        } else {
+            bool valid[kP], surv[kP];
+#pragma unroll
+            for (int p = 0; p < kP; p++) {
+                valid[p] = (i0 + p < n);
+                surv[p] = valid[p] && survives(c.ap_type, c.ap_x, c.ap_y, v[p][0], v[p][2]);
+            }
+            const int cnt = (int)surv[0] + (int)surv[1];
+            int inc = cnt;                                     // warp inclusive scan
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += t;
+            }
+            if (lane == 31) s_warp[wid] = inc;
+            __syncthreads();
+            int woff = 0, btotal = 0;
+#pragma unroll
+            for (int w = 0; w < kWarps; w++) {
+                const int x = s_warp[w];
+                if (w < wid) woff += x;
+                btotal += x;
+            }
+            const int excl_local = woff + inc - cnt;
+            if (wid == 0) {                                    // decoupled look-back over earlier tiles
+                long long excl = 0;
+                if (tile > 0) {
+                    if (lane == 0) st_relaxed(c.tile_status + tile, pack_status(c.epoch, kFlagA, (unsigned long long)btotal));
+                    long long look = tile - 1;
+                    while (true) {
+                        const long long idx = look - lane;
+                        unsigned long long stt;
+                        bool ready;
+                        do {
+                            stt = (idx >= 0) ? ld_relaxed(c.tile_status + idx) : pack_status(c.epoch, kFlagP, 0);
+                            ready = ((unsigned int)(stt >> 34) == c.epoch) && (((stt >> 32) & 3ull) != 0);
+                        } while (__any_sync(0xffffffffu, !ready));
+                        const unsigned int pmask = __ballot_sync(0xffffffffu, ((stt >> 32) & 3ull) == kFlagP);
+                        const int first_p = pmask ? (__ffs(pmask) - 1) : 32;
+                        long long val = (lane <= first_p) ? (long long)(stt & 0xffffffffull) : 0;
+#pragma unroll
+                        for (int d = 16; d > 0; d >>= 1) val += __shfl_xor_sync(0xffffffffu, val, d);
+                        excl += val;
+                        if (pmask) break;
+                        look -= 32;
+                    }
+                }
+                if (lane == 0) {
+                    st_relaxed(c.tile_status + tile, pack_status(c.epoch, kFlagP, (unsigned long long)(excl + btotal)));
+                    s_base = excl;
+                    if (tile == n_tiles - 1) {                 // the last tile knows the totals
+                        const long long ns = excl + btotal;
+                        c.st->n_alive[c.cur ^ 1] = ns;
+                        c.st->n_lost[c.cur ^ 1] = c.st->n_lost[c.cur] + (n - ns);
+                    }
+                }
+            }
+            __syncthreads();
+            long long pos = s_base + excl_local;               // rank among survivors = destination
+            const long long lost_base = c.st->n_lost[c.cur];
+#pragma unroll
+            for (int p = 0; p < kP; p++) {
+                if (surv[p]) {
+#pragma unroll
+                    for (int cc = 0; cc < 6; cc++) c.dst[cc][pos] = v[p][cc];
+                    c.id_dst[pos] = id[p];
+                    if (c.want_minmax) { mn = fmin(mn, v[p][4]); mx = fmax(mx, v[p][4]); }
+                    pos++;
+                } else if (valid[p]) {
+                    const long long lpos = lost_base + (i0 + p) - pos;   // lost before me = index - survivors before me
+                    if (lpos < c.lost_cap) {
+                        c.lost_id[lpos] = id[p];
+                        c.lost_te[lpos] = c.te_code;
+#pragma unroll
+                        for (int cc = 0; cc < 6; cc++) c.lost_v[cc * c.lost_cap + lpos] = v[p][cc];
+                    }
+                }
+            }
+            __syncthreads();                                   // s_tile / s_warp / s_base reuse
+        }
+    }
+
+    if (c.want_minmax) {                                       // exact min/max of s (a8): order-independent
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, d));
+            mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+        }
+        __shared__ double s_mn[kWarps], s_mx[kWarps];
+        if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
+            c.mm_partial[2 * blockIdx.x] = mn;
+            c.mm_partial[2 * blockIdx.x + 1] = mx;
+        }
+    }
+    if (COMPACT) {                                             // last block out resets the counters
+        if (threadIdx.x == 0) {
+            __threadfence();
+            const unsigned int d = atomicAdd(&c.st->done_counter, 1u);
+            if (d == gridDim.x - 1) {
+                if (n_tiles == 0) {
+                    c.st->n_alive[c.cur ^ 1] = 0;
+                    c.st->n_lost[c.cur ^ 1] = c.st->n_lost[c.cur];
+                }
+                c.st->tile_counter = 0;
+                c.st->done_counter = 0;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// window_kernel (a8 -> G10): reduce the per-block min/max partials (exact in any order), derive the
+// histogram window with the same fp64 operations as the definition, the occupied bin range used for
+// shared-memory privatisation, and zero the counts.  One block.
+// ---------------------------------------------------------------------------------------------------
+struct WindowArgs {
+    DevState* st;
+    int cur;
+    const double* mm_partial;
+    int n_partial;
+    int mode;            // ELG_WIN_*
+    int nb;
+    double t_lo_rel, dt_in, t_design, inv_bc;
+    unsigned int* counts;
+};
+
+__global__ void __launch_bounds__(kBlock) window_kernel(const WindowArgs a) {
+    __shared__ double s_mn[kWarps], s_mx[kWarps];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double mn = INFINITY, mx = -INFINITY;
+    for (int i = threadIdx.x; i < a.n_partial; i += kBlock) {
+        mn = fmin(mn, a.mm_partial[2 * i]);
+        mx = fmax(mx, a.mm_partial[2 * i + 1]);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, d));
+        mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+    }
+    if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
+    for (int i = threadIdx.x; i < a.nb; i += kBlock) a.counts[i] = 0u;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
+        const long long n = a.st->n_alive[a.cur];
+        if (n == 0) { mn = 0.0; mx = 0.0; }                                  // G28
+        double t_lo, dt;
+        const double t_min = mn * a.inv_bc, t_max = mx * a.inv_bc;
+        if (a.mode == 0) {                                                   // EXPLICIT
+            t_lo = a.t_design + a.t_lo_rel;
+            dt = a.dt_in;
+        } else if (a.mode == 1) {                                            // AUTO_MINMAX
+            dt = (t_max - t_min) / (double)(a.nb - 1);
+            if (!(dt > 0.0)) dt = 1e-15;
+            t_lo = t_min - 0.5 * dt;
+        } else {                                                             // AUTO_TABLE
+            dt = a.dt_in;
+            const double tc = 0.5 * (t_min + t_max);
+            t_lo = tc - (0.5 * (double)a.nb) * dt;
+        }
+        const double inv_dt = 1.0 / dt;
+        a.st->win[0] = t_lo; a.st->win[1] = dt; a.st->win[2] = inv_dt; a.st->win[3] = 0.0;
+        a.st->smin = mn; a.st->smax = mx;
+        // the bin function is monotone in s, so every particle falls in [bin(smin), bin(smax)]
+        long long lo = (long long)floor(fmax(fmin((mn * a.inv_bc - t_lo) * inv_dt, 4.0e9), -4.0e9));
+        long long hi = (long long)floor(fmax(fmin((mx * a.inv_bc - t_lo) * inv_dt, 4.0e9), -4.0e9));
+        if (lo < 0) lo = 0;
+        if (hi > a.nb - 1) hi = a.nb - 1;
+        if (n == 0 || !(mn <= mx)) { lo = 0; hi = -1; }
+        a.st->bin_lo = lo; a.st->bin_hi = hi;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// hist_kernel (a9): threads increment shared-memory bins atomically; several private
+// sub-histograms per block (one per warp when they fit) cut contention; sub-histograms are combined
+// with integer global atomics (exact, order-independent).  Only the occupied bin range is privatised,
+// so nb = 65536 (256 KB) still fits; bins outside the first kHistSmemBins of the range fall back to
+// global atomics.  Persistent grid, 2 x 128-bit loads of s per thread and iteration.
+// ---------------------------------------------------------------------------------------------------
+struct HistArgs {
+    const double* s;
+    const DevState* st;
+    int cur;
+    long long n_fixed;     // >= 0: use this n and the explicit window below (test hook); < 0: device state
+    double inv_bc, t_lo, inv_dt;
+    int nb;
+    int aggregate;         // 1: warp-aggregate equal bins with match.any before the shared atomic
+    unsigned int* counts;
+};
+
+__global__ void __launch_bounds__(kBlock) hist_kernel(const HistArgs a) {
+    extern __shared__ unsigned int sh[];
+    long long n, blo, bhi;
+    double t_lo, inv_dt;
+    if (a.n_fixed >= 0) { n = a.n_fixed; blo = 0; bhi = a.nb - 1; t_lo = a.t_lo; inv_dt = a.inv_dt; }
+    else { n = a.st->n_alive[a.cur]; blo = a.st->bin_lo; bhi = a.st->bin_hi; t_lo = a.st->win[0]; inv_dt = a.st->win[2]; }
+    long long span = bhi - blo + 1;
+    if (span < 1) span = 1;
+    const int S = (int)(span < kHistSmemBins ? span : kHistSmemBins);
+    int R = kHistSmemBins / S;
+    if (R > kWarps) R = kWarps;
+    const int wid = threadIdx.x >> 5;
+    unsigned int* mine = sh + (wid % R) * S;
+    for (int i = threadIdx.x; i < R * S; i += kBlock) sh[i] = 0u;
+    __syncthreads();
+
+    constexpr int kPer = 4;
+    const long long stride = (long long)gridDim.x * kBlock * kPer;
+    // warp-uniform trip count (the aggregated path uses full-mask warp votes)
+    for (long long w0 = ((long long)blockIdx.x * kBlock + (threadIdx.x & ~31)) * kPer; w0 < n; w0 += stride) {
+        const long long i0 = w0 + (long long)(threadIdx.x & 31) * kPer;
+        double sv[kPer];
+        int nv = 0;
+        if (i0 + kPer <= n) {
+            const double2 t0 = ld_stream2(a.s + i0), t1 = ld_stream2(a.s + i0 + 2);
+            sv[0] = t0.x; sv[1] = t0.y; sv[2] = t1.x; sv[3] = t1.y;
+            nv = kPer;
+        } else {
+            for (; nv < kPer && i0 + nv < n; nv++) sv[nv] = a.s[i0 + nv];
+        }
+#pragma unroll
+        for (int p = 0; p < kPer; p++) {
+            double u;
+            const int b = (p < nv) ? bin_of(sv[p], a.inv_bc, t_lo, inv_dt, a.nb, &u) : -1;
+            if (a.aggregate) {
+                const unsigned int act = __ballot_sync(0xffffffffu, b >= 0);   // loop trip count is warp-uniform
+                if (b >= 0) {
+                    const unsigned int peers = __match_any_sync(act, b);
+                    if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) {
+                        const long long rel = (long long)b - blo;
+                        if (rel < S) atomicAdd(mine + rel, (unsigned int)__popc(peers));
+                        else atomicAdd(a.counts + b, (unsigned int)__popc(peers));
+                    }
+                }
+            } else if (b >= 0) {
+                const long long rel = (long long)b - blo;
+                if (rel < S) atomicAdd(mine + rel, 1u);
+                else atomicAdd(a.counts + b, 1u);
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < S; i += kBlock) {
+        unsigned int tot = 0;
+        for (int r = 0; r < R; r++) tot += sh[r * S + i];
+        if (tot) atomicAdd(a.counts + blo + i, tot);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// wake_samples_kernel (a10; G11, G12): W_k = W(k dt), k < nb, in V/C.
+// ---------------------------------------------------------------------------------------------------
+struct WakeArgs {
+    const DevState* st;    // dt from win[1] unless dt_fixed > 0
+    double dt_fixed;
+    int kind;              // ELG_WAKE_*
+    int nb;
+    double kloss, alpha, wbar, ratio;     // resonator constants, computed once on the host at load time
+    const double* table;
+    long long n_table;
+    double dt_table;
+    double* W;
+};
+
+__global__ void __launch_bounds__(kBlock) wake_samples_kernel(const WakeArgs a) {
+    const int k = blockIdx.x * kBlock + threadIdx.x;
+    if (k >= a.nb) return;
+    const double dt = (a.dt_fixed > 0.0) ? a.dt_fixed : a.st->win[1];
+    double w;
+    if (a.kind == 0) {
+        if (k == 0) w = a.kloss;                                             // beam-loading theorem (G11)
+        else {
+            const double tau = (double)k * dt;
+            w = 2.0 * a.kloss * exp(-a.alpha * tau) * (cos(a.wbar * tau) - a.ratio * sin(a.wbar * tau));
+        }
+    } else {
+        if (dt == a.dt_table) {
+            w = (k < a.n_table) ? a.table[k] : 0.0;
+        } else {
+            const double pos = ((double)k * dt) / a.dt_table;
+            const double fl = floor(pos);
+            if (!(fl >= 0.0) || fl > (double)(a.n_table - 1)) w = 0.0;
+            else {
+                const long long j = (long long)fl;
+                const double fr = pos - fl;
+                if (j == a.n_table - 1) w = (fr == 0.0) ? a.table[j] : 0.0;
+                else w = a.table[j] + fr * (a.table[j + 1] - a.table[j]);
+            }
+        }
+    }
+    a.W[k] = w;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// conv_kernel (a11, G13): V_i = q sum_{j<=i} counts_j W_{i-j}.  The paper's version
+// accumulates partial results with fp64 atomicAdd (order non-deterministic); here one warp owns one
+// output: lanes take j = j0 + lane (step 32) in ascending order and a fixed butterfly combines them,
+// so the result is run-to-run deterministic.  Empty bins outside the occupied range are skipped
+// (they contribute exact zeros).
+// ---------------------------------------------------------------------------------------------------
+struct ConvArgs {
+    const unsigned int* counts;
+    const double* W;
+    const DevState* st;    // occupied range; NULL: whole range
+    int nb;
+    double q;
+    double* V;
+};
+
+__global__ void __launch_bounds__(kBlock) conv_kernel(const ConvArgs a) {
+    const int lane = threadIdx.x & 31;
+    const int i = blockIdx.x * kWarps + (threadIdx.x >> 5);
+    if (i >= a.nb) return;
+    long long jlo = 0, jhi = i;
+    if (a.st) {
+        if (a.st->bin_lo > jlo) jlo = a.st->bin_lo;
+        if (a.st->bin_hi < jhi) jhi = a.st->bin_hi;
+    }
+    double acc = 0.0;
+    for (long long j = jlo + lane; j <= jhi; j += 32) acc = fma((double)a.counts[j], a.W[i - j], acc);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+    if (lane == 0) a.V[i] = a.q * acc;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// kick_kernel: test hook for a12 on caller-supplied arrays (the tracking path applies the kick as the
+// first op of the next fused run, OP_KICK above; same arithmetic).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlock) kick_kernel(const double* s, double* delta, long long n, double inv_bc,
+                                                      double t_lo, double inv_dt, int nb, const double* V,
+                                                      double inv_E, int interp) {
+    const long long stride = (long long)gridDim.x * kBlock;
+    for (long long i = (long long)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) {
+        double u0;
+        const int b = bin_of(s[i], inv_bc, t_lo, inv_dt, nb, &u0);
+        if (b < 0) continue;
+        double Vt;
+        if (!interp || nb < 2) Vt = V[b];
+        else {
+            const double u = u0 - 0.5;
+            double k = floor(u);
+            if (k < 0.0) k = 0.0;
+            if (k > (double)(nb - 2)) k = (double)(nb - 2);
+            double fr = u - k;
+            if (fr < 0.0) fr = 0.0;
+            if (fr > 1.0) fr = 1.0;
+            const int ki = (int)k;
+            Vt = fma(fr, V[ki + 1] - V[ki], V[ki]);
+        }
+        delta[i] = fma(-Vt, inv_E, delta[i]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// moments_kernel (a13; G20): n, centroid and 6x6 central second moments in one
+// pass over the six coordinate arrays.  s is an absolute path length, so raw second
+// moments would cancel catastrophically; sums are taken of (v - K) with K = coordinates of the first
+// live particle (a shift inside the distribution), which makes the one-pass formula well conditioned.
+// Deterministic: fixed grid, fixed per-thread order, shuffle tree, partials combined in block order by
+// the last block to finish (the paper's "last block" scheme).
+// ---------------------------------------------------------------------------------------------------
+struct MomArgs {
+    const double* src[6];
+    DevState* st;
+    int cur;
+    double* partial;       // [kNMom][gridDim.x]
+    double* record;        // 43 doubles: n, C[6], Sigma[36]
+};
+
+__global__ void __launch_bounds__(kBlock) moments_kernel(const MomArgs a) {
+    const long long n = a.st->n_alive[a.cur];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double K[6];
+#pragma unroll
+    for (int c = 0; c < 6; c++) K[c] = (n > 0) ? __ldg(a.src[c]) : 0.0;
+    double acc[kNMom];
+#pragma unroll
+    for (int q = 0; q < kNMom; q++) acc[q] = 0.0;
+
+    const long long stride = (long long)gridDim.x * kTile;
+    for (long long i0 = (long long)blockIdx.x * kTile + (long long)threadIdx.x * kP; i0 < n; i0 += stride) {
+        double d[kP][6];
+        const bool full = (i0 + kP <= n);
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+            if (full) {
+                const double2 t = ld_stream2(a.src[c] + i0);
+                d[0][c] = t.x - K[c]; d[1][c] = t.y - K[c];
+            } else {
+                d[0][c] = ld_stream1(a.src[c] + i0) - K[c]; d[1][c] = 0.0;
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < kP; p++) {
+            if (p == 1 && !full) break;
+            int q = 6;
+#pragma unroll
+            for (int r = 0; r < 6; r++) {
+                acc[r] += d[p][r];
+#pragma unroll
+                for (int c = r; c < 6; c++) { acc[q] = fma(d[p][r], d[p][c], acc[q]); q++; }
+            }
+        }
+    }
+    __shared__ double s_part[kWarps][kNMom];
+#pragma unroll
+    for (int q = 0; q < kNMom; q++) {
+        double x = acc[q];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
+        if (lane == 0) s_part[wid][q] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x < kNMom) {
+        double x = 0.0;
+        for (int w = 0; w < kWarps; w++) x += s_part[w][threadIdx.x];
+        a.partial[(long long)threadIdx.x * gridDim.x + blockIdx.x] = x;
+    }
+    __shared__ bool s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(&a.st->mom_done, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    __shared__ double s_tot[kNMom];
+    for (int q = wid; q < kNMom; q += kWarps) {                 // one warp per quantity, blocks in order
+        double x = 0.0;
+        for (int b = lane; b < (int)gridDim.x; b += 32) x += __ldcg(a.partial + (long long)q * gridDim.x + b);
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
+        if (lane == 0) s_tot[q] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double* rec = a.record;
+        rec[0] = (double)n;
+        if (n <= 0) {
+            for (int k = 1; k < 43; k++) rec[k] = 0.0;                       // G28
+        } else {
+            const double inv_n = 1.0 / (double)n;
+            double m[6];
+            for (int c = 0; c < 6; c++) { m[c] = s_tot[c] * inv_n; rec[1 + c] = K[c] + m[c]; }
+            int q = 6;
+            for (int r = 0; r < 6; r++)
+                for (int c = r; c < 6; c++) {
+                    const double val = s_tot[q] * inv_n - m[r] * m[c];
+                    rec[7 + 6 * r + c] = val;
+                    rec[7 + 6 * c + r] = val;
+                    q++;
+                }
+        }
+        a.st->mom_done = 0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlock) iota_kernel(long long* id, long long n) {
+    const long long stride = (long long)gridDim.x * kBlock;
+    for (long long i = (long long)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) id[i] = i;
+}
+
+__global__ void init_state_kernel(DevState* st, long long n0) {
+    st->n_alive[0] = n0; st->n_alive[1] = n0;
+    st->n_lost[0] = 0; st->n_lost[1] = 0;
+    st->win[0] = 0.0; st->win[1] = 1.0; st->win[2] = 1.0; st->win[3] = 0.0;
+    st->smin = 0.0; st->smax = 0.0;
+    st->bin_lo = 0; st->bin_hi = -1;
+    st->tile_counter = 0; st->done_counter = 0; st->mom_done = 0; st->pad = 0;
+}
+
+}  // namespace elg

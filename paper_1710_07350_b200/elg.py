@@ -1,0 +1,406 @@
+"""Thin ctypes binding of libelg.so (include/elg.h): argument marshalling only.
+
+Same names as the C ABI: Beamline ~ elg_beamline_load, Bunch ~ elg_bunch_create, Bunch.track ~
+elg_track, Bunch.moments ~ elg_moments, Bunch.lost ~ elg_lost.  PyTorch supplies device memory and the
+stream; every step of the path runs in the library's CUDA kernels.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+from .build import LIB, build
+
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ECAPACITY = 0, -1, -2, -3, -4, -5
+DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO = 1, 2, 3, 4, 5, 6, 7
+WIN = {"EXPLICIT": 0, "AUTO_MINMAX": 1, "AUTO_TABLE": 2}
+WAKEKIND = {"RESONATOR": 0, "TABLE": 1}
+MOM = {"none": 0, "turn": 1, "element": 2}
+ELECTRON_MC2_EV = 0.51099895e6
+
+_dp = C.POINTER(C.c_double)
+_i64p = C.POINTER(C.c_int64)
+_i32p = C.POINTER(C.c_int32)
+_u32p = C.POINTER(C.c_uint32)
+
+EXPORTS = (
+    "elg_version", "elg_last_error", "elg_launch_count", "elg_soa_stride", "elg_soa_bytes",
+    "elg_beamline_load", "elg_beamline_destroy", "elg_beamline_n_elements", "elg_beamline_length",
+    "elg_beamline_s_design", "elg_beamline_launches_per_turn", "elg_workspace_bytes",
+    "elg_bunch_create", "elg_bunch_destroy", "elg_bunch_upload", "elg_bunch_rewind", "elg_track",
+    "elg_moments", "elg_lost", "elg_n_alive", "elg_bunch_read", "elg_bunch_device_array",
+    "elg_dbg_histogram", "elg_dbg_wake_samples", "elg_dbg_convolve", "elg_dbg_kick",
+)
+
+
+class ElgError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"elg error {code}: {msg}")
+        self.code = code
+
+
+class Element(C.Structure):
+    _fields_ = [
+        ("type", C.c_int32), ("nb", C.c_int32), ("window", C.c_int32), ("wake", C.c_int32),
+        ("interp", C.c_int32), ("reserved", C.c_int32),
+        ("L", C.c_double), ("V", C.c_double), ("f", C.c_double), ("phi", C.c_double),
+        ("ax", C.c_double), ("ay", C.c_double), ("Q", C.c_double), ("Rs", C.c_double),
+        ("t_lo_rel", C.c_double), ("dt", C.c_double), ("dt_table", C.c_double),
+        ("R", _dp), ("C", _dp), ("table", _dp), ("n_table", C.c_int64),
+    ]
+
+
+class TrackOpts(C.Structure):
+    _fields_ = [
+        ("moments_every", C.c_int32), ("reserved", C.c_int32),
+        ("records", _dp), ("capacity_records", C.c_int64), ("n_records", C.c_int64),
+        ("hist_out", _u32p), ("hist_capacity", C.c_int64), ("hist_written", C.c_int64),
+        ("V_out", _dp), ("V_capacity", C.c_int64), ("V_written", C.c_int64),
+        ("window_out", _dp), ("window_capacity", C.c_int64), ("window_written", C.c_int64),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    """Load libelg.so (building it with nvcc if it is stale).  Fails loudly if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = LIB
+    if not os.path.exists(path) or os.environ.get("ELG_REBUILD"):
+        path = build()
+    else:
+        try:
+            path = build()          # no-op when up to date
+        except Exception:
+            pass                    # no nvcc on this box: use the shipped library
+    L = C.CDLL(path)
+    v6 = _dp * 6
+    vp = C.c_void_p
+    L.elg_version.restype = C.c_char_p
+    L.elg_last_error.restype = C.c_char_p
+    L.elg_launch_count.restype = C.c_int64
+    L.elg_soa_stride.argtypes = [C.c_int64]; L.elg_soa_stride.restype = C.c_int64
+    L.elg_soa_bytes.argtypes = [C.c_int64]; L.elg_soa_bytes.restype = C.c_int64
+    L.elg_beamline_load.argtypes = [C.POINTER(vp), C.POINTER(Element), C.c_int64, C.c_int32]
+    L.elg_beamline_load.restype = C.c_int32
+    L.elg_beamline_destroy.argtypes = [vp]; L.elg_beamline_destroy.restype = None
+    L.elg_beamline_n_elements.argtypes = [vp]; L.elg_beamline_n_elements.restype = C.c_int64
+    L.elg_beamline_length.argtypes = [vp]; L.elg_beamline_length.restype = C.c_double
+    L.elg_beamline_s_design.argtypes = [vp, C.c_int64]; L.elg_beamline_s_design.restype = C.c_double
+    L.elg_beamline_launches_per_turn.argtypes = [vp, C.c_int32]
+    L.elg_beamline_launches_per_turn.restype = C.c_int64
+    L.elg_workspace_bytes.argtypes = [C.c_int64, vp, C.c_int64, _i64p]; L.elg_workspace_bytes.restype = C.c_int32
+    L.elg_bunch_create.argtypes = [C.POINTER(vp), C.c_int64, vp, vp, C.c_int64, vp, C.c_int64,
+                                   C.c_double, C.c_double, C.c_double, vp]
+    L.elg_bunch_create.restype = C.c_int32
+    L.elg_bunch_destroy.argtypes = [vp]; L.elg_bunch_destroy.restype = None
+    L.elg_bunch_upload.argtypes = [vp, v6, _i64p]; L.elg_bunch_upload.restype = C.c_int32
+    L.elg_bunch_rewind.argtypes = [vp]; L.elg_bunch_rewind.restype = C.c_int32
+    L.elg_track.argtypes = [vp, vp, C.c_int64, C.POINTER(TrackOpts)]; L.elg_track.restype = C.c_int32
+    L.elg_moments.argtypes = [vp, _i64p, _dp, _dp]; L.elg_moments.restype = C.c_int32
+    L.elg_lost.argtypes = [vp, _i64p, C.c_int64, _i64p, _i32p, _i32p, _dp]; L.elg_lost.restype = C.c_int32
+    L.elg_n_alive.argtypes = [vp, _i64p]; L.elg_n_alive.restype = C.c_int32
+    L.elg_bunch_read.argtypes = [vp, v6, _i64p, C.c_int64]; L.elg_bunch_read.restype = C.c_int32
+    L.elg_bunch_device_array.argtypes = [vp, C.c_int32, C.POINTER(vp)]; L.elg_bunch_device_array.restype = C.c_int32
+    L.elg_dbg_histogram.argtypes = [vp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32, vp, vp]
+    L.elg_dbg_histogram.restype = C.c_int32
+    L.elg_dbg_wake_samples.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
+                                       vp, C.c_int64, C.c_double, vp, vp]
+    L.elg_dbg_wake_samples.restype = C.c_int32
+    L.elg_dbg_convolve.argtypes = [vp, vp, C.c_int32, C.c_double, vp, vp]; L.elg_dbg_convolve.restype = C.c_int32
+    L.elg_dbg_kick.argtypes = [vp, vp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32, vp,
+                               C.c_double, C.c_int32, vp]
+    L.elg_dbg_kick.restype = C.c_int32
+    _lib = L
+    return L
+
+
+def _ck(rc: int) -> None:
+    if rc != OK:
+        raise ElgError(rc, lib().elg_last_error().decode())
+
+
+def _p(a: Optional[np.ndarray], typ=_dp):
+    return None if a is None else a.ctypes.data_as(typ)
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def launch_count() -> int:
+    return lib().elg_launch_count()
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise ElgError(ECUDA, "no CUDA device: libelg has no CPU fallback")
+    return torch
+
+
+def _elements_to_c(elements):
+    """Workload element dictionaries -> (elg_element array, keep-alive list).  Layout only."""
+    arr = (Element * max(1, len(elements)))()
+    keep = []
+    for k, d in enumerate(elements):
+        e = arr[k]
+        t = d["type"]
+        if t == "DRIFT":
+            e.type, e.L = DRIFT, float(d["L"])
+        elif t == "MATRIX":
+            R = _f64(d["R"]).reshape(36); keep.append(R)
+            e.type, e.R = MATRIX, _p(R)
+            if d.get("C") is not None:
+                Cv = _f64(d["C"]).reshape(6); keep.append(Cv); e.C = _p(Cv)
+        elif t == "RFKICK":
+            e.type, e.V, e.f, e.phi = RFKICK, float(d["V"]), float(d["f"]), float(d["phi"])
+        elif t == "RCOL":
+            e.type, e.ax, e.ay = RCOL, float(d["ax"]), float(d["ay"])
+        elif t == "ECOL":
+            e.type, e.ax, e.ay = ECOL, float(d["a"]), float(d["b"])
+        elif t in ("WAKE", "HISTO"):
+            e.type = WAKE if t == "WAKE" else HISTO
+            e.nb = int(d["nb"])
+            e.window = WIN[d["window"]]
+            e.t_lo_rel = float(d.get("t_lo_rel", 0.0))
+            e.dt = float(d.get("dt", 0.0))
+            if t == "WAKE":
+                e.wake = WAKEKIND[d["wake"]]
+                e.interp = 1 if d.get("interp", True) else 0
+                if d["wake"] == "RESONATOR":
+                    e.f, e.Q, e.Rs = float(d["f"]), float(d["Q"]), float(d["Rs"])
+                else:
+                    tb = _f64(d["table"]); keep.append(tb)
+                    e.table, e.n_table, e.dt_table = _p(tb), tb.shape[0], float(d["dt_table"])
+        else:
+            raise ValueError(f"unknown element type {t!r}")
+    return arr, keep
+
+
+class Beamline:
+    """elg_beamline_load: host-only object (needs no device)."""
+
+    def __init__(self, elements, ring: bool = False):
+        arr, keep = _elements_to_c(elements)
+        self.elements = list(elements)
+        self.n_elems = len(elements)
+        self.ring = bool(ring)
+        h = C.c_void_p()
+        _ck(lib().elg_beamline_load(C.byref(h), arr, self.n_elems, 1 if ring else 0))
+        self._h = h
+
+    @property
+    def length(self) -> float:
+        return lib().elg_beamline_length(self._h)
+
+    def s_design(self, k: int) -> float:
+        return lib().elg_beamline_s_design(self._h, k)
+
+    def launches_per_turn(self, moments_every: str = "none") -> int:
+        return lib().elg_beamline_launches_per_turn(self._h, MOM[moments_every])
+
+    @property
+    def has_aperture(self) -> bool:
+        return any(e["type"] in ("RCOL", "ECOL") for e in self.elements)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().elg_beamline_destroy(self._h)
+            self._h = None
+
+
+class Bunch:
+    """elg_bunch_create on torch-allocated device memory.
+
+    coords: (6, n0) float64 host array (numpy, or a pinned torch CPU tensor) uploaded with
+    elg_bunch_upload; or None with n0 given, when the caller fills `soa` on the device itself and then
+    calls rewind()."""
+
+    def __init__(self, coords=None, p0c_eV: float = 1e9, charge_C: float = 1e-9, ids=None,
+                 beamline: Optional[Beamline] = None, lost_capacity: Optional[int] = None,
+                 mc2_eV: float = ELECTRON_MC2_EV, n0: Optional[int] = None, device: str = "cuda:0",
+                 stream=None):
+        torch = _torch()
+        L = lib()
+        if coords is not None:
+            n0 = int(coords.shape[1])
+        assert n0 is not None
+        self.n0 = n0
+        self.device = torch.device(device)
+        self.stride = L.elg_soa_stride(n0)
+        if lost_capacity is None:
+            lost_capacity = n0 if (beamline is None or beamline.has_aperture) else 0
+        self.lost_capacity = int(lost_capacity)
+        wb = C.c_int64()
+        _ck(L.elg_workspace_bytes(n0, beamline._h if beamline else None, self.lost_capacity, C.byref(wb)))
+        with torch.cuda.device(self.device):
+            self.soa = torch.empty(7 * self.stride, dtype=torch.float64, device=self.device)
+            self.work = torch.empty((wb.value + 7) // 8, dtype=torch.float64, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            _ck(L.elg_bunch_create(C.byref(h), n0, self.soa.data_ptr(), self.work.data_ptr(), wb.value,
+                                   beamline._h if beamline else None, self.lost_capacity,
+                                   p0c_eV, mc2_eV, charge_C, self._stream.cuda_stream))
+        self._h = h
+        if coords is not None:
+            self.upload(coords, ids)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().elg_bunch_destroy(self._h)
+            self._h = None
+
+    # -- data movement -------------------------------------------------------------------------
+    def upload(self, coords, ids=None) -> None:
+        """elg_bunch_upload from host memory ((6, n0) numpy array or pinned torch tensor)."""
+        if hasattr(coords, "data_ptr"):          # torch CPU tensor (possibly pinned)
+            assert coords.dtype.is_floating_point and coords.element_size() == 8 and coords.is_contiguous()
+            base = coords.data_ptr()
+            ptrs = (_dp * 6)(*[C.cast(base + c * self.n0 * 8, _dp) for c in range(6)])
+            self._keep = coords
+        else:
+            coords = _f64(coords)
+            assert coords.shape == (6, self.n0)
+            ptrs = (_dp * 6)(*[_p(coords[c]) for c in range(6)])
+            self._keep = coords
+        idp = None
+        if ids is not None:
+            ids = np.ascontiguousarray(ids, dtype=np.int64)
+            idp = _p(ids, _i64p)
+        _ck(lib().elg_bunch_upload(self._h, ptrs, idp))
+        if not hasattr(coords, "is_pinned") or not coords.is_pinned():
+            self.synchronize()                   # pageable source: make the copy complete before returning
+
+    def rewind(self) -> None:
+        _ck(lib().elg_bunch_rewind(self._h))
+
+    def synchronize(self) -> None:
+        self._stream.synchronize()
+
+    # -- tracking ------------------------------------------------------------------------------
+    def track(self, bl: Beamline, n_turns: int = 1, moments_every: str = "none",
+              want_stage_outputs: bool = False, records: bool = True):
+        """elg_track.  Returns dict(records (k,43)[, hist, V, window])."""
+        o = TrackOpts()
+        o.moments_every = MOM[moments_every]
+        n_rec = {"none": 0, "turn": n_turns, "element": n_turns * bl.n_elems}[moments_every]
+        rec = None
+        if records and n_rec:
+            rec = np.zeros((n_rec, 43), dtype=np.float64)
+            o.records, o.capacity_records = _p(rec), n_rec
+        hist = V = win = None
+        if want_stage_outputs:
+            nh = sum(e["nb"] for e in bl.elements if e["type"] in ("WAKE", "HISTO")) * n_turns
+            nv = sum(e["nb"] for e in bl.elements if e["type"] == "WAKE") * n_turns
+            nw = sum(1 for e in bl.elements if e["type"] in ("WAKE", "HISTO")) * n_turns
+            hist = np.zeros(max(nh, 1), dtype=np.uint32)
+            V = np.zeros(max(nv, 1), dtype=np.float64)
+            win = np.zeros((max(nw, 1), 3), dtype=np.float64)
+            o.hist_out, o.hist_capacity = _p(hist, _u32p), nh
+            o.V_out, o.V_capacity = _p(V), nv
+            o.window_out, o.window_capacity = _p(win), nw
+        _ck(lib().elg_track(self._h, bl._h, n_turns, C.byref(o)))
+        out = {"n_records": o.n_records}
+        if rec is not None:
+            out["records"] = rec[: o.n_records]
+        if want_stage_outputs:
+            out["hist"] = hist[: o.hist_written]
+            out["V"] = V[: o.V_written]
+            out["window"] = win[: o.window_written]
+        return out
+
+    # -- read-backs (synchronise) ----------------------------------------------------------------
+    @property
+    def n_alive(self) -> int:
+        n = C.c_int64()
+        _ck(lib().elg_n_alive(self._h, C.byref(n)))
+        return n.value
+
+    def read(self, out: Optional[np.ndarray] = None):
+        n = self.n_alive
+        v = np.empty((6, n), dtype=np.float64) if out is None else out[:, :n]
+        ids = np.empty(n, dtype=np.int64)
+        if n:
+            ptrs = (_dp * 6)(*[_p(v[c]) for c in range(6)])
+            _ck(lib().elg_bunch_read(self._h, ptrs, _p(ids, _i64p), n))
+        return v, ids
+
+    def moments(self):
+        n = C.c_int64()
+        cen = np.empty(6); sig = np.empty(36)
+        _ck(lib().elg_moments(self._h, C.byref(n), _p(cen), _p(sig)))
+        return n.value, cen, sig.reshape(6, 6)
+
+    def lost(self):
+        nl = C.c_int64()
+        rc = lib().elg_lost(self._h, C.byref(nl), 0, None, None, None, None)
+        if rc not in (OK, ECAPACITY):
+            _ck(rc)
+        n = min(nl.value, self.lost_capacity)
+        ids = np.empty(n, dtype=np.int64); turn = np.empty(n, dtype=np.int32)
+        elem = np.empty(n, dtype=np.int32); co = np.empty((n, 6), dtype=np.float64)
+        if n:
+            rc = lib().elg_lost(self._h, C.byref(nl), n, _p(ids, _i64p), _p(turn, _i32p), _p(elem, _i32p), _p(co))
+            if rc not in (OK, ECAPACITY):
+                _ck(rc)
+        return ids, turn, elem, co
+
+    def device_array(self, c: int):
+        """torch view of coordinate c (0..5; 6 = IDs as int64) of the CURRENT store, live prefix not applied."""
+        torch = _torch()
+        p = C.c_void_p()
+        _ck(lib().elg_bunch_device_array(self._h, c, C.byref(p)))
+        for base in (self.soa, self.work):
+            off = p.value - base.data_ptr()
+            if 0 <= off < base.numel() * 8:
+                t = base[off // 8: off // 8 + self.stride]
+                return t.view(torch.int64) if c == 6 else t
+        raise ElgError(ESTATE, "device array outside the lent buffers")
+
+
+# ------------------------------------------------------------------------------- single-stage hooks
+def dbg_histogram(s, inv_bc: float, t_lo: float, inv_dt: float, nb: int) -> np.ndarray:
+    torch = _torch()
+    d_s = torch.as_tensor(_f64(s), device="cuda")
+    d_c = torch.empty(nb, dtype=torch.int32, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    _ck(lib().elg_dbg_histogram(d_s.data_ptr(), d_s.numel(), inv_bc, t_lo, inv_dt, nb, d_c.data_ptr(), st))
+    return d_c.cpu().numpy().view(np.uint32)
+
+
+def dbg_wake_samples(kind: int, nb: int, dt: float, f=0.0, Q=0.0, Rs=0.0, table=None, dt_table=0.0) -> np.ndarray:
+    torch = _torch()
+    d_t = None if table is None else torch.as_tensor(_f64(table), device="cuda")
+    d_W = torch.empty(nb, dtype=torch.float64, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    _ck(lib().elg_dbg_wake_samples(kind, nb, dt, f, Q, Rs, None if d_t is None else d_t.data_ptr(),
+                                   0 if d_t is None else d_t.numel(), dt_table, d_W.data_ptr(), st))
+    return d_W.cpu().numpy()
+
+
+def dbg_convolve(counts, W, q: float) -> np.ndarray:
+    torch = _torch()
+    d_c = torch.as_tensor(np.ascontiguousarray(counts, dtype=np.uint32).view(np.int32), device="cuda")
+    d_W = torch.as_tensor(_f64(W), device="cuda")
+    d_V = torch.empty(d_c.numel(), dtype=torch.float64, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    _ck(lib().elg_dbg_convolve(d_c.data_ptr(), d_W.data_ptr(), d_c.numel(), q, d_V.data_ptr(), st))
+    return d_V.cpu().numpy()
+
+
+def dbg_kick(s, delta, inv_bc, t_lo, inv_dt, nb, V, inv_E, interp=True) -> np.ndarray:
+    torch = _torch()
+    d_s = torch.as_tensor(_f64(s), device="cuda")
+    d_d = torch.as_tensor(_f64(delta), device="cuda").clone()
+    d_V = torch.as_tensor(_f64(V), device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    _ck(lib().elg_dbg_kick(d_s.data_ptr(), d_d.data_ptr(), d_s.numel(), inv_bc, t_lo, inv_dt, nb, d_V.data_ptr(),
+                           inv_E, 1 if interp else 0, st))
+    return d_d.cpu().numpy()

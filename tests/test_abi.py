@@ -1,0 +1,109 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/elg.h declares, and its
+host-only logic (beamline validation, design orbit, run planning, workspace sizing) behaves.  No compute
+call is made here (there is no GPU on this box, and libelg has no CPU fallback)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from elg_inputs import make_workload
+from paper_1710_07350_b200 import elg
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "elg.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(elg_[a-z0-9_]+)\s*\(", hdr))
+    assert len(declared) >= 25
+    L = elg.lib()
+    for name in sorted(declared):
+        assert hasattr(L, name), f"libelg.so does not export {name}"
+    assert declared == set(elg.EXPORTS)
+    assert b"sm_100a" in L.elg_version()
+
+
+def test_element_struct_matches_header_layout():
+    # 6 int32 + 11 doubles + 3 pointers + int64 = 24 + 88 + 24 + 8
+    assert C.sizeof(elg.Element) == 144
+    assert elg.Element.L.offset == 24 and elg.Element.R.offset == 112 and elg.Element.n_table.offset == 136
+    assert C.sizeof(elg.TrackOpts) == 8 + 3 * 8 + 3 * 8 * 3
+
+
+def test_soa_geometry():
+    L = elg.lib()
+    assert L.elg_soa_stride(1) == 32 and L.elg_soa_stride(32) == 32 and L.elg_soa_stride(33) == 64
+    assert L.elg_soa_stride(100_000_000) == 100_000_000
+    assert L.elg_soa_bytes(1000) == 7 * 1024 * 8
+
+
+def test_beamline_design_orbit_and_validation():
+    w = make_workload("cfg0")
+    bl = elg.Beamline(w.elements)
+    assert bl.length == 1.5 and bl.s_design(0) == 0.0 and bl.s_design(1) == 1.0 and bl.s_design(4) == 1.5
+    w3 = make_workload("cfg3", n=8)
+    bl3 = elg.Beamline(w3.elements, ring=True)
+    assert bl3.length == 200.0
+    for bad, frag in (
+        ([{"type": "DRIFT", "L": float("nan")}], "element 0"),
+        ([{"type": "DRIFT", "L": 1.0}, {"type": "RCOL", "ax": 0.0, "ay": 1.0}], "element 1"),
+        ([{"type": "WAKE", "nb": 1, "window": "AUTO_MINMAX", "wake": "RESONATOR", "f": 1e9, "Q": 1.0, "Rs": 1.0}], "nb"),
+        ([{"type": "WAKE", "nb": 8, "window": "AUTO_MINMAX", "wake": "RESONATOR", "f": 1e9, "Q": 0.5, "Rs": 1.0}], "Q"),
+        ([{"type": "HISTO", "nb": 8, "window": "EXPLICIT", "dt": 0.0}], "dt"),
+        ([{"type": "WAKE", "nb": 8, "window": "AUTO_TABLE", "wake": "RESONATOR", "f": 1e9, "Q": 1.0, "Rs": 1.0}], "AUTO_TABLE"),
+    ):
+        with pytest.raises(elg.ElgError) as ei:
+            elg.Beamline(bad)
+        assert ei.value.code == elg.EINVAL and frag in str(ei.value)
+
+
+def test_run_planning_fuses_elements():
+    """north_star part 1: runs of consecutive elements are one launch."""
+    # cfg0: [DRIFT, MATRIX, RCOL] -> 1 fused compacting launch; WAKE -> window, histogram, samples,
+    # convolution; the kick is flushed as one launch; + 1 moments kernel per turn
+    bl = elg.Beamline(make_workload("cfg0").elements)
+    assert bl.launches_per_turn("none") == 1 + 4 + 1
+    assert bl.launches_per_turn("turn") == 1 + 4 + 1 + 1
+    # cfg3: 201 maps -> ceil(201/80) = 3 chain launches (last one carries the min/max epilogue)
+    bl = elg.Beamline(make_workload("cfg3", n=8).elements, ring=True)
+    assert bl.launches_per_turn("none") == 3 + 4 + 1
+    # p1: DRIFT + MATRIX -> one launch
+    assert elg.Beamline(make_workload("p1-chain", n=8).elements).launches_per_turn("none") == 1
+    # cfg4: 20 x [RCOL, HISTO, DRIFT]: every RCOL launch carries the preceding DRIFT and the min/max
+    # epilogue for the HISTO: 20 x (1 + 2) + the trailing DRIFT
+    assert elg.Beamline(make_workload("cfg4", n=8).elements).launches_per_turn("none") == 20 * 3 + 1
+    # cfg1 with moments after every element: one chain launch + one moments launch per element
+    bl = elg.Beamline(make_workload("cfg1", n=8).elements)
+    assert bl.launches_per_turn("element") == 77 * 2
+    assert bl.launches_per_turn("none") == 25 + 1
+
+
+def test_workspace_bytes_scales():
+    L = elg.lib()
+    out = C.c_int64()
+    bl = elg.Beamline(make_workload("cfg4", n=8).elements)
+    assert L.elg_workspace_bytes(1000, bl._h, 0, C.byref(out)) == 0
+    small = out.value
+    assert L.elg_workspace_bytes(1000, bl._h, 1000, C.byref(out)) == 0
+    assert out.value - small >= 1000 * 8 * 8
+    assert L.elg_workspace_bytes(10_000_000, bl._h, 0, C.byref(out)) == 0
+    assert out.value >= 7 * 10_000_000 * 8
+    assert L.elg_workspace_bytes(-1, None, 0, C.byref(out)) == elg.EINVAL
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(elg.ElgError) as ei:
+        elg.Bunch(np.zeros((6, 4)), 1e9, 1e-9)
+    assert ei.value.code == elg.ECUDA
+    # the raw C call also refuses without a device
+    h = C.c_void_p()
+    buf = (C.c_char * 4096)()
+    addr = (C.addressof(buf) + 255) & ~255
+    rc = elg.lib().elg_bunch_create(C.byref(h), 0, addr, addr, 1 << 30, None, 0, 1e9, 0.511e6, 1e-9, None)
+    assert rc == elg.ECUDA
