@@ -1,0 +1,465 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the tracking hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg3]
+
+Workload: BASELINE.json quotes its metric "at 1e8 particles on one B200", i.e.
+configs[3]: 1e8-particle Gaussian bunch, ring of 200 MATRIX elements + RFKICK + resonator WAKE
+(1024 bins), moments every turn.  One STEP = one turn of that ring over the whole bunch.  The metric is
+Mparticle-element passes/s (a pass = one live particle entering one DRIFT/MATRIX/RFKICK/RCOL/ECOL/WAKE
+element; histogram-only elements and moments are not elements, their time is included).
+
+One JSON line is printed by rank 0.  `value` is device-timed with the bunch resident in HBM; `e2e`
+re-uploads the bunch from pinned host memory through the C ABI every step and reads the moments record
+back.  `roofline` describes the dominant kernel of the step; `probes` gives the HBM-bound kernels
+north_star's target names (fused chain, chain + compaction, histogram, moments) at the same particle count.
+N > 1: replicas only (no data-path collective): every rank tracks its own bunch; value = total passes / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Mparticle-element passes/s"
+UNIT = "Mpasses/s"
+# algorithmic fp64 flops per particle per element (MATRIX = 36 FMA, the constant C
+# rides as the accumulator's start value; DRIFT = 5 FMA + sqrt; RFKICK = sub, mul, 2 FMA (+ sin, not counted);
+# wake KICK = bin index and interpolation: mul, sub, mul, sub, sub, sub, FMA, FMA)
+FLOPS = {"MATRIX": 72.0, "DRIFT": 11.0, "RFKICK": 6.0, "WAKE": 10.0}
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x DFMA/clk/SM x 2 flop x clocks.max.sm
+NOMINAL_HBM_GBS = 8000.0                              # BASELINE.json: "vs 8 TB/s roofline"
+
+
+# ------------------------------------------------------------------------------------------- helpers
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel: str, workload: str):
+    """dram bytes per launch from the committed ncu --set full capture (profiles/*_traffic.csv), or None."""
+    import glob
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
+        for line in open(path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 3 and f[0] == kernel and f[1] == workload:
+                try:
+                    best = float(f[2])
+                except ValueError:
+                    pass
+    return best
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return self
+        def pump():
+            for line in self.proc.stdout:
+                self.rows.append((time.perf_counter(), line))
+        self.thread = threading.Thread(target=pump, daemon=True)
+        self.thread.start()
+        return self
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+            if self.thread is not None:
+                self.thread.join(timeout=2)
+
+    def summary(self, t0=None, t1=None):
+        sm, mx, pw, reasons = [], [], [], set()
+        for (t, line) in self.rows:
+            if t0 is not None and not (t0 <= t <= t1 + 0.15):
+                continue
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(self.NAMES, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def flops_per_particle_turn(elements):
+    return sum(FLOPS.get(e["type"], 0.0) for e in elements)
+
+
+# ------------------------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores, on a bounded sample of the same
+    workload (one step = one turn of the workload's beamline over `sample` particles)."""
+    from paper_1710_07350_b200.dist import env_rank
+    rank, _, world = env_rank()
+    if rank != 0:
+        return 0
+    from elg_inputs import make_workload
+    from oracle import elgo
+    elgo.build()
+    cores = os.cpu_count() or 1
+    threads = max(1, min(cores, 64))
+    w = make_workload(args.workload, n=args.cpu_sample)
+    v0 = w.particles()
+    ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
+    obl = elgo.Beamline(w.elements, ring=w.ring)
+    mom = w.moments_every
+    per_turn = w.n_pass_elements
+    for _ in range(args.warmup):
+        ob.track(obl, 1, moments_every=mom, n_threads=threads)
+    passes = 0
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        n_in = ob.n_alive
+        ob.track(obl, 1, moments_every=mom, n_threads=threads)
+        passes += n_in * per_turn          # ring workloads have no aperture; line workloads: upper bound
+    dt = time.perf_counter() - t0
+    value = passes / dt / 1e6
+    sample = f"{args.cpu_sample} particles of {w.name}, {args.steps} turn(s), {threads} threads"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / max(args.steps, 1) * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "particles": args.cpu_sample, "elements_per_turn": per_turn,
+                   "note": "CPU oracle (oracle/elgo.cpp) on a bounded sample of the workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def cpu_baseline(workload_name: str, sample: int):
+    from elg_inputs import make_workload
+    from oracle import elgo
+    elgo.build()
+    cores = os.cpu_count() or 1
+    threads = max(1, min(cores, 64))
+    w = make_workload(workload_name, n=sample)
+    v0 = w.particles()
+    ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
+    obl = elgo.Beamline(w.elements, ring=w.ring)
+    ob.track(obl, 1, moments_every=w.moments_every, n_threads=threads)          # warm-up turn
+    turns = 0
+    t0 = time.perf_counter()
+    while True:
+        ob.track(obl, 1, moments_every=w.moments_every, n_threads=threads)
+        turns += 1
+        if time.perf_counter() - t0 > 10.0 or turns >= 50:
+            break
+    dt = time.perf_counter() - t0
+    value = sample * w.n_pass_elements * turns / dt / 1e6
+    return {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{sample} particles of {w.name} x {turns} turn(s) in {dt:.1f} s, {threads} threads "
+                      f"of {cores} host cores"}
+
+
+# ------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    from paper_1710_07350_b200 import dist as pdist
+    rank, local_rank, world = pdist.env_rank()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (libelg has no CPU fallback)"
+    if world > 1:
+        pdist.init_process_group("nccl")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    from elg_inputs import make_workload
+    from paper_1710_07350_b200 import elg
+    elg.lib()
+
+    w = make_workload(args.workload, n=args.n)
+    n0 = w.n0
+    hbm_peak, peak_src = measured_peaks()
+
+    # ---- inputs: generated once on the host (counter-based, G25) straight into pinned memory
+    t_gen = time.perf_counter()
+    h_pinned = torch.empty((6, n0), dtype=torch.float64, pin_memory=True)
+    w.particles(n0, start=pdist.shard_start(rank, n0), out=h_pinned.numpy())
+    t_gen = time.perf_counter() - t_gen
+
+    want_probes = (not args.no_probes) and world == 1 and rank == 0
+    lossy = any(e["type"] in ("RCOL", "ECOL") for e in w.elements)
+    gb = elg.Bunch(None, w.p0c_eV, w.charge_C, beamline=None, n0=n0, device=str(dev),
+                   lost_capacity=(n0 if (lossy or want_probes) else 0))
+    gbl = elg.Beamline(w.elements, ring=w.ring)
+    gb.upload(h_pinned)
+    gb.synchronize()
+    pristine = gb.soa.clone() if (want_probes or not w.ring) else None
+
+    def restore():
+        gb.soa.copy_(pristine)
+        gb.rewind()
+
+    mom = w.moments_every
+    per_turn = w.n_pass_elements
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        gb.track(gbl, 1, moments_every=mom, records=False)
+
+    # ---- headline: W warm-up steps, then EXACTLY K timed steps
+    if not w.ring:
+        # a line is traversed once: every step starts from the pristine bunch (restore is not timed)
+        for _ in range(args.warmup):
+            restore(); step()
+        gb.synchronize()
+    else:
+        for _ in range(args.warmup):
+            step()
+    gb.synchronize()
+    pdist.barrier()
+    torch.cuda.synchronize(dev)
+    gb.profile(True); gb.profile_read()
+    launches0 = elg.launch_count()
+    sampler = ClockSampler(local_rank).start()
+    time.sleep(0.25)
+    t_wall0 = time.perf_counter()
+    passes = 0.0
+    if w.ring:
+        n_in = gb.n_alive
+        ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(args.steps):
+            step()
+        ev1.record(stream)
+        torch.cuda.synchronize(dev)
+        elapsed_ms = ev0.elapsed_time(ev1)
+        n_out = gb.n_alive
+        assert n_in == n_out or lossy
+        passes = float(n_in) * per_turn * args.steps
+    else:
+        elapsed_ms = 0.0
+        for _ in range(args.steps):
+            restore()
+            ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+            ev0.record(stream); step(); ev1.record(stream)
+            torch.cuda.synchronize(dev)
+            elapsed_ms += ev0.elapsed_time(ev1)
+            passes += line_passes(gb, w)
+    t_wall1 = time.perf_counter()
+    launches = elg.launch_count() - launches0
+    prof = gb.profile_read()
+    pdist.barrier()
+    torch.cuda.synchronize(dev)
+    time.sleep(0.15)
+    sampler.stop()
+    clocks = sampler.summary(t_wall0, t_wall1)
+    gb.profile(False)
+    t_max, passes_all = pdist.aggregate(elapsed_ms, passes, dev if world > 1 else None)
+    value = passes_all / (t_max * 1e-3) / 1e6
+
+    # ---- roofline of the dominant kernel of the step
+    roofline = None
+    kinds = {k: v for k, v in prof.items() if v[0] > 0}
+    total_kernel_ms = sum(v[1] for v in kinds.values())
+    dominant = max(kinds, key=lambda k: kinds[k][1]) if kinds else None
+    shares = {k: round(v[1] / total_kernel_ms, 4) for k, v in kinds.items()} if kinds else {}
+    if dominant == "chain" and w.ring:
+        fl = flops_per_particle_turn(w.elements) * float(n0) * args.steps        # all chain launches together
+        n_l, ms = kinds["chain"]
+        ach = fl / (ms * 1e-3) / 1e12
+        by = 96.0 * n0 * n_l                                                      # 48 B in + 48 B out per launch
+        roofline = {"kernel": "chain_kernel", "bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS,
+                    "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
+                    "peak_source": "derived: 148 SMs x 64 DFMA/clk/SM x 2 x 1.965 GHz (DESIGN.md)",
+                    "traffic": ncu_traffic("chain_kernel", w.name),
+                    "launches": n_l, "avg_launch_ms": ms / n_l,
+                    "flops_per_launch": fl / n_l, "algorithmic_bytes_per_launch": by / n_l,
+                    "hbm_gbs": by / (ms * 1e-3) / 1e9, "hbm_frac_of_measured": by / (ms * 1e-3) / 1e9 / hbm_peak,
+                    "share_of_step": shares.get("chain")}
+    elif dominant is not None:
+        bpp = {"chain": 96.0, "chain_compact": 112.0, "hist": 8.0, "moments": 48.0}.get(dominant)
+        n_l, ms = kinds[dominant]
+        if bpp is not None:
+            ach = bpp * n0 * n_l / (ms * 1e-3) / 1e9
+            roofline = {"kernel": dominant + "_kernel", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
+                        "unit": "GB/s", "frac": ach / hbm_peak, "peak_source": peak_src,
+                        "traffic": ncu_traffic(dominant + "_kernel", w.name), "launches": n_l,
+                        "avg_launch_ms": ms / n_l, "algorithmic_bytes_per_launch": bpp * n0,
+                        "note": "bytes use n0 live particles per launch (upper bound when particles are lost)",
+                        "share_of_step": shares.get(dominant)}
+
+    # ---- end to end through the C ABI with HOST buffers: upload (pinned H2D) + one turn + record D2H
+    e2e = None
+    if not args.no_e2e:
+        k_e2e = max(1, min(args.steps, args.e2e_steps))
+        gb.upload(h_pinned); gb.track(gbl, 1, moments_every="turn"); gb.synchronize()      # warm-up
+        pdist.barrier(); torch.cuda.synchronize(dev)
+        ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        ev0.record(stream)
+        e_passes = 0.0
+        rec = None
+        for _ in range(k_e2e):
+            gb.upload(h_pinned)                                   # elg_bunch_upload: 6 x n0 x 8 B from pinned host
+            out = gb.track(gbl, 1, moments_every="turn")          # elg_track with a HOST record buffer (syncs)
+            rec = out["records"]
+            e_passes += float(n0) * per_turn if w.ring else line_passes(gb, w)
+        ev1.record(stream)
+        torch.cuda.synchronize(dev)
+        e_ms = max(ev0.elapsed_time(ev1), (time.perf_counter() - t0) * 1e3)
+        e_max, e_all = pdist.aggregate(e_ms, e_passes, dev if world > 1 else None)
+        e2e = {"value": e_all / (e_max * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 6 * n0 * 8,
+               "d2h_bytes_per_step": int(rec.size * 8), "steps": k_e2e, "ms_per_step": e_max / k_e2e,
+               "what": "elg_bunch_upload from pinned host memory + elg_track(1 turn, host moments record)"}
+
+    # ---- HBM-bound probes at the same particle count (north_star target kernels)
+    probes = []
+    if want_probes:
+        probes = run_probes(elg, gb, restore, n0, w, hbm_peak, stream, dev, args)
+
+    if rank != 0:
+        return 0
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        cpu = cpu_baseline(w.name, args.cpu_sample)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "particles_per_gpu": n0, "elements_per_turn": per_turn,
+                   "step": "one turn of the beamline over the whole bunch" if w.ring else "one pass of the line",
+                   "moments_every": mom, "parallelism": "replicas only (no data-path collective)" if world > 1 else "1 GPU",
+                   "l2": "inputs larger than L2 (%.1f GB of particle data per step)" % (7 * n0 * 8 / 1e9),
+                   "notes": w.notes, "input_generation_s": round(t_gen, 2)},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "kernel_ms_per_step": {k: round(v[1] / args.steps, 4) for k, v in kinds.items()},
+        "kernel_share": shares,
+        "roofline": roofline, "probes": probes, "cpu_baseline": cpu,
+        "hbm_peak_gbs": hbm_peak, "hbm_peak_source": peak_src,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def line_passes(gb, w):
+    """Passes of one traversal of a (possibly lossy) line: sum over elements of the particles entering it,
+    from the lost log's element indices (exact)."""
+    ids, turn, elem, _ = gb.lost()
+    lost_at = np.bincount(elem, minlength=len(w.elements)) if elem.size else np.zeros(len(w.elements), dtype=np.int64)
+    n = w.n0
+    total = 0
+    for k, e in enumerate(w.elements):
+        if e["type"] != "HISTO":
+            total += n
+        n -= int(lost_at[k])
+    return float(total)
+
+
+def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
+    """cfg0's beamline (DRIFT, MATRIX, RCOL, WAKE 512 bins, moments) and its prefixes at n0 particles."""
+    import torch
+    from elg_inputs import make_workload
+    out = []
+    cases = [
+        ("p1-chain", "none", {"chain": 96.0}),
+        ("p2-chain-rcol", "none", {"chain_compact": 112.0}),
+        ("cfg0", "turn", {"chain_compact": 112.0, "hist": 8.0, "moments": 48.0, "chain": 24.0}),
+    ]
+    for name, mom, bytes_pp in cases:
+        w = make_workload(name, n=n0)
+        bl = elg.Beamline(w.elements, ring=False)
+        for _ in range(3):
+            restore(); gb.track(bl, 1, moments_every=mom, records=False)
+        gb.synchronize()
+        gb.profile(True); gb.profile_read()
+        ms_total = 0.0
+        k = args.probe_steps
+        passes = 0.0
+        for _ in range(k):
+            restore()
+            ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+            ev0.record(stream)
+            gb.track(bl, 1, moments_every=mom, records=False)
+            ev1.record(stream)
+            torch.cuda.synchronize(dev)
+            ms_total += ev0.elapsed_time(ev1)
+        prof = gb.profile_read()
+        gb.profile(False)
+        passes = line_passes(gb, w)
+        n_alive = gb.n_alive
+        for kind, bpp in bytes_pp.items():
+            n_l, ms = prof[kind]
+            if n_l == 0:
+                continue
+            n_eff = n0 if kind in ("chain_compact",) or name == "p1-chain" else n_alive
+            ach = bpp * n_eff * n_l / (ms * 1e-3) / 1e9
+            out.append({"workload": name, "kernel": kind + "_kernel", "bound": "hbm", "particles": int(n_eff),
+                        "bytes_per_particle": bpp, "avg_launch_ms": ms / n_l, "achieved": ach, "unit": "GB/s",
+                        "peak": hbm_peak, "frac": ach / hbm_peak, "frac_of_8TBs": ach / NOMINAL_HBM_GBS})
+        out.append({"workload": name, "kernel": "whole pass", "ms_per_pass": ms_total / k,
+                    "value": passes / (ms_total / k * 1e-3) / 1e6, "unit": UNIT, "n_alive_after": int(n_alive)})
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--n", type=int, default=None, help="particles per GPU (default: the workload's own count)")
+    ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="particles of the oracle's bounded sample")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--probe-steps", type=int, default=5)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-probes", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                                        # timing rule: W >= 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -169,6 +169,16 @@ int32_t elg_bunch_read(elg_bunch*, double* const h_coords[6], int64_t* h_ids, in
  * between d_soa and a copy in the workspace). */
 int32_t elg_bunch_device_array(elg_bunch*, int32_t c, void** d_ptr);
 
+/* ---- per-kernel device timing (for bench.py's roofline object) ---------------------------------------
+ * With profiling on, every kernel the bunch launches is bracketed by a pair of CUDA events on the bunch's
+ * stream.  elg_profile_read synchronises the stream, returns per kernel kind the number of launches and
+ * their summed device time since the last read (h_launches, h_ms: ELG_K_COUNT entries each) and resets
+ * the counters.  Off by default (no events are recorded). */
+enum { ELG_K_CHAIN = 0, ELG_K_CHAIN_COMPACT = 1, ELG_K_WINDOW = 2, ELG_K_HIST = 3, ELG_K_WAKE_SAMPLES = 4,
+       ELG_K_CONV = 5, ELG_K_MOMENTS = 6, ELG_K_COUNT = 7 };
+int32_t elg_profile_enable(elg_bunch*, int32_t on);
+int32_t elg_profile_read(elg_bunch*, int64_t* h_launches, double* h_ms);
+
 /* ---- single-stage test hooks (same kernels as elg_track; device arrays supplied by the caller) ----- */
 int32_t elg_dbg_histogram(const double* d_s, int64_t n, double inv_bc, double t_lo, double inv_dt, int32_t nb,
                           uint32_t* d_counts, void* stream);

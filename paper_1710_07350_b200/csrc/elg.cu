@@ -94,6 +94,33 @@ struct elg_bunch {
     int grid_chain[2][2] = {{0, 0}, {0, 0}};            // [large][compact]
     int grid_hist = 0, grid_mom = 0;
     int hist_aggregate = 0;
+    // optional per-kernel event timing (elg_profile_*)
+    bool prof_on = false;
+    struct ProfRec { int kind; cudaEvent_t t0, t1; };
+    std::vector<ProfRec> prof_recs;
+    std::vector<cudaEvent_t> prof_pool;
+    long long prof_launches[ELG_K_COUNT] = {0};
+    double prof_ms[ELG_K_COUNT] = {0};
+
+    cudaEvent_t prof_event() {
+        cudaEvent_t e = nullptr;
+        if (!prof_pool.empty()) { e = prof_pool.back(); prof_pool.pop_back(); }
+        else if (cudaEventCreate(&e) != cudaSuccess) e = nullptr;
+        return e;
+    }
+    // drain finished records into the per-kind sums (the caller has synchronised the stream)
+    void prof_drain() {
+        for (ProfRec& r : prof_recs) {
+            float ms = 0.f;
+            if (r.t0 && r.t1 && cudaEventElapsedTime(&ms, r.t0, r.t1) == cudaSuccess) {
+                prof_launches[r.kind]++;
+                prof_ms[r.kind] += (double)ms;
+            }
+            if (r.t0) prof_pool.push_back(r.t0);
+            if (r.t1) prof_pool.push_back(r.t1);
+        }
+        prof_recs.clear();
+    }
 
     double* coord(int buf, int c) const { return reinterpret_cast<double*>((buf ? soaB : d_soa) + (long long)c * stride * 8); }
     long long* ids(int buf) const { return reinterpret_cast<long long*>((buf ? soaB : d_soa) + 6LL * stride * 8); }
@@ -102,6 +129,22 @@ struct elg_bunch {
 namespace {
 
 unsigned long long g_bl_serial = 0;
+
+// brackets one kernel launch with CUDA events when profiling is on
+struct ProfScope {
+    elg_bunch* b;
+    int idx = -1;
+    ProfScope(elg_bunch* b_, int kind) : b(b_) {
+        if (!b || !b->prof_on) return;
+        elg_bunch::ProfRec r{kind, b->prof_event(), b->prof_event()};
+        if (r.t0) cudaEventRecord(r.t0, b->stream);
+        b->prof_recs.push_back(r);
+        idx = (int)b->prof_recs.size() - 1;
+    }
+    ~ProfScope() {
+        if (idx >= 0 && b->prof_recs[idx].t1) cudaEventRecord(b->prof_recs[idx].t1, b->stream);
+    }
+};
 
 // ------------------------------------------------------------------------------------- workspace
 struct WorkLayout {
@@ -327,8 +370,29 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     return ELG_OK;
 }
 extern "C" void elg_bunch_destroy(elg_bunch* b) {
-    if (b) cudaStreamSynchronize(b->stream);
+    if (b) {
+        cudaStreamSynchronize(b->stream);
+        b->prof_drain();
+        for (cudaEvent_t e : b->prof_pool) cudaEventDestroy(e);
+    }
     delete b;
+}
+
+extern "C" int32_t elg_profile_enable(elg_bunch* b, int32_t on) {
+    if (!b) return fail(ELG_EINVAL, "elg_profile_enable: NULL bunch");
+    b->prof_on = on != 0;
+    return ELG_OK;
+}
+
+extern "C" int32_t elg_profile_read(elg_bunch* b, int64_t* h_launches, double* h_ms) {
+    if (!b || !h_launches || !h_ms) return fail(ELG_EINVAL, "elg_profile_read: bad arguments");
+    ELG_CK(cudaStreamSynchronize(b->stream));
+    b->prof_drain();
+    for (int k = 0; k < ELG_K_COUNT; k++) {
+        h_launches[k] = b->prof_launches[k]; h_ms[k] = b->prof_ms[k];
+        b->prof_launches[k] = 0; b->prof_ms[k] = 0.0;
+    }
+    return ELG_OK;
 }
 
 extern "C" int32_t elg_bunch_upload(elg_bunch* b, const double* const h_coords[6], const int64_t* h_ids) {
@@ -403,7 +467,10 @@ struct Tracker {
         }
         const int grid = b->grid_chain[MAXOPS == kMaxOpsLarge ? 1 : 0][COMPACT ? 1 : 0];
         if (want_mm) mm_grid = grid;
-        chain_kernel<MAXOPS, COMPACT><<<grid, kBlock, 0, b->stream>>>(a);
+        {
+            ProfScope ps(b, COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN);
+            chain_kernel<MAXOPS, COMPACT><<<grid, kBlock, 0, b->stream>>>(a);
+        }
         check(cudaGetLastError(), "chain_kernel launch");
         if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
     }
@@ -448,7 +515,10 @@ struct Tracker {
         for (int k = 0; k < 6; k++) m.src[k] = b->coord(b->cur_buf, k);
         m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial;
         m.record = b->records + 43 * b->rec_count;
-        moments_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(m);
+        {
+            ProfScope ps(b, ELG_K_MOMENTS);
+            moments_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(m);
+        }
         check(cudaGetLastError(), "moments_kernel launch");
         b->rec_count++;
     }
@@ -481,13 +551,19 @@ struct Tracker {
             w.mode = e.window; w.nb = e.nb; w.t_lo_rel = e.t_lo_rel;
             w.dt_in = (e.window == ELG_WIN_AUTO_TABLE) ? e.dt_table : e.dt;
             w.t_design = s_here * b->inv_bc; w.inv_bc = b->inv_bc; w.counts = b->counts;
-            window_kernel<<<1, kBlock, 0, b->stream>>>(w);
+            {
+                ProfScope ps(b, ELG_K_WINDOW);
+                window_kernel<<<1, kBlock, 0, b->stream>>>(w);
+            }
             check(cudaGetLastError(), "window_kernel launch");
             HistArgs h;
             h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1;
             h.inv_bc = b->inv_bc; h.t_lo = 0; h.inv_dt = 0; h.nb = e.nb; h.counts = b->counts;
             h.aggregate = b->hist_aggregate < 0 ? 0 : b->hist_aggregate;
-            hist_kernel<<<b->grid_hist, kBlock, kHistSmemBins * 4, b->stream>>>(h);
+            {
+                ProfScope ps(b, ELG_K_HIST);
+                hist_kernel<<<b->grid_hist, kBlock, kHistSmemBins * 4, b->stream>>>(h);
+            }
             check(cudaGetLastError(), "hist_kernel launch");
             stage_out_hist(e.nb);
         } else if (o) { o->window_written++; o->hist_written += e.nb; }
@@ -500,11 +576,17 @@ struct Tracker {
             const ResConst& r = bl->res[k];
             wa.kloss = r.kloss; wa.alpha = r.alpha; wa.wbar = r.wbar; wa.ratio = r.ratio;
             wa.table = b->table + bl->table_off[k]; wa.n_table = e.n_table; wa.dt_table = e.dt_table; wa.W = b->W;
-            wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
+            {
+                ProfScope ps(b, ELG_K_WAKE_SAMPLES);
+                wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
+            }
             check(cudaGetLastError(), "wake_samples_kernel launch");
             ConvArgs cv;
             cv.counts = b->counts; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro; cv.V = b->V;
-            conv_kernel<<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
+            {
+                ProfScope ps(b, ELG_K_CONV);
+                conv_kernel<<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
+            }
             check(cudaGetLastError(), "conv_kernel launch");
             if (o && o->V_out && o->V_written + e.nb <= o->V_capacity)
                 check(cudaMemcpyAsync(o->V_out + o->V_written, b->V, (size_t)e.nb * 8, cudaMemcpyDeviceToHost, b->stream), "V D2H");

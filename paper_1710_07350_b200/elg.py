@@ -32,8 +32,10 @@ EXPORTS = (
     "elg_beamline_s_design", "elg_beamline_launches_per_turn", "elg_workspace_bytes",
     "elg_bunch_create", "elg_bunch_destroy", "elg_bunch_upload", "elg_bunch_rewind", "elg_track",
     "elg_moments", "elg_lost", "elg_n_alive", "elg_bunch_read", "elg_bunch_device_array",
+    "elg_profile_enable", "elg_profile_read",
     "elg_dbg_histogram", "elg_dbg_wake_samples", "elg_dbg_convolve", "elg_dbg_kick",
 )
+KERNEL_KINDS = ("chain", "chain_compact", "window", "hist", "wake_samples", "conv", "moments")
 
 
 class ElgError(RuntimeError):
@@ -108,6 +110,8 @@ def lib():
     L.elg_n_alive.argtypes = [vp, _i64p]; L.elg_n_alive.restype = C.c_int32
     L.elg_bunch_read.argtypes = [vp, v6, _i64p, C.c_int64]; L.elg_bunch_read.restype = C.c_int32
     L.elg_bunch_device_array.argtypes = [vp, C.c_int32, C.POINTER(vp)]; L.elg_bunch_device_array.restype = C.c_int32
+    L.elg_profile_enable.argtypes = [vp, C.c_int32]; L.elg_profile_enable.restype = C.c_int32
+    L.elg_profile_read.argtypes = [vp, _i64p, _dp]; L.elg_profile_read.restype = C.c_int32
     L.elg_dbg_histogram.argtypes = [vp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32, vp, vp]
     L.elg_dbg_histogram.restype = C.c_int32
     L.elg_dbg_wake_samples.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
@@ -351,6 +355,17 @@ class Bunch:
             if rc not in (OK, ECAPACITY):
                 _ck(rc)
         return ids, turn, elem, co
+
+    def profile(self, on: bool = True) -> None:
+        """elg_profile_enable: bracket every kernel launch of this bunch with CUDA events."""
+        _ck(lib().elg_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self) -> dict:
+        """elg_profile_read: {kernel kind: (launches, summed device ms)} since the last read."""
+        n = len(KERNEL_KINDS)
+        cnt = np.zeros(n, dtype=np.int64); ms = np.zeros(n, dtype=np.float64)
+        _ck(lib().elg_profile_read(self._h, _p(cnt, _i64p), _p(ms)))
+        return {k: (int(cnt[i]), float(ms[i])) for i, k in enumerate(KERNEL_KINDS)}
 
     def device_array(self, c: int):
         """torch view of coordinate c (0..5; 6 = IDs as int64) of the CURRENT store, live prefix not applied."""
