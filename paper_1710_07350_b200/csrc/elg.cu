@@ -33,6 +33,7 @@ constexpr double kCLight = 299792458.0;                 // m/s
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr int kMaxOpsSmall = 8;
 constexpr int kMaxOpsLarge = 80;                        // 80 x 42 x 8 B = 26.9 KB of kernel parameters
+constexpr int kMatricesForP4 = 3;                       // runs with >= 3 MATRIX maps use 4 particles per thread
 constexpr int kMaxGrid = 4096;
 constexpr long long kRecCap = 2048;                     // device ring of moment records
 constexpr int kNbDefault = 65536;
@@ -91,7 +92,8 @@ struct elg_bunch {
     long long rec_count = 0;                            // records in the device ring
     // launch geometry
     int sms = 0;
-    int grid_chain[2][2] = {{0, 0}, {0, 0}};            // [large][compact]
+    int grid_chain[3][2] = {{0, 0}, {0, 0}, {0, 0}};    // [variant][compact]; variants: <8 ops, P=2>, <8, P=4>, <80, P=4>
+    int force_p = 0;                                    // ELG_CHAIN_P = 2 | 4 overrides the planner's choice
     int grid_hist = 0, grid_mom = 0;
     int hist_aggregate = 0;
     // optional per-kernel event timing (elg_profile_*)
@@ -352,16 +354,20 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     b->lost_v = (double*)(w + L.off_lost_v);
     b->sms = sms;
     int32_t rc = ELG_OK;
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, false>, sms, 0, &b->grid_chain[0][0]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, true>, sms, 0, &b->grid_chain[0][1]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsLarge, false>, sms, 0, &b->grid_chain[1][0]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsLarge, true>, sms, 0, &b->grid_chain[1][1]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, false, 2>, sms, 0, &b->grid_chain[0][0]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, true, 2>, sms, 0, &b->grid_chain[0][1]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, false, 4>, sms, 0, &b->grid_chain[1][0]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, true, 4>, sms, 0, &b->grid_chain[1][1]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsLarge, false, 4>, sms, 0, &b->grid_chain[2][0]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsLarge, true, 4>, sms, 0, &b->grid_chain[2][1]);
     if (rc == ELG_OK) rc = hist_setup_once();
     if (rc == ELG_OK) rc = grid_for(hist_kernel, sms, kHistSmemBins * 4, &b->grid_hist);
     if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, &b->grid_mom);
     if (rc != ELG_OK) { delete b; return rc; }
     const char* agg = std::getenv("ELG_HIST_AGGREGATE");
     b->hist_aggregate = agg ? std::atoi(agg) : -1;                 // -1: automatic
+    const char* fp = std::getenv("ELG_CHAIN_P");
+    b->force_p = fp ? std::atoi(fp) : 0;
     cudaError_t ce = cudaMemsetAsync(b->tile_status, 0, (b->stride / kTile + 2) * 8, b->stream);
     if (ce != cudaSuccess) { delete b; return fail(ELG_ECUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(ce)); }
     rc = elg_bunch_rewind(b);
@@ -439,7 +445,7 @@ struct Tracker {
         if (e != cudaSuccess && rc == ELG_OK) rc = fail(ELG_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
     }
 
-    template <int MAXOPS, bool COMPACT>
+    template <int MAXOPS, bool COMPACT, int P>
     void launch_chain(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm, unsigned rmask, unsigned wmask) {
         count();
         if (!b) return;
@@ -465,11 +471,11 @@ struct Tracker {
             a.type[k] = pending[k].type;
             std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
         }
-        const int grid = b->grid_chain[MAXOPS == kMaxOpsLarge ? 1 : 0][COMPACT ? 1 : 0];
+        const int grid = b->grid_chain[MAXOPS == kMaxOpsLarge ? 2 : (P == 4 ? 1 : 0)][COMPACT ? 1 : 0];
         if (want_mm) mm_grid = grid;
         {
             ProfScope ps(b, COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN);
-            chain_kernel<MAXOPS, COMPACT><<<grid, kBlock, 0, b->stream>>>(a);
+            chain_kernel<MAXOPS, COMPACT, P><<<grid, kBlock, 0, b->stream>>>(a);
         }
         check(cudaGetLastError(), "chain_kernel launch");
         if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
@@ -490,10 +496,18 @@ struct Tracker {
         if (want_mm) rmask |= 0x10;
         const bool large = pending.size() > (size_t)kMaxOpsSmall;
         const bool compact = ap_type != AP_NONE;
-        if (large) { if (compact) launch_chain<kMaxOpsLarge, true>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask);
-                     else launch_chain<kMaxOpsLarge, false>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask); }
-        else       { if (compact) launch_chain<kMaxOpsSmall, true>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask);
-                     else launch_chain<kMaxOpsSmall, false>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask); }
+        // particles per thread: 2 while the run is HBM-bound; 4 once it holds enough MATRIX maps for the
+        // coefficient fetches (one per 2 particles) to matter
+        int n_mat = 0;
+        for (const HostOp& op : pending) n_mat += op.type == OP_MATRIX;
+        bool p4 = n_mat >= kMatricesForP4;
+        if (b && b->force_p == 2) p4 = false;
+        if (b && b->force_p == 4) p4 = true;
+#define ELG_LAUNCH(M, C, PP) launch_chain<M, C, PP>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
+        if (large)   { if (compact) ELG_LAUNCH(kMaxOpsLarge, true, 4); else ELG_LAUNCH(kMaxOpsLarge, false, 4); }
+        else if (p4) { if (compact) ELG_LAUNCH(kMaxOpsSmall, true, 4); else ELG_LAUNCH(kMaxOpsSmall, false, 4); }
+        else         { if (compact) ELG_LAUNCH(kMaxOpsSmall, true, 2); else ELG_LAUNCH(kMaxOpsSmall, false, 2); }
+#undef ELG_LAUNCH
         if (compact || (wmask & 0x10)) mm_valid = want_mm;
         else mm_valid = mm_valid || want_mm;
         pending.clear();

@@ -109,20 +109,22 @@ __device__ __forceinline__ int bin_of(double s, double inv_bc, double t_lo, doub
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Element maps on kP particles held in registers.  Coefficients come straight from the kernel parameter
+// Element maps on P particles held in registers.  Coefficients come straight from the kernel parameter
 // constant bank (uniform operands of DFMA), so a MATRIX costs 42 DFMA per particle and no LSU traffic.
+// One coefficient fetch (LDCU) feeds P DFMAs: P = 4 keeps the fp64 pipe, not the constant path, the
+// limiter of long runs (profiles/r01a_first_path.md).
 // ---------------------------------------------------------------------------------------------------
-template <int MAXOPS>
-__device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v)[kP][6]) {
+template <int MAXOPS, int P>
+__device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
     for (int op = 0; op < a.c.n_ops; op++) {
         const double* c = a.coef[op];
         const int ty = a.type[op];
         if (ty == OP_MATRIX) {                                   // G3
-            double w[kP][6];
+            double w[P][6];
 #pragma unroll
             for (int r = 0; r < 6; r++) {
 #pragma unroll
-                for (int p = 0; p < kP; p++) {
+                for (int p = 0; p < P; p++) {
                     double acc = c[36 + r];
 #pragma unroll
                     for (int cc = 0; cc < 6; cc++) acc = fma(c[6 * r + cc], v[p][cc], acc);
@@ -130,13 +132,13 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
                 }
             }
 #pragma unroll
-            for (int p = 0; p < kP; p++)
+            for (int p = 0; p < P; p++)
 #pragma unroll
                 for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
         } else if (ty == OP_DRIFT) {                             // PAPER.md:75-77, G2
             const double L = c[0];
 #pragma unroll
-            for (int p = 0; p < kP; p++) {
+            for (int p = 0; p < P; p++) {
                 v[p][0] = fma(v[p][1], L, v[p][0]);
                 v[p][2] = fma(v[p][3], L, v[p][2]);
                 double u = fma(v[p][1], v[p][1], 1.0);
@@ -146,7 +148,7 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
         } else if (ty == OP_RFKICK) {                            // G8
             const double A = c[0], omega = c[1], phi0 = c[2], s_ref = c[3], inv_bc = c[4];
 #pragma unroll
-            for (int p = 0; p < kP; p++) {
+            for (int p = 0; p < P; p++) {
                 const double tau = (v[p][4] - s_ref) * inv_bc;
                 const double arg = fma(omega, tau, phi0);
                 v[p][5] = fma(A, sin(arg), v[p][5]);
@@ -156,7 +158,7 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
             const double t_lo = a.c.st->win[0], inv_dt = a.c.st->win[2];
             const int nb = a.c.nb;
 #pragma unroll
-            for (int p = 0; p < kP; p++) {
+            for (int p = 0; p < P; p++) {
                 double u0;
                 const int b = bin_of(v[p][4], inv_bc, t_lo, inv_dt, nb, &u0);
                 if (b < 0) continue;
@@ -198,96 +200,131 @@ __device__ __forceinline__ unsigned long long pack_status(unsigned int epoch, un
 // chain_kernel: one launch applies a RUN of consecutive elements to every live particle: each
 // coordinate is loaded once (128-bit), carried in registers through all maps and stored once
 // (north_star part 1; the paper launches one kernel per element).
+//
+// Work decomposition: a tile is kBlock * P consecutive particles made of H = P/2 sub-tiles of
+// 2 * kBlock; thread t owns particles 2t, 2t+1 of every sub-tile (one 128-bit access per coordinate and
+// sub-tile, warp accesses are 512 contiguous bytes), so a warp owns H "chunks" of 64 consecutive particles.
+//
 // COMPACT: the run ends in an aperture; survivors are written out of place in their original order and
 // the lost particles are appended to the lost log in position order (north_star part 2), with the
-// survivor ranks from a single-pass decoupled look-back scan over tiles.  Persistent grid.
+// survivor ranks from a single-pass decoupled look-back scan over tiles.  Every warp partitions each of
+// its chunks in shared memory (survivors first, lost after, both in order) and writes both parts with
+// coalesced stores: a chunk's survivors are contiguous in the destination, its lost in the log.
 // ---------------------------------------------------------------------------------------------------
-template <int MAXOPS, bool COMPACT>
-__global__ void __launch_bounds__(kBlock) chain_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+template <int MAXOPS, bool COMPACT, int P>
+__global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+    constexpr int H = P / 2;                    // sub-tiles per tile
+    constexpr int kSub = 2 * kBlock;            // particles per sub-tile
+    constexpr int kTileP = kBlock * P;
     const ChainCommon& c = a.c;
     const long long n = c.st->n_alive[c.cur];
-    const long long n_tiles = (n + kTile - 1) / kTile;
+    const long long n_tiles = (n + kTileP - 1) / kTileP;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double mn = INFINITY, mx = -INFINITY;
 
-    __shared__ int s_warp[kWarps];
+    __shared__ int s_chunk[COMPACT ? H * kWarps : 1];          // survivors per chunk, chunk = h * kWarps + warp
     __shared__ long long s_base;
     __shared__ long long s_tile;
+    __shared__ double s_stage[COMPACT ? kWarps : 1][7][64];    // per-warp partition buffer: 6 coordinates + ID
 
     long long tile = blockIdx.x;
+    if (COMPACT) {                              // dynamic tile order: predecessors are always running
+        if (threadIdx.x == 0) s_tile = (long long)atomicAdd(&c.st->tile_counter, 1u);
+        __syncthreads();
+    }
     while (true) {
-        if (COMPACT) {                          // dynamic tile order: predecessors are always running
-            if (threadIdx.x == 0) s_tile = (long long)atomicAdd(&c.st->tile_counter, 1u);
-            __syncthreads();
-            tile = s_tile;
-        }
+        if (COMPACT) tile = s_tile;
         if (tile >= n_tiles) break;
-        const long long i0 = tile * kTile + (long long)threadIdx.x * kP;
-        double v[kP][6];
-        long long id[kP];
-        const bool full = (i0 + kP <= n);
+        const long long t0 = tile * kTileP + (long long)threadIdx.x * 2;
+        double v[P][6];
+        long long id[P];
         const unsigned int rmask = COMPACT ? 0x3Fu : c.rmask;
 #pragma unroll
-        for (int cc = 0; cc < 6; cc++) {
-            v[0][cc] = 0.0; v[1][cc] = 0.0;
-            if (rmask & (1u << cc)) {
+        for (int h = 0; h < H; h++) {
+            const long long i0 = t0 + (long long)h * kSub;
+            const bool full = (i0 + 2 <= n);
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) {
+                v[2 * h][cc] = 0.0; v[2 * h + 1][cc] = 0.0;
+                if (rmask & (1u << cc)) {
+                    if (full) {
+                        const double2 t = ld_stream2(c.src[cc] + i0);
+                        v[2 * h][cc] = t.x; v[2 * h + 1][cc] = t.y;
+                    } else if (i0 < n) {
+                        v[2 * h][cc] = ld_stream1(c.src[cc] + i0);
+                    }
+                }
+            }
+            if (COMPACT) {
+                id[2 * h] = 0; id[2 * h + 1] = 0;
                 if (full) {
-                    const double2 t = ld_stream2(c.src[cc] + i0);
-                    v[0][cc] = t.x; v[1][cc] = t.y;
+                    const longlong2 t = *reinterpret_cast<const longlong2*>(c.id_src + i0);
+                    id[2 * h] = t.x; id[2 * h + 1] = t.y;
                 } else if (i0 < n) {
-                    v[0][cc] = ld_stream1(c.src[cc] + i0);
+                    id[2 * h] = c.id_src[i0];
                 }
             }
         }
-        if (COMPACT) {
-            id[0] = 0; id[1] = 0;
-            if (full) {
-                const longlong2 t = *reinterpret_cast<const longlong2*>(c.id_src + i0);
-                id[0] = t.x; id[1] = t.y;
-            } else if (i0 < n) {
-                id[0] = c.id_src[i0];
-            }
-        }
 
-        apply_ops(a, v);
+        apply_ops<MAXOPS, P>(a, v);
 
         if (!COMPACT) {
 #pragma unroll
-            for (int cc = 0; cc < 6; cc++) {
-                if (c.wmask & (1u << cc)) {
-                    if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[0][cc], v[1][cc]);
-                    else if (i0 < n) c.dst[cc][i0] = v[0][cc];
+            for (int h = 0; h < H; h++) {
+                const long long i0 = t0 + (long long)h * kSub;
+                const bool full = (i0 + 2 <= n);
+#pragma unroll
+                for (int cc = 0; cc < 6; cc++) {
+                    if (c.wmask & (1u << cc)) {
+                        if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[2 * h][cc], v[2 * h + 1][cc]);
+                        else if (i0 < n) c.dst[cc][i0] = v[2 * h][cc];
+                    }
                 }
-            }
-            if (c.want_minmax) {
-                if (i0 < n) { mn = fmin(mn, v[0][4]); mx = fmax(mx, v[0][4]); }
-                if (full) { mn = fmin(mn, v[1][4]); mx = fmax(mx, v[1][4]); }
+                if (c.want_minmax) {
+                    if (i0 < n) { mn = fmin(mn, v[2 * h][4]); mx = fmax(mx, v[2 * h][4]); }
+                    if (full) { mn = fmin(mn, v[2 * h + 1][4]); mx = fmax(mx, v[2 * h + 1][4]); }
+                }
             }
             tile += gridDim.x;
         } else {
-            bool valid[kP], surv[kP];
+            bool valid[P], surv[P];
+            int cnt[H];
+            int packed = 0;                                    // 16 bits per sub-tile (a chunk holds <= 64)
 #pragma unroll
-            for (int p = 0; p < kP; p++) {
-                valid[p] = (i0 + p < n);
-                surv[p] = valid[p] && survives(c.ap_type, c.ap_x, c.ap_y, v[p][0], v[p][2]);
+            for (int h = 0; h < H; h++) {
+#pragma unroll
+                for (int q = 0; q < 2; q++) {
+                    const int p = 2 * h + q;
+                    valid[p] = (t0 + (long long)h * kSub + q < n);
+                    surv[p] = valid[p] && survives(c.ap_type, c.ap_x, c.ap_y, v[p][0], v[p][2]);
+                }
+                cnt[h] = (int)surv[2 * h] + (int)surv[2 * h + 1];
+                packed |= cnt[h] << (16 * h);
             }
-            const int cnt = (int)surv[0] + (int)surv[1];
-            int inc = cnt;                                     // warp inclusive scan
+            int inc = packed;                                  // warp inclusive scan of all sub-tiles at once
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
                 const int t = __shfl_up_sync(0xffffffffu, inc, d);
                 if (lane >= d) inc += t;
             }
-            if (lane == 31) s_warp[wid] = inc;
-            __syncthreads();
-            int woff = 0, btotal = 0;
+            if (lane == 31) {
 #pragma unroll
-            for (int w = 0; w < kWarps; w++) {
-                const int x = s_warp[w];
-                if (w < wid) woff += x;
+                for (int h = 0; h < H; h++) s_chunk[h * kWarps + wid] = (inc >> (16 * h)) & 0xffff;
+            }
+            __syncthreads();                                   // (A) chunk counts visible; everyone has read s_tile
+            int coff[H], ccnt[H], btotal = 0;                  // survivors in earlier chunks of the tile / in mine
+#pragma unroll
+            for (int h = 0; h < H; h++) { coff[h] = 0; ccnt[h] = 0; }
+#pragma unroll
+            for (int ch = 0; ch < H * kWarps; ch++) {
+                const int x = s_chunk[ch];
+#pragma unroll
+                for (int h = 0; h < H; h++) {
+                    if (ch < h * kWarps + wid) coff[h] += x;
+                    if (ch == h * kWarps + wid) ccnt[h] = x;
+                }
                 btotal += x;
             }
-            const int excl_local = woff + inc - cnt;
             if (wid == 0) {                                    // decoupled look-back over earlier tiles
                 long long excl = 0;
                 if (tile > 0) {
@@ -314,6 +351,9 @@ __global__ void __launch_bounds__(kBlock) chain_kernel(const __grid_constant__ C
                 if (lane == 0) {
                     st_relaxed(c.tile_status + tile, pack_status(c.epoch, kFlagP, (unsigned long long)(excl + btotal)));
                     s_base = excl;
+                    // next ticket, taken as late as possible: a tile's prefix must follow its ticket closely or
+                    // the look-back windows of its successors grow (they are sized by tickets issued meanwhile)
+                    s_tile = (long long)atomicAdd(&c.st->tile_counter, 1u);
                     if (tile == n_tiles - 1) {                 // the last tile knows the totals
                         const long long ns = excl + btotal;
                         c.st->n_alive[c.cur ^ 1] = ns;
@@ -321,28 +361,55 @@ __global__ void __launch_bounds__(kBlock) chain_kernel(const __grid_constant__ C
                     }
                 }
             }
-            __syncthreads();
-            long long pos = s_base + excl_local;               // rank among survivors = destination
+            __syncthreads();                                   // (B) s_base and the next ticket visible
+            const long long tile_base = s_base;                // survivors before this tile
             const long long lost_base = c.st->n_lost[c.cur];
+            double (*stg)[64] = s_stage[wid];
 #pragma unroll
-            for (int p = 0; p < kP; p++) {
-                if (surv[p]) {
+            for (int h = 0; h < H; h++) {
+                const long long chunk0 = tile * kTileP + (long long)h * kSub + wid * 64;   // first particle of my chunk
+                long long nv = n - chunk0;                                                  // valid particles in it
+                nv = nv < 0 ? 0 : (nv > 64 ? 64 : nv);
+                const int nvalid = (int)nv;
+                const int nsurv = ccnt[h];
+                const long long dst0 = tile_base + coff[h];                                 // rank of the chunk's first survivor
+                const long long lost0 = lost_base + (chunk0 - dst0);                        // lost before the chunk = index - survivors before
+                int e = ((inc >> (16 * h)) & 0xffff) - cnt[h];                              // survivors before me in the chunk
 #pragma unroll
-                    for (int cc = 0; cc < 6; cc++) c.dst[cc][pos] = v[p][cc];
-                    c.id_dst[pos] = id[p];
-                    if (c.want_minmax) { mn = fmin(mn, v[p][4]); mx = fmax(mx, v[p][4]); }
-                    pos++;
-                } else if (valid[p]) {
-                    const long long lpos = lost_base + (i0 + p) - pos;   // lost before me = index - survivors before me
-                    if (lpos < c.lost_cap) {
-                        c.lost_id[lpos] = id[p];
-                        c.lost_te[lpos] = c.te_code;
+                for (int q = 0; q < 2; q++) {
+                    const int p = 2 * h + q;
+                    // stable partition of the chunk: survivors to [0, nsurv), lost to [nsurv, nvalid), each in order
+                    const int slot = surv[p] ? e : nsurv + (2 * lane + q - e);
+                    if (valid[p]) {
 #pragma unroll
-                        for (int cc = 0; cc < 6; cc++) c.lost_v[cc * c.lost_cap + lpos] = v[p][cc];
+                        for (int cc = 0; cc < 6; cc++) stg[cc][slot] = v[p][cc];
+                        stg[6][slot] = __longlong_as_double(id[p]);
+                    }
+                    if (surv[p]) {
+                        e++;
+                        if (c.want_minmax) { mn = fmin(mn, v[p][4]); mx = fmax(mx, v[p][4]); }
                     }
                 }
+                __syncwarp();
+#pragma unroll
+                for (int q = 0; q < 2; q++) {
+                    const int k = lane + 32 * q;
+                    if (k < nsurv) {
+#pragma unroll
+                        for (int cc = 0; cc < 6; cc++) c.dst[cc][dst0 + k] = stg[cc][k];
+                        c.id_dst[dst0 + k] = __double_as_longlong(stg[6][k]);
+                    } else if (k < nvalid) {
+                        const long long lpos = lost0 + (k - nsurv);
+                        if (lpos < c.lost_cap) {
+                            c.lost_id[lpos] = __double_as_longlong(stg[6][k]);
+                            c.lost_te[lpos] = c.te_code;
+#pragma unroll
+                            for (int cc = 0; cc < 6; cc++) c.lost_v[cc * c.lost_cap + lpos] = stg[cc][k];
+                        }
+                    }
+                }
+                __syncwarp();                                  // staging buffer reuse by the next sub-tile / tile
             }
-            __syncthreads();                                   // s_tile / s_warp / s_base reuse
         }
     }
 
