@@ -92,7 +92,7 @@ struct elg_bunch {
     long long rec_count = 0;                            // records in the device ring
     // launch geometry
     int sms = 0;
-    int grid_chain[3][2] = {{0, 0}, {0, 0}, {0, 0}};    // [variant][compact]; variants: <8 ops, P=2>, <8, P=4>, <80, P=4>
+    int grid_chain[3][2] = {{0, 0}, {0, 0}, {0, 0}};    // [variant][compact]; variants: <8 ops, P=2>, <8, P=4>, long run <80, P=6>
     int force_p = 0;                                    // ELG_CHAIN_P = 2 | 4 overrides the planner's choice
     int grid_hist = 0, grid_mom = 0;
     int hist_aggregate = 0;
@@ -195,6 +195,16 @@ int32_t device_sms(int* sms) {
     int dev = 0;
     ELG_CK(cudaGetDevice(&dev));
     ELG_CK(cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, dev));
+    return ELG_OK;
+}
+
+int32_t long_setup_once() {
+    static bool done = false;
+    if (!done) {
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    chain_long_smem_bytes<kMaxOpsLarge>()));
+        done = true;
+    }
     return ELG_OK;
 }
 
@@ -358,8 +368,9 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, true, 2>, sms, 0, &b->grid_chain[0][1]);
     if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, false, 4>, sms, 0, &b->grid_chain[1][0]);
     if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, true, 4>, sms, 0, &b->grid_chain[1][1]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsLarge, false, 4>, sms, 0, &b->grid_chain[2][0]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsLarge, true, 4>, sms, 0, &b->grid_chain[2][1]);
+    if (rc == ELG_OK) rc = long_setup_once();
+    if (rc == ELG_OK) rc = grid_for(chain_long_kernel<kMaxOpsLarge>, sms, chain_long_smem_bytes<kMaxOpsLarge>(), &b->grid_chain[2][0]);
+    b->grid_chain[2][1] = b->grid_chain[2][0];
     if (rc == ELG_OK) rc = hist_setup_once();
     if (rc == ELG_OK) rc = grid_for(hist_kernel, sms, kHistSmemBins * 4, &b->grid_hist);
     if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, &b->grid_mom);
@@ -475,7 +486,10 @@ struct Tracker {
         if (want_mm) mm_grid = grid;
         {
             ProfScope ps(b, COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN);
-            chain_kernel<MAXOPS, COMPACT, P><<<grid, kBlock, 0, b->stream>>>(a);
+            if constexpr (MAXOPS == kMaxOpsLarge)
+                chain_long_kernel<MAXOPS><<<grid, kBlock, chain_long_smem_bytes<MAXOPS>(), b->stream>>>(a);
+            else
+                chain_kernel<MAXOPS, COMPACT, P><<<grid, kBlock, 0, b->stream>>>(a);
         }
         check(cudaGetLastError(), "chain_kernel launch");
         if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
@@ -485,6 +499,9 @@ struct Tracker {
     void flush(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm) {
         if (!ok()) return;
         if (ap_type == AP_NONE && pending.empty() && !want_mm) return;
+        // a long run that ends in an aperture: the maps go through the fp64-bound long-run kernel, the
+        // aperture and the compaction follow as a run of their own (112 B per particle more, rare)
+        if (ap_type != AP_NONE && pending.size() > (size_t)kMaxOpsSmall) flush(AP_NONE, 0, 0, 0, false);
         unsigned rmask = 0, wmask = 0;
         for (const HostOp& op : pending) {
             switch (op.type) {
@@ -504,7 +521,7 @@ struct Tracker {
         if (b && b->force_p == 2) p4 = false;
         if (b && b->force_p == 4) p4 = true;
 #define ELG_LAUNCH(M, C, PP) launch_chain<M, C, PP>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
-        if (large)   { if (compact) ELG_LAUNCH(kMaxOpsLarge, true, 4); else ELG_LAUNCH(kMaxOpsLarge, false, 4); }
+        if (large)   { ELG_LAUNCH(kMaxOpsLarge, false, kPL); }
         else if (p4) { if (compact) ELG_LAUNCH(kMaxOpsSmall, true, 4); else ELG_LAUNCH(kMaxOpsSmall, false, 4); }
         else         { if (compact) ELG_LAUNCH(kMaxOpsSmall, true, 2); else ELG_LAUNCH(kMaxOpsSmall, false, 2); }
 #undef ELG_LAUNCH

@@ -114,71 +114,105 @@ __device__ __forceinline__ int bin_of(double s, double inv_bc, double t_lo, doub
 // One coefficient fetch (LDCU) feeds P DFMAs: P = 4 keeps the fp64 pipe, not the constant path, the
 // limiter of long runs (profiles/r01a_first_path.md).
 // ---------------------------------------------------------------------------------------------------
+// v -> w through one MATRIX (G3): row r accumulates from C[r] over c = 0..5 with FMAs, in that order.
+template <int P>
+__device__ __forceinline__ void matrix_map(const double* __restrict__ c, const double (&v)[P][6], double (&w)[P][6]) {
+#pragma unroll
+    for (int r = 0; r < 6; r++) {
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            double acc = c[36 + r];
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) acc = fma(c[6 * r + cc], v[p][cc], acc);
+            w[p][r] = acc;
+        }
+    }
+}
+
+// the same map with the 42 coefficients fetched from shared memory 128 bits at a time (16-byte aligned block)
+template <int P>
+__device__ __forceinline__ void matrix_map_s128(const double* c, const double (&v)[P][6], double (&w)[P][6]) {
+    const double2* c2 = reinterpret_cast<const double2*>(c);
+    const double2 C01 = c2[18], C23 = c2[19], C45 = c2[20];
+    const double Cc[6] = {C01.x, C01.y, C23.x, C23.y, C45.x, C45.y};
+#pragma unroll
+    for (int r = 0; r < 6; r++) {
+        const double2 k01 = c2[3 * r], k23 = c2[3 * r + 1], k45 = c2[3 * r + 2];
+        const double k[6] = {k01.x, k01.y, k23.x, k23.y, k45.x, k45.y};
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            double acc = Cc[r];
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) acc = fma(k[cc], v[p][cc], acc);
+            w[p][r] = acc;
+        }
+    }
+}
+
+// DRIFT, RFKICK and the wake KICK, in place
+template <int P>
+__device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, const ChainCommon& cm, double (&v)[P][6]) {
+    if (ty == OP_DRIFT) {                                        // PAPER.md:75-77, G2
+        const double L = c[0];
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            v[p][0] = fma(v[p][1], L, v[p][0]);
+            v[p][2] = fma(v[p][3], L, v[p][2]);
+            double u = fma(v[p][1], v[p][1], 1.0);
+            u = fma(v[p][3], v[p][3], u);
+            v[p][4] = fma(L, sqrt(u), v[p][4]);
+        }
+    } else if (ty == OP_RFKICK) {                                // G8
+        const double A = c[0], omega = c[1], phi0 = c[2], s_ref = c[3], inv_bc = c[4];
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            const double tau = (v[p][4] - s_ref) * inv_bc;
+            const double arg = fma(omega, tau, phi0);
+            v[p][5] = fma(A, sin(arg), v[p][5]);
+        }
+    } else if (ty == OP_KICK) {                                  // G14: wake kick of the preceding WAKE
+        const double inv_bc = c[0], inv_E = c[1];
+        const double t_lo = cm.st->win[0], inv_dt = cm.st->win[2];
+        const int nb = cm.nb;
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            double u0;
+            const int b = bin_of(v[p][4], inv_bc, t_lo, inv_dt, nb, &u0);
+            if (b < 0) continue;
+            double Vt;
+            if (!cm.interp || nb < 2) {
+                Vt = __ldg(cm.V + b);
+            } else {
+                const double u = u0 - 0.5;
+                double k = floor(u);
+                if (k < 0.0) k = 0.0;
+                if (k > (double)(nb - 2)) k = (double)(nb - 2);
+                double fr = u - k;
+                if (fr < 0.0) fr = 0.0;
+                if (fr > 1.0) fr = 1.0;
+                const int ki = (int)k;
+                const double V0 = __ldg(cm.V + ki), V1 = __ldg(cm.V + ki + 1);
+                Vt = fma(fr, V1 - V0, V0);
+            }
+            v[p][5] = fma(-Vt, inv_E, v[p][5]);
+        }
+    }
+}
+
 template <int MAXOPS, int P>
 __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
     for (int op = 0; op < a.c.n_ops; op++) {
         const double* c = a.coef[op];
         const int ty = a.type[op];
-        if (ty == OP_MATRIX) {                                   // G3
+        if (ty == OP_MATRIX) {
             double w[P][6];
-#pragma unroll
-            for (int r = 0; r < 6; r++) {
-#pragma unroll
-                for (int p = 0; p < P; p++) {
-                    double acc = c[36 + r];
-#pragma unroll
-                    for (int cc = 0; cc < 6; cc++) acc = fma(c[6 * r + cc], v[p][cc], acc);
-                    w[p][r] = acc;
-                }
-            }
+            matrix_map<P>(c, v, w);
 #pragma unroll
             for (int p = 0; p < P; p++)
 #pragma unroll
                 for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
-        } else if (ty == OP_DRIFT) {                             // PAPER.md:75-77, G2
-            const double L = c[0];
-#pragma unroll
-            for (int p = 0; p < P; p++) {
-                v[p][0] = fma(v[p][1], L, v[p][0]);
-                v[p][2] = fma(v[p][3], L, v[p][2]);
-                double u = fma(v[p][1], v[p][1], 1.0);
-                u = fma(v[p][3], v[p][3], u);
-                v[p][4] = fma(L, sqrt(u), v[p][4]);
-            }
-        } else if (ty == OP_RFKICK) {                            // G8
-            const double A = c[0], omega = c[1], phi0 = c[2], s_ref = c[3], inv_bc = c[4];
-#pragma unroll
-            for (int p = 0; p < P; p++) {
-                const double tau = (v[p][4] - s_ref) * inv_bc;
-                const double arg = fma(omega, tau, phi0);
-                v[p][5] = fma(A, sin(arg), v[p][5]);
-            }
-        } else if (ty == OP_KICK) {                              // G14: wake kick of the preceding WAKE
-            const double inv_bc = c[0], inv_E = c[1];
-            const double t_lo = a.c.st->win[0], inv_dt = a.c.st->win[2];
-            const int nb = a.c.nb;
-#pragma unroll
-            for (int p = 0; p < P; p++) {
-                double u0;
-                const int b = bin_of(v[p][4], inv_bc, t_lo, inv_dt, nb, &u0);
-                if (b < 0) continue;
-                double Vt;
-                if (!a.c.interp || nb < 2) {
-                    Vt = __ldg(a.c.V + b);
-                } else {
-                    const double u = u0 - 0.5;
-                    double k = floor(u);
-                    if (k < 0.0) k = 0.0;
-                    if (k > (double)(nb - 2)) k = (double)(nb - 2);
-                    double fr = u - k;
-                    if (fr < 0.0) fr = 0.0;
-                    if (fr > 1.0) fr = 1.0;
-                    const int ki = (int)k;
-                    const double V0 = __ldg(a.c.V + ki), V1 = __ldg(a.c.V + ki + 1);
-                    Vt = fma(fr, V1 - V0, V0);
-                }
-                v[p][5] = fma(-Vt, inv_E, v[p][5]);
-            }
+        } else {
+            other_map<P>(ty, c, a.c, v);
         }
     }
 }
@@ -440,6 +474,138 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
                 c.st->tile_counter = 0;
                 c.st->done_counter = 0;
             }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// chain_long_kernel: runs of more than kMaxOpsSmall maps (cfg3: 80 MATRIX per launch), bound by the fp64
+// pipe, not by HBM.  On sm_100 every operand fetch that returns through the MIO (LDS, LDC) costs DFMA
+// issue slots (profiles/r01c_*.md: a broadcast LDS.128 costs about two DFMA), so the design minimises
+// coefficient fetches per DFMA:
+//   * kPL = 6 particles per thread: one 128-bit coefficient fetch feeds 12 DFMA;
+//   * the run's coefficients are copied once per block from the parameter bank to shared memory and read
+//     with LDS.128;
+//   * consecutive MATRIX maps are applied in pairs (v -> w -> v), so no register copy-back;
+//   * one block of 256 threads per SM (about 220 registers per thread); the next tile is prefetched into
+//     shared memory with cp.async while the current one is in the fp64 pipe, every thread copying exactly
+//     the 16-byte chunks it will read itself (no block-wide barrier in the tile loop).
+// Same arithmetic, in the same order, as chain_kernel.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kPL = 6;
+constexpr int kTileL = kBlock * kPL;
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
+    const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+template <int MAXOPS>
+constexpr int chain_long_smem_bytes() { return MAXOPS * 42 * 8 + 6 * kTileL * 8; }
+
+template <int MAXOPS>
+__global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+    constexpr int H = kPL / 2;
+    constexpr int kSub = 2 * kBlock;
+    extern __shared__ __align__(16) double sm_long[];
+    double* s_coef = sm_long;                                    // [n_ops][42]
+    double* s_tile = sm_long + MAXOPS * 42;                      // [6][H][kSub]: thread t owns doubles 2t, 2t+1 of each row
+    const ChainCommon& c = a.c;
+    const long long n = c.st->n_alive[c.cur];
+    const long long n_tiles = (n + kTileL - 1) / kTileL;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double mn = INFINITY, mx = -INFINITY;
+
+    for (int i = threadIdx.x; i < c.n_ops * 42; i += kBlock) s_coef[i] = a.coef[i / 42][i % 42];
+
+    auto prefetch = [&](long long tile) {
+        const long long t0 = tile * kTileL + (long long)threadIdx.x * 2;
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            const long long i0 = t0 + (long long)h * kSub;
+            const long long left = n - i0;
+            const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);          // zero-fill beyond the live prefix
+            const long long is = left >= 1 ? i0 : 0;
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++)
+                if (c.rmask & (1u << cc))
+                    cp_async16(s_tile + (cc * H + h) * kSub + threadIdx.x * 2, c.src[cc] + is, bytes);
+        }
+    };
+
+    long long tile = blockIdx.x;
+    if (tile < n_tiles) prefetch(tile);
+    __syncthreads();                                             // s_coef complete
+    while (tile < n_tiles) {
+        double v[kPL][6];
+        cp_async_wait_all();
+#pragma unroll
+        for (int h = 0; h < H; h++)
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) {
+                double2 t = make_double2(0.0, 0.0);
+                if (c.rmask & (1u << cc)) t = *reinterpret_cast<const double2*>(s_tile + (cc * H + h) * kSub + threadIdx.x * 2);
+                v[2 * h][cc] = t.x; v[2 * h + 1][cc] = t.y;
+            }
+        const long long next = tile + gridDim.x;
+        if (next < n_tiles) prefetch(next);                      // own slots only: already in registers
+
+        int op = 0;
+        while (op < c.n_ops) {
+            const int ty = a.type[op];
+            if (ty == OP_MATRIX && op + 1 < c.n_ops && a.type[op + 1] == OP_MATRIX) {
+                double w[kPL][6];
+                matrix_map_s128<kPL>(s_coef + 42 * op, v, w);
+                matrix_map_s128<kPL>(s_coef + 42 * (op + 1), w, v);
+                op += 2;
+            } else if (ty == OP_MATRIX) {
+                double w[kPL][6];
+                matrix_map_s128<kPL>(s_coef + 42 * op, v, w);
+#pragma unroll
+                for (int p = 0; p < kPL; p++)
+#pragma unroll
+                    for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+                op++;
+            } else {
+                other_map<kPL>(ty, s_coef + 42 * op, c, v);
+                op++;
+            }
+        }
+
+        const long long t0 = tile * kTileL + (long long)threadIdx.x * 2;
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            const long long i0 = t0 + (long long)h * kSub;
+            const bool full = (i0 + 2 <= n);
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) {
+                if (c.wmask & (1u << cc)) {
+                    if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[2 * h][cc], v[2 * h + 1][cc]);
+                    else if (i0 < n) c.dst[cc][i0] = v[2 * h][cc];
+                }
+            }
+            if (c.want_minmax) {
+                if (i0 < n) { mn = fmin(mn, v[2 * h][4]); mx = fmax(mx, v[2 * h][4]); }
+                if (full) { mn = fmin(mn, v[2 * h + 1][4]); mx = fmax(mx, v[2 * h + 1][4]); }
+            }
+        }
+        tile = next;
+    }
+
+    if (c.want_minmax) {                                         // exact min/max of s (a8)
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, d));
+            mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+        }
+        __shared__ double s_mn[kWarps], s_mx[kWarps];
+        if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
+            c.mm_partial[2 * blockIdx.x] = mn;
+            c.mm_partial[2 * blockIdx.x + 1] = mx;
         }
     }
 }
