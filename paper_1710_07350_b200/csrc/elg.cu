@@ -181,9 +181,9 @@ void caps_for(const elg_beamline* bl, long long* nb_cap, long long* table_cap) {
 }
 
 template <class K>
-int32_t grid_for(K kernel, int sms, int smem, int* out) {
+int32_t grid_for(K kernel, int sms, int smem, int threads, int* out) {
     int occ = 0;
-    ELG_CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kBlock, smem));
+    ELG_CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem));
     if (occ < 1) return fail(ELG_ECUDA, "kernel does not fit on an SM");
     long long g = (long long)occ * sms;
     if (g > kMaxGrid) g = kMaxGrid / sms * sms;
@@ -364,16 +364,16 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     b->lost_v = (double*)(w + L.off_lost_v);
     b->sms = sms;
     int32_t rc = ELG_OK;
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, false, 2>, sms, 0, &b->grid_chain[0][0]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, true, 2>, sms, 0, &b->grid_chain[0][1]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, false, 4>, sms, 0, &b->grid_chain[1][0]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, true, 4>, sms, 0, &b->grid_chain[1][1]);
     if (rc == ELG_OK) rc = long_setup_once();
-    if (rc == ELG_OK) rc = grid_for(chain_long_kernel<kMaxOpsLarge>, sms, chain_long_smem_bytes<kMaxOpsLarge>(), &b->grid_chain[2][0]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, 2>, sms, 0, kBlock, &b->grid_chain[0][0]);
+    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, 4>, sms, 0, kBlock, &b->grid_chain[1][0]);
+    if (rc == ELG_OK) rc = grid_for(compact_kernel<kMaxOpsSmall>, sms, 0, kBlock, &b->grid_chain[0][1]);
+    b->grid_chain[1][1] = b->grid_chain[0][1];
+    if (rc == ELG_OK) rc = grid_for(chain_long_kernel<kMaxOpsLarge>, sms, chain_long_smem_bytes<kMaxOpsLarge>(), kBlock, &b->grid_chain[2][0]);
     b->grid_chain[2][1] = b->grid_chain[2][0];
     if (rc == ELG_OK) rc = hist_setup_once();
-    if (rc == ELG_OK) rc = grid_for(hist_kernel, sms, kHistSmemBins * 4, &b->grid_hist);
-    if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, &b->grid_mom);
+    if (rc == ELG_OK) rc = grid_for(hist_kernel, sms, kHistSmemBins * 4, kBlock, &b->grid_hist);
+    if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, kBlock, &b->grid_mom);
     if (rc != ELG_OK) { delete b; return rc; }
     const char* agg = std::getenv("ELG_HIST_AGGREGATE");
     b->hist_aggregate = agg ? std::atoi(agg) : -1;                 // -1: automatic
@@ -488,8 +488,14 @@ struct Tracker {
             ProfScope ps(b, COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN);
             if constexpr (MAXOPS == kMaxOpsLarge)
                 chain_long_kernel<MAXOPS><<<grid, kBlock, chain_long_smem_bytes<MAXOPS>(), b->stream>>>(a);
+            else if constexpr (COMPACT)
+            {
+                void* kargs[] = {(void*)&a};                     // cooperative: every block resident (static tiles)
+                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS>, dim3(grid), dim3(kBlock), kargs, 0, b->stream),
+                      "compact_kernel cooperative launch");
+            }
             else
-                chain_kernel<MAXOPS, COMPACT, P><<<grid, kBlock, 0, b->stream>>>(a);
+                chain_kernel<MAXOPS, P><<<grid, kBlock, 0, b->stream>>>(a);
         }
         check(cudaGetLastError(), "chain_kernel launch");
         if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
@@ -522,8 +528,9 @@ struct Tracker {
         if (b && b->force_p == 4) p4 = true;
 #define ELG_LAUNCH(M, C, PP) launch_chain<M, C, PP>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
         if (large)   { ELG_LAUNCH(kMaxOpsLarge, false, kPL); }
-        else if (p4) { if (compact) ELG_LAUNCH(kMaxOpsSmall, true, 4); else ELG_LAUNCH(kMaxOpsSmall, false, 4); }
-        else         { if (compact) ELG_LAUNCH(kMaxOpsSmall, true, 2); else ELG_LAUNCH(kMaxOpsSmall, false, 2); }
+        else if (compact) { ELG_LAUNCH(kMaxOpsSmall, true, 2); }
+        else if (p4) { ELG_LAUNCH(kMaxOpsSmall, false, 4); }
+        else         { ELG_LAUNCH(kMaxOpsSmall, false, 2); }
 #undef ELG_LAUNCH
         if (compact || (wmask & 0x10)) mm_valid = want_mm;
         else mm_valid = mm_valid || want_mm;
@@ -820,7 +827,7 @@ extern "C" int32_t elg_dbg_histogram(const double* d_s, int64_t n, double inv_bc
     if (n < 0 || nb < 1 || !d_counts || (n > 0 && !d_s)) return fail(ELG_EINVAL, "elg_dbg_histogram: bad arguments");
     int grid = 0;
     { int32_t rc = hist_setup_once(); if (rc != ELG_OK) return rc; }
-    { int32_t rc = grid_for(hist_kernel, 1, kHistSmemBins * 4, &grid); if (rc != ELG_OK) return rc; }
+    { int32_t rc = grid_for(hist_kernel, 1, kHistSmemBins * 4, kBlock, &grid); if (rc != ELG_OK) return rc; }
     int sms = 0;
     { int32_t rc = device_sms(&sms); if (rc != ELG_OK) return rc; }
     ELG_CK(cudaMemsetAsync(d_counts, 0, (size_t)nb * 4, (cudaStream_t)stream));

@@ -224,7 +224,7 @@ __device__ __forceinline__ bool survives(int ap_type, double ax, double ay, doub
     return r2 <= 1.0;
 }
 
-constexpr unsigned long long kFlagA = 1ull, kFlagP = 2ull;    // aggregate / inclusive prefix available
+constexpr unsigned long long kFlagA = 1ull;                  // aggregate available
 __device__ __forceinline__ unsigned long long pack_status(unsigned int epoch, unsigned long long flag,
                                                           unsigned long long value) {
     return ((unsigned long long)epoch << 34) | (flag << 32) | value;
@@ -237,15 +237,10 @@ __device__ __forceinline__ unsigned long long pack_status(unsigned int epoch, un
 //
 // Work decomposition: a tile is kBlock * P consecutive particles made of H = P/2 sub-tiles of
 // 2 * kBlock; thread t owns particles 2t, 2t+1 of every sub-tile (one 128-bit access per coordinate and
-// sub-tile, warp accesses are 512 contiguous bytes), so a warp owns H "chunks" of 64 consecutive particles.
-//
-// COMPACT: the run ends in an aperture; survivors are written out of place in their original order and
-// the lost particles are appended to the lost log in position order (north_star part 2), with the
-// survivor ranks from a single-pass decoupled look-back scan over tiles.  Every warp partitions each of
-// its chunks in shared memory (survivors first, lost after, both in order) and writes both parts with
-// coalesced stores: a chunk's survivors are contiguous in the destination, its lost in the log.
+// sub-tile, warp accesses are 512 contiguous bytes).  Only the coordinates the run reads / writes are
+// loaded / stored (accessor masks).
 // ---------------------------------------------------------------------------------------------------
-template <int MAXOPS, bool COMPACT, int P>
+template <int MAXOPS, int P>
 __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
     constexpr int H = P / 2;                    // sub-tiles per tile
     constexpr int kSub = 2 * kBlock;            // particles per sub-tile
@@ -256,23 +251,9 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double mn = INFINITY, mx = -INFINITY;
 
-    __shared__ int s_chunk[COMPACT ? H * kWarps : 1];          // survivors per chunk, chunk = h * kWarps + warp
-    __shared__ long long s_base;
-    __shared__ long long s_tile;
-    __shared__ double s_stage[COMPACT ? kWarps : 1][7][64];    // per-warp partition buffer: 6 coordinates + ID
-
-    long long tile = blockIdx.x;
-    if (COMPACT) {                              // dynamic tile order: predecessors are always running
-        if (threadIdx.x == 0) s_tile = (long long)atomicAdd(&c.st->tile_counter, 1u);
-        __syncthreads();
-    }
-    while (true) {
-        if (COMPACT) tile = s_tile;
-        if (tile >= n_tiles) break;
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const long long t0 = tile * kTileP + (long long)threadIdx.x * 2;
         double v[P][6];
-        long long id[P];
-        const unsigned int rmask = COMPACT ? 0x3Fu : c.rmask;
 #pragma unroll
         for (int h = 0; h < H; h++) {
             const long long i0 = t0 + (long long)h * kSub;
@@ -280,7 +261,7 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
 #pragma unroll
             for (int cc = 0; cc < 6; cc++) {
                 v[2 * h][cc] = 0.0; v[2 * h + 1][cc] = 0.0;
-                if (rmask & (1u << cc)) {
+                if (c.rmask & (1u << cc)) {
                     if (full) {
                         const double2 t = ld_stream2(c.src[cc] + i0);
                         v[2 * h][cc] = t.x; v[2 * h + 1][cc] = t.y;
@@ -289,160 +270,24 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
                     }
                 }
             }
-            if (COMPACT) {
-                id[2 * h] = 0; id[2 * h + 1] = 0;
-                if (full) {
-                    const longlong2 t = *reinterpret_cast<const longlong2*>(c.id_src + i0);
-                    id[2 * h] = t.x; id[2 * h + 1] = t.y;
-                } else if (i0 < n) {
-                    id[2 * h] = c.id_src[i0];
-                }
-            }
         }
 
         apply_ops<MAXOPS, P>(a, v);
 
-        if (!COMPACT) {
 #pragma unroll
-            for (int h = 0; h < H; h++) {
-                const long long i0 = t0 + (long long)h * kSub;
-                const bool full = (i0 + 2 <= n);
+        for (int h = 0; h < H; h++) {
+            const long long i0 = t0 + (long long)h * kSub;
+            const bool full = (i0 + 2 <= n);
 #pragma unroll
-                for (int cc = 0; cc < 6; cc++) {
-                    if (c.wmask & (1u << cc)) {
-                        if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[2 * h][cc], v[2 * h + 1][cc]);
-                        else if (i0 < n) c.dst[cc][i0] = v[2 * h][cc];
-                    }
-                }
-                if (c.want_minmax) {
-                    if (i0 < n) { mn = fmin(mn, v[2 * h][4]); mx = fmax(mx, v[2 * h][4]); }
-                    if (full) { mn = fmin(mn, v[2 * h + 1][4]); mx = fmax(mx, v[2 * h + 1][4]); }
+            for (int cc = 0; cc < 6; cc++) {
+                if (c.wmask & (1u << cc)) {
+                    if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[2 * h][cc], v[2 * h + 1][cc]);
+                    else if (i0 < n) c.dst[cc][i0] = v[2 * h][cc];
                 }
             }
-            tile += gridDim.x;
-        } else {
-            bool valid[P], surv[P];
-            int cnt[H];
-            int packed = 0;                                    // 16 bits per sub-tile (a chunk holds <= 64)
-#pragma unroll
-            for (int h = 0; h < H; h++) {
-#pragma unroll
-                for (int q = 0; q < 2; q++) {
-                    const int p = 2 * h + q;
-                    valid[p] = (t0 + (long long)h * kSub + q < n);
-                    surv[p] = valid[p] && survives(c.ap_type, c.ap_x, c.ap_y, v[p][0], v[p][2]);
-                }
-                cnt[h] = (int)surv[2 * h] + (int)surv[2 * h + 1];
-                packed |= cnt[h] << (16 * h);
-            }
-            int inc = packed;                                  // warp inclusive scan of all sub-tiles at once
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const int t = __shfl_up_sync(0xffffffffu, inc, d);
-                if (lane >= d) inc += t;
-            }
-            if (lane == 31) {
-#pragma unroll
-                for (int h = 0; h < H; h++) s_chunk[h * kWarps + wid] = (inc >> (16 * h)) & 0xffff;
-            }
-            __syncthreads();                                   // (A) chunk counts visible; everyone has read s_tile
-            int coff[H], ccnt[H], btotal = 0;                  // survivors in earlier chunks of the tile / in mine
-#pragma unroll
-            for (int h = 0; h < H; h++) { coff[h] = 0; ccnt[h] = 0; }
-#pragma unroll
-            for (int ch = 0; ch < H * kWarps; ch++) {
-                const int x = s_chunk[ch];
-#pragma unroll
-                for (int h = 0; h < H; h++) {
-                    if (ch < h * kWarps + wid) coff[h] += x;
-                    if (ch == h * kWarps + wid) ccnt[h] = x;
-                }
-                btotal += x;
-            }
-            if (wid == 0) {                                    // decoupled look-back over earlier tiles
-                long long excl = 0;
-                if (tile > 0) {
-                    if (lane == 0) st_relaxed(c.tile_status + tile, pack_status(c.epoch, kFlagA, (unsigned long long)btotal));
-                    long long look = tile - 1;
-                    while (true) {
-                        const long long idx = look - lane;
-                        unsigned long long stt;
-                        bool ready;
-                        do {
-                            stt = (idx >= 0) ? ld_relaxed(c.tile_status + idx) : pack_status(c.epoch, kFlagP, 0);
-                            ready = ((unsigned int)(stt >> 34) == c.epoch) && (((stt >> 32) & 3ull) != 0);
-                        } while (__any_sync(0xffffffffu, !ready));
-                        const unsigned int pmask = __ballot_sync(0xffffffffu, ((stt >> 32) & 3ull) == kFlagP);
-                        const int first_p = pmask ? (__ffs(pmask) - 1) : 32;
-                        long long val = (lane <= first_p) ? (long long)(stt & 0xffffffffull) : 0;
-#pragma unroll
-                        for (int d = 16; d > 0; d >>= 1) val += __shfl_xor_sync(0xffffffffu, val, d);
-                        excl += val;
-                        if (pmask) break;
-                        look -= 32;
-                    }
-                }
-                if (lane == 0) {
-                    st_relaxed(c.tile_status + tile, pack_status(c.epoch, kFlagP, (unsigned long long)(excl + btotal)));
-                    s_base = excl;
-                    // next ticket, taken as late as possible: a tile's prefix must follow its ticket closely or
-                    // the look-back windows of its successors grow (they are sized by tickets issued meanwhile)
-                    s_tile = (long long)atomicAdd(&c.st->tile_counter, 1u);
-                    if (tile == n_tiles - 1) {                 // the last tile knows the totals
-                        const long long ns = excl + btotal;
-                        c.st->n_alive[c.cur ^ 1] = ns;
-                        c.st->n_lost[c.cur ^ 1] = c.st->n_lost[c.cur] + (n - ns);
-                    }
-                }
-            }
-            __syncthreads();                                   // (B) s_base and the next ticket visible
-            const long long tile_base = s_base;                // survivors before this tile
-            const long long lost_base = c.st->n_lost[c.cur];
-            double (*stg)[64] = s_stage[wid];
-#pragma unroll
-            for (int h = 0; h < H; h++) {
-                const long long chunk0 = tile * kTileP + (long long)h * kSub + wid * 64;   // first particle of my chunk
-                long long nv = n - chunk0;                                                  // valid particles in it
-                nv = nv < 0 ? 0 : (nv > 64 ? 64 : nv);
-                const int nvalid = (int)nv;
-                const int nsurv = ccnt[h];
-                const long long dst0 = tile_base + coff[h];                                 // rank of the chunk's first survivor
-                const long long lost0 = lost_base + (chunk0 - dst0);                        // lost before the chunk = index - survivors before
-                int e = ((inc >> (16 * h)) & 0xffff) - cnt[h];                              // survivors before me in the chunk
-#pragma unroll
-                for (int q = 0; q < 2; q++) {
-                    const int p = 2 * h + q;
-                    // stable partition of the chunk: survivors to [0, nsurv), lost to [nsurv, nvalid), each in order
-                    const int slot = surv[p] ? e : nsurv + (2 * lane + q - e);
-                    if (valid[p]) {
-#pragma unroll
-                        for (int cc = 0; cc < 6; cc++) stg[cc][slot] = v[p][cc];
-                        stg[6][slot] = __longlong_as_double(id[p]);
-                    }
-                    if (surv[p]) {
-                        e++;
-                        if (c.want_minmax) { mn = fmin(mn, v[p][4]); mx = fmax(mx, v[p][4]); }
-                    }
-                }
-                __syncwarp();
-#pragma unroll
-                for (int q = 0; q < 2; q++) {
-                    const int k = lane + 32 * q;
-                    if (k < nsurv) {
-#pragma unroll
-                        for (int cc = 0; cc < 6; cc++) c.dst[cc][dst0 + k] = stg[cc][k];
-                        c.id_dst[dst0 + k] = __double_as_longlong(stg[6][k]);
-                    } else if (k < nvalid) {
-                        const long long lpos = lost0 + (k - nsurv);
-                        if (lpos < c.lost_cap) {
-                            c.lost_id[lpos] = __double_as_longlong(stg[6][k]);
-                            c.lost_te[lpos] = c.te_code;
-#pragma unroll
-                            for (int cc = 0; cc < 6; cc++) c.lost_v[cc * c.lost_cap + lpos] = stg[cc][k];
-                        }
-                    }
-                }
-                __syncwarp();                                  // staging buffer reuse by the next sub-tile / tile
+            if (c.want_minmax) {
+                if (i0 < n) { mn = fmin(mn, v[2 * h][4]); mx = fmax(mx, v[2 * h][4]); }
+                if (full) { mn = fmin(mn, v[2 * h + 1][4]); mx = fmax(mx, v[2 * h + 1][4]); }
             }
         }
     }
@@ -460,20 +305,6 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
             for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
             c.mm_partial[2 * blockIdx.x] = mn;
             c.mm_partial[2 * blockIdx.x + 1] = mx;
-        }
-    }
-    if (COMPACT) {                                             // last block out resets the counters
-        if (threadIdx.x == 0) {
-            __threadfence();
-            const unsigned int d = atomicAdd(&c.st->done_counter, 1u);
-            if (d == gridDim.x - 1) {
-                if (n_tiles == 0) {
-                    c.st->n_alive[c.cur ^ 1] = 0;
-                    c.st->n_lost[c.cur ^ 1] = c.st->n_lost[c.cur];
-                }
-                c.st->tile_counter = 0;
-                c.st->done_counter = 0;
-            }
         }
     }
 }
@@ -499,7 +330,14 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int
     const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(src_bytes) : "memory");
 }
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc, int src_bytes) {
+    const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gsrc), "r"(src_bytes) : "memory");
+}
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <int MAXOPS>
 constexpr int chain_long_smem_bytes() { return MAXOPS * 42 * 8 + 6 * kTileL * 8; }
@@ -607,6 +445,209 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
             c.mm_partial[2 * blockIdx.x] = mn;
             c.mm_partial[2 * blockIdx.x + 1] = mx;
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// compact_kernel: a run of maps that ends in an aperture (a6) followed by the stable stream compaction
+// (a7; north_star part 2): survivors are written out of place in their original order, lost particles
+// are appended to the lost log in position order.  Single pass over HBM: survivor ranks come from a
+// decoupled look-back scan over 512-particle tiles.  The grid is persistent and launched cooperatively
+// (every block resident), tiles are dealt round-robin, so a tile's predecessors always make progress.
+//
+// What made the first version latency-bound (profiles/r01b: 37 % of the HBM peak, 10 us per tile) and
+// what this one does about it (profiles/r01c_compaction.md).  Under streaming load every global round
+// trip costs 2-3 us, and ticket atomic -> load -> aggregate -> look-back windows -> prefix were 5+ of them
+// in series per tile:
+//   * no ticket: tiles are dealt round-robin, so the next tile is known and is cp.async'd into shared
+//     memory while the current one is scanned and stored;
+//   * no chained look-back: a block keeps its own inclusive prefix from its previous tile and adds the
+//     aggregates of the gridDim.x - 1 tiles in between, all 256 threads polling their share at once: one
+//     round trip, and no block ever waits for another block's look-back, only for its count;
+//   * thread t owns particles t and t + 256 of the tile, so survivors of consecutive lanes have consecutive
+//     ranks: the stores from registers are dense 256-byte warp accesses without a shared-memory partition;
+//   * 64 registers: four blocks (32 warps) per SM.
+// ---------------------------------------------------------------------------------------------------
+#ifndef ELG_COMPACT_BLOCKS
+#define ELG_COMPACT_BLOCKS 2
+#endif
+constexpr int kPoll = 3;                                // status words per thread and tile: grids up to 3 * 256 + 1 blocks
+constexpr int kCompactMaxGrid = kPoll * kBlock + 1;
+
+template <int MAXOPS>
+__global__ void __launch_bounds__(kBlock, ELG_COMPACT_BLOCKS) compact_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+    const ChainCommon& c = a.c;
+    const long long n = c.st->n_alive[c.cur];
+    const long long n_tiles = (n + kTile - 1) / kTile;
+    const long long lost_base = c.st->n_lost[c.cur];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double mn = INFINITY, mx = -INFINITY;
+
+    __shared__ __align__(16) double s_in[7][kTile];              // next tile, cp.async'd: thread t owns [.][t], [.][t + kBlock]
+    __shared__ int s_wtot[kWarps];                               // per warp: survivors of sub-tile 0 | sub-tile 1 << 16
+    __shared__ unsigned int s_part[kWarps];
+
+    auto prefetch = [&](long long tile) {                        // 8-byte copies of exactly the elements this thread reads
+#pragma unroll
+        for (int q = 0; q < 2; q++) {
+            const long long i = tile * kTile + threadIdx.x + q * kBlock;
+            const int bytes = i < n ? 8 : 0;                     // zero-fill past the live prefix
+            const long long is = i < n ? i : 0;
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) cp_async8(&s_in[cc][threadIdx.x + q * kBlock], c.src[cc] + is, bytes);
+            cp_async8(&s_in[6][threadIdx.x + q * kBlock], c.id_src + is, bytes);
+        }
+    };
+
+    // the tile counted in the previous iteration, held in registers until its base is known
+    double pv[2][6];
+    long long pid[2] = {0, 0};
+    bool pok[2] = {false, false}, psurv[2] = {false, false};
+    int prank[2] = {0, 0}, ptotal = 0;
+    long long ptile = -1;                                        // -1: nothing held
+    long long my_incl = 0, pptile = -1;                          // inclusive prefix at this block's tile before ptile
+#pragma unroll
+    for (int q = 0; q < 2; q++)
+#pragma unroll
+        for (int cc = 0; cc < 6; cc++) pv[q][cc] = 0.0;
+
+    long long tile = blockIdx.x;                                 // static round-robin tiles: the launch is cooperative,
+    if (tile < n_tiles) prefetch(tile);                          // every block is resident, predecessors always progress
+    for (;; tile += gridDim.x) {
+        const bool cur_valid = tile < n_tiles;
+        // (0) the aggregates between this block's last two tiles were published an iteration ago: request them
+        //     now, they arrive while the current tile is counted
+        unsigned long long stt[kPoll];
+#pragma unroll
+        for (int j = 0; j < kPoll; j++) {
+            const long long w = pptile + 1 + threadIdx.x + j * kBlock;
+            stt[j] = (ptile >= 0 && w < ptile) ? ld_relaxed(c.tile_status + w) : pack_status(c.epoch, kFlagA, 0);
+        }
+
+        double v[2][6];
+        long long id[2];
+        bool ok[2] = {false, false}, surv[2] = {false, false};
+        int rank[2] = {0, 0}, total = 0;
+        if (cur_valid) {
+            const long long i0 = tile * kTile + threadIdx.x;     // my particles: i0 and i0 + kBlock
+            cp_async_wait_all();
+#pragma unroll
+            for (int q = 0; q < 2; q++) {
+                ok[q] = i0 + q * kBlock < n;
+#pragma unroll
+                for (int cc = 0; cc < 6; cc++) v[q][cc] = s_in[cc][threadIdx.x + q * kBlock];
+                id[q] = __double_as_longlong(s_in[6][threadIdx.x + q * kBlock]);
+            }
+            if (tile + gridDim.x < n_tiles) prefetch(tile + gridDim.x);   // streams in during this iteration
+
+            apply_ops<MAXOPS, 2>(a, v);
+
+#pragma unroll
+            for (int q = 0; q < 2; q++) surv[q] = ok[q] && survives(c.ap_type, c.ap_x, c.ap_y, v[q][0], v[q][2]);
+            const int cnt = (int)surv[0] | ((int)surv[1] << 16);
+            int inc = cnt;                                       // warp inclusive scan of both sub-tiles at once
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += t;
+            }
+            if (lane == 31) s_wtot[wid] = inc;
+            __syncthreads();                                     // (A) warp totals visible
+            int before = 0, all = 0;
+#pragma unroll
+            for (int w = 0; w < kWarps; w++) {
+                const int x = s_wtot[w];
+                if (w < wid) before += x;
+                all += x;
+            }
+            const int total0 = all & 0xffff;
+            total = total0 + (all >> 16);
+            if (threadIdx.x == 0 && tile + 1 < n_tiles)          // published at count time: nobody waits for more than a count
+                st_relaxed(c.tile_status + tile, pack_status(c.epoch, kFlagA, (unsigned long long)total));
+            const int ex = inc - cnt;                            // survivors before me in my warp, both sub-tiles
+            rank[0] = (before & 0xffff) + (ex & 0xffff);
+            rank[1] = total0 + (before >> 16) + (ex >> 16);
+        } else {
+#pragma unroll
+            for (int q = 0; q < 2; q++)
+#pragma unroll
+                for (int cc = 0; cc < 6; cc++) v[q][cc] = 0.0;
+            id[0] = 0; id[1] = 0;
+        }
+
+        if (ptile >= 0) {
+            // (1) survivors before the held tile = own inclusive prefix one tile earlier + the aggregates in between
+            unsigned int part = 0;
+#pragma unroll
+            for (int j = 0; j < kPoll; j++) {
+                const long long w = pptile + 1 + threadIdx.x + j * kBlock;
+                if (w < ptile) {
+                    while ((unsigned int)(stt[j] >> 34) != c.epoch || ((stt[j] >> 32) & 3ull) == 0) stt[j] = ld_relaxed(c.tile_status + w);
+                    part += (unsigned int)(stt[j] & 0xffffffffull);
+                }
+            }
+            part = __reduce_add_sync(0xffffffffu, part);
+            if (lane == 0) s_part[wid] = part;
+            __syncthreads();                                     // (B) partial sums visible
+            long long base = my_incl;
+#pragma unroll
+            for (int w = 0; w < kWarps; w++) base += s_part[w];
+            my_incl = base + ptotal;
+            pptile = ptile;
+            if (ptile == n_tiles - 1 && threadIdx.x == 0) {      // the last tile knows the totals
+                c.st->n_alive[c.cur ^ 1] = my_incl;
+                c.st->n_lost[c.cur ^ 1] = lost_base + (n - my_incl);
+            }
+            const long long lost0 = lost_base + (ptile * kTile - base);      // lost before the tile = index - survivors before
+#pragma unroll
+            for (int q = 0; q < 2; q++) {
+                if (psurv[q]) {
+                    const long long d = base + prank[q];
+#pragma unroll
+                    for (int cc = 0; cc < 6; cc++) c.dst[cc][d] = pv[q][cc];
+                    c.id_dst[d] = pid[q];
+                    if (c.want_minmax) { mn = fmin(mn, pv[q][4]); mx = fmax(mx, pv[q][4]); }
+                } else if (pok[q]) {
+                    const long long lpos = lost0 + ((int)threadIdx.x + q * kBlock - prank[q]);
+                    if (lpos < c.lost_cap) {
+                        c.lost_id[lpos] = pid[q];
+                        c.lost_te[lpos] = c.te_code;
+#pragma unroll
+                        for (int cc = 0; cc < 6; cc++) c.lost_v[cc * c.lost_cap + lpos] = pv[q][cc];
+                    }
+                }
+            }
+            __syncthreads();                                     // s_part free before the next iteration's (B)
+        }
+        if (!cur_valid) break;
+#pragma unroll
+        for (int q = 0; q < 2; q++) {                            // hold the counted tile
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) pv[q][cc] = v[q][cc];
+            pid[q] = id[q]; pok[q] = ok[q]; psurv[q] = surv[q]; prank[q] = rank[q];
+        }
+        ptotal = total;
+        ptile = tile;
+    }
+
+    if (c.want_minmax) {                                         // exact min/max of s over the survivors (a8)
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, d));
+            mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+        }
+        __shared__ double s_mn[kWarps], s_mx[kWarps];
+        if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
+            c.mm_partial[2 * blockIdx.x] = mn;
+            c.mm_partial[2 * blockIdx.x + 1] = mx;
+        }
+    }
+    if (n_tiles == 0 && blockIdx.x == 0 && threadIdx.x == 0) {   // nothing alive: carry the counts over
+        c.st->n_alive[c.cur ^ 1] = 0;
+        c.st->n_lost[c.cur ^ 1] = lost_base;
     }
 }
 

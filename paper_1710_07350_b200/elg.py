@@ -74,7 +74,11 @@ def lib():
     if _lib is not None:
         return _lib
     path = LIB
-    if not os.path.exists(path) or os.environ.get("ELG_REBUILD"):
+    if os.environ.get("ELG_LIB"):                       # a tuning variant built with build(out=..., extra=...)
+        path = os.environ["ELG_LIB"]
+        if not os.path.exists(path):
+            raise RuntimeError(f"ELG_LIB={path} does not exist")
+    elif not os.path.exists(path) or os.environ.get("ELG_REBUILD"):
         path = build()
     else:
         try:

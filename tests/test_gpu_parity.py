@@ -114,6 +114,47 @@ def test_each_map_alone(elg, elgo):
             assert np.array_equal(gv[:5], ov[:5])                    # only delta sees sin (<= 2 ulp)
 
 
+def _long_line(n_mat, extra):
+    """n_mat distinct symplectic drift x quad matrices (cfg3's generator) with other maps spliced in."""
+    ring = make_workload("cfg3", n=8, n_matrices=n_mat)
+    mats = [e for e in ring.elements if e["type"] == "MATRIX"]
+    out = []
+    for k, m in enumerate(mats):
+        out.append(m)
+        if k in extra:
+            out.append(extra[k])
+    return out
+
+
+@pytest.mark.parametrize("n", [1, 1535, 1536, 1537, 3 * 1536 + 7, 200_001])
+def test_long_run_kernel_bitexact(elg, elgo, n):
+    """Runs of more than 8 maps go through chain_long_kernel (6 particles per thread, 1536-particle tiles,
+    coefficients in shared memory, matrix pairs): odd matrix counts, DRIFT / RFKICK inside the run, ragged tails."""
+    elems = _long_line(23, {4: {"type": "DRIFT", "L": 0.75}, 11: {"type": "RFKICK", "V": 2e6, "f": 1.3e9, "phi": 2.1},
+                            12: {"type": "DRIFT", "L": 0.25}})
+    v0 = make_workload("cfg0", n=n).particles()
+    ob = elgo.Bunch(v0, 1e9, 1e-9); ob.track(elgo.Beamline(elems), 1)
+    gbl = elg.Beamline(elems)
+    assert gbl.launches_per_turn("none") == 1                      # one fused run
+    gb = elg.Bunch(v0, 1e9, 1e-9, beamline=gbl); gb.track(gbl, 1)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid)
+    assert np.array_equal(gv[:5], ov[:5])
+    assert rel_err(gv, ov) <= 1e-12
+
+
+def test_long_run_ending_in_aperture(elg, elgo):
+    """More than 8 maps and then a collimator: long-run kernel, then the aperture as a compacting run."""
+    elems = _long_line(12, {}) + [{"type": "ECOL", "a": 400e-6, "b": 350e-6}, {"type": "DRIFT", "L": 1.0}]
+    v0 = make_workload("cfg0", n=50_003).particles()
+    ob = elgo.Bunch(v0, 1e9, 1e-9); ob.track(elgo.Beamline(elems), 1)
+    gbl = elg.Beamline(elems); gb = elg.Bunch(v0, 1e9, 1e-9, beamline=gbl); gb.track(gbl, 1)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert 0 < gid.size < 50_003
+    assert np.array_equal(gid, oid) and np.array_equal(gv, ov)
+    check_lost(ob, gb)
+
+
 # ------------------------------------------------------------------------------------ (ii) loss
 def test_compaction_hand_placed(elg, elgo):
     """Edge-inclusive, NaN lost, Fig. 2 shape (20 particles, 4 lost)."""
