@@ -175,7 +175,7 @@ int32_t elg_bunch_device_array(elg_bunch*, int32_t c, void** d_ptr);
  * their summed device time since the last read (h_launches, h_ms: ELG_K_COUNT entries each) and resets
  * the counters.  Off by default (no events are recorded). */
 enum { ELG_K_CHAIN = 0, ELG_K_CHAIN_COMPACT = 1, ELG_K_WINDOW = 2, ELG_K_HIST = 3, ELG_K_WAKE_SAMPLES = 4,
-       ELG_K_CONV = 5, ELG_K_MOMENTS = 6, ELG_K_COUNT = 7 };
+       ELG_K_CONV = 5, ELG_K_MOMENTS = 6, ELG_K_CHAIN_LONG = 7, ELG_K_COUNT = 8 };
 int32_t elg_profile_enable(elg_bunch*, int32_t on);
 int32_t elg_profile_read(elg_bunch*, int64_t* h_launches, double* h_ms);
 

@@ -368,6 +368,7 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, 2>, sms, 0, kBlock, &b->grid_chain[0][0]);
     if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, 4>, sms, 0, kBlock, &b->grid_chain[1][0]);
     if (rc == ELG_OK) rc = grid_for(compact_kernel<kMaxOpsSmall>, sms, 0, kBlock, &b->grid_chain[0][1]);
+    if (b->grid_chain[0][1] > kCompactMaxGrid) b->grid_chain[0][1] = kCompactMaxGrid;   // kPoll status words per thread
     b->grid_chain[1][1] = b->grid_chain[0][1];
     if (rc == ELG_OK) rc = grid_for(chain_long_kernel<kMaxOpsLarge>, sms, chain_long_smem_bytes<kMaxOpsLarge>(), kBlock, &b->grid_chain[2][0]);
     b->grid_chain[2][1] = b->grid_chain[2][0];
@@ -485,7 +486,7 @@ struct Tracker {
         const int grid = b->grid_chain[MAXOPS == kMaxOpsLarge ? 2 : (P == 4 ? 1 : 0)][COMPACT ? 1 : 0];
         if (want_mm) mm_grid = grid;
         {
-            ProfScope ps(b, COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN);
+            ProfScope ps(b, MAXOPS == kMaxOpsLarge ? ELG_K_CHAIN_LONG : (COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN));
             if constexpr (MAXOPS == kMaxOpsLarge)
                 chain_long_kernel<MAXOPS><<<grid, kBlock, chain_long_smem_bytes<MAXOPS>(), b->stream>>>(a);
             else if constexpr (COMPACT)
@@ -591,7 +592,7 @@ struct Tracker {
             w.t_design = s_here * b->inv_bc; w.inv_bc = b->inv_bc; w.counts = b->counts;
             {
                 ProfScope ps(b, ELG_K_WINDOW);
-                window_kernel<<<1, kBlock, 0, b->stream>>>(w);
+                window_kernel<<<(e.nb + 4 * kBlock - 1) / (4 * kBlock), kBlock, 0, b->stream>>>(w);
             }
             check(cudaGetLastError(), "window_kernel launch");
             HistArgs h;

@@ -217,6 +217,34 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
     }
 }
 
+// the run's maps with the coefficients in shared memory (copied there once per block): 128-bit fetches, and
+// consecutive MATRIX maps applied in pairs (v -> w -> v) so that no register copy-back is needed
+template <int MAXOPS, int P>
+__device__ __forceinline__ void apply_ops_smem(const ChainArgs<MAXOPS>& a, const double* s_coef, double (&v)[P][6]) {
+    const ChainCommon& c = a.c;
+    int op = 0;
+    while (op < c.n_ops) {
+        const int ty = a.type[op];
+        if (ty == OP_MATRIX && op + 1 < c.n_ops && a.type[op + 1] == OP_MATRIX) {
+            double w[P][6];
+            matrix_map_s128<P>(s_coef + 42 * op, v, w);
+            matrix_map_s128<P>(s_coef + 42 * (op + 1), w, v);
+            op += 2;
+        } else if (ty == OP_MATRIX) {
+            double w[P][6];
+            matrix_map_s128<P>(s_coef + 42 * op, v, w);
+#pragma unroll
+            for (int p = 0; p < P; p++)
+#pragma unroll
+                for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+            op++;
+        } else {
+            other_map<P>(ty, s_coef + 42 * op, c, v);
+            op++;
+        }
+    }
+}
+
 __device__ __forceinline__ bool survives(int ap_type, double ax, double ay, double x, double y) {
     if (ap_type == AP_RCOL) return (fabs(x) <= ax) && (fabs(y) <= ay);        // NaN -> false (G17)
     const double xa = x * ax, yb = y * ay;                                    // ECOL: ax, ay hold 1/a, 1/b
@@ -312,7 +340,7 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
 // ---------------------------------------------------------------------------------------------------
 // chain_long_kernel: runs of more than kMaxOpsSmall maps (cfg3: 80 MATRIX per launch), bound by the fp64
 // pipe, not by HBM.  On sm_100 every operand fetch that returns through the MIO (LDS, LDC) costs DFMA
-// issue slots (profiles/r01c_*.md: a broadcast LDS.128 costs about two DFMA), so the design minimises
+// issue slots (profiles/r01d_long_chain_and_compaction.md: a broadcast LDS.128 costs about two DFMA), so the design minimises
 // coefficient fetches per DFMA:
 //   * kPL = 6 particles per thread: one 128-bit coefficient fetch feeds 12 DFMA;
 //   * the run's coefficients are copied once per block from the parameter bank to shared memory and read
@@ -389,27 +417,7 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
         const long long next = tile + gridDim.x;
         if (next < n_tiles) prefetch(next);                      // own slots only: already in registers
 
-        int op = 0;
-        while (op < c.n_ops) {
-            const int ty = a.type[op];
-            if (ty == OP_MATRIX && op + 1 < c.n_ops && a.type[op + 1] == OP_MATRIX) {
-                double w[kPL][6];
-                matrix_map_s128<kPL>(s_coef + 42 * op, v, w);
-                matrix_map_s128<kPL>(s_coef + 42 * (op + 1), w, v);
-                op += 2;
-            } else if (ty == OP_MATRIX) {
-                double w[kPL][6];
-                matrix_map_s128<kPL>(s_coef + 42 * op, v, w);
-#pragma unroll
-                for (int p = 0; p < kPL; p++)
-#pragma unroll
-                    for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
-                op++;
-            } else {
-                other_map<kPL>(ty, s_coef + 42 * op, c, v);
-                op++;
-            }
-        }
+        apply_ops_smem<MAXOPS, kPL>(a, s_coef, v);
 
         const long long t0 = tile * kTileL + (long long)threadIdx.x * 2;
 #pragma unroll
@@ -456,7 +464,7 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
 // (every block resident), tiles are dealt round-robin, so a tile's predecessors always make progress.
 //
 // What made the first version latency-bound (profiles/r01b: 37 % of the HBM peak, 10 us per tile) and
-// what this one does about it (profiles/r01c_compaction.md).  Under streaming load every global round
+// what this one does about it (profiles/r01d_long_chain_and_compaction.md).  Under streaming load every global round
 // trip costs 2-3 us, and ticket atomic -> load -> aggregate -> look-back windows -> prefix were 5+ of them
 // in series per tile:
 //   * no ticket: tiles are dealt round-robin, so the next tile is known and is cp.async'd into shared
@@ -540,7 +548,7 @@ __global__ void __launch_bounds__(kBlock, ELG_COMPACT_BLOCKS) compact_kernel(con
             }
             if (tile + gridDim.x < n_tiles) prefetch(tile + gridDim.x);   // streams in during this iteration
 
-            apply_ops<MAXOPS, 2>(a, v);
+            apply_ops<MAXOPS, 2>(a, v);       // short run: coefficients straight from the parameter bank
 
 #pragma unroll
             for (int q = 0; q < 2; q++) surv[q] = ok[q] && survives(c.ap_type, c.ap_x, c.ap_y, v[q][0], v[q][2]);
@@ -654,7 +662,7 @@ __global__ void __launch_bounds__(kBlock, ELG_COMPACT_BLOCKS) compact_kernel(con
 // ---------------------------------------------------------------------------------------------------
 // window_kernel (a8 -> G10): reduce the per-block min/max partials (exact in any order), derive the
 // histogram window with the same fp64 operations as the definition, the occupied bin range used for
-// shared-memory privatisation, and zero the counts.  One block.
+// shared-memory privatisation, and zero the counts (every block zeroes a slice, block 0 does the rest).
 // ---------------------------------------------------------------------------------------------------
 struct WindowArgs {
     DevState* st;
@@ -668,6 +676,8 @@ struct WindowArgs {
 };
 
 __global__ void __launch_bounds__(kBlock) window_kernel(const WindowArgs a) {
+    for (int i = blockIdx.x * kBlock + threadIdx.x; i < a.nb; i += gridDim.x * kBlock) a.counts[i] = 0u;   // all blocks
+    if (blockIdx.x != 0) return;                                 // block 0 derives the window
     __shared__ double s_mn[kWarps], s_mx[kWarps];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double mn = INFINITY, mx = -INFINITY;
@@ -681,7 +691,6 @@ __global__ void __launch_bounds__(kBlock) window_kernel(const WindowArgs a) {
         mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
     }
     if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
-    for (int i = threadIdx.x; i < a.nb; i += kBlock) a.counts[i] = 0u;
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
@@ -719,7 +728,7 @@ __global__ void __launch_bounds__(kBlock) window_kernel(const WindowArgs a) {
 // sub-histograms per block (one per warp when they fit) cut contention; sub-histograms are combined
 // with integer global atomics (exact, order-independent).  Only the occupied bin range is privatised,
 // so nb = 65536 (256 KB) still fits; bins outside the first kHistSmemBins of the range fall back to
-// global atomics.  Persistent grid, 2 x 128-bit loads of s per thread and iteration.
+// global atomics.  Persistent grid, 4 x 128-bit loads of s per thread and iteration.
 // ---------------------------------------------------------------------------------------------------
 struct HistArgs {
     const double* s;
@@ -748,24 +757,26 @@ __global__ void __launch_bounds__(kBlock) hist_kernel(const HistArgs a) {
     for (int i = threadIdx.x; i < R * S; i += kBlock) sh[i] = 0u;
     __syncthreads();
 
-    constexpr int kPer = 4;
+    constexpr int kPer = 8;                                      // 4 x 128-bit loads in flight per thread
     const long long stride = (long long)gridDim.x * kBlock * kPer;
     // warp-uniform trip count (the aggregated path uses full-mask warp votes)
     for (long long w0 = ((long long)blockIdx.x * kBlock + (threadIdx.x & ~31)) * kPer; w0 < n; w0 += stride) {
-        const long long i0 = w0 + (long long)(threadIdx.x & 31) * kPer;
+        // lane l owns particles w0 + 2l + 64k + {0, 1}, k < 4: every load is a 512-byte warp access
+        const long long i0 = w0 + (long long)(threadIdx.x & 31) * 2;
         double sv[kPer];
-        int nv = 0;
-        if (i0 + kPer <= n) {
-            const double2 t0 = ld_stream2(a.s + i0), t1 = ld_stream2(a.s + i0 + 2);
-            sv[0] = t0.x; sv[1] = t0.y; sv[2] = t1.x; sv[3] = t1.y;
-            nv = kPer;
-        } else {
-            for (; nv < kPer && i0 + nv < n; nv++) sv[nv] = a.s[i0 + nv];
+        bool have[kPer];
+#pragma unroll
+        for (int k = 0; k < kPer / 2; k++) {
+            const long long i = i0 + 64 * k;
+            have[2 * k] = i < n; have[2 * k + 1] = i + 1 < n;
+            sv[2 * k] = 0.0; sv[2 * k + 1] = 0.0;
+            if (have[2 * k + 1]) { const double2 t = ld_stream2(a.s + i); sv[2 * k] = t.x; sv[2 * k + 1] = t.y; }
+            else if (have[2 * k]) sv[2 * k] = ld_stream1(a.s + i);
         }
 #pragma unroll
         for (int p = 0; p < kPer; p++) {
             double u;
-            const int b = (p < nv) ? bin_of(sv[p], a.inv_bc, t_lo, inv_dt, a.nb, &u) : -1;
+            const int b = have[p] ? bin_of(sv[p], a.inv_bc, t_lo, inv_dt, a.nb, &u) : -1;
             if (a.aggregate) {
                 const unsigned int act = __ballot_sync(0xffffffffu, b >= 0);   // loop trip count is warp-uniform
                 if (b >= 0) {

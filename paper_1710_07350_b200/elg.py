@@ -35,7 +35,7 @@ EXPORTS = (
     "elg_profile_enable", "elg_profile_read",
     "elg_dbg_histogram", "elg_dbg_wake_samples", "elg_dbg_convolve", "elg_dbg_kick",
 )
-KERNEL_KINDS = ("chain", "chain_compact", "window", "hist", "wake_samples", "conv", "moments")
+KERNEL_KINDS = ("chain", "chain_compact", "window", "hist", "wake_samples", "conv", "moments", "chain_long")
 
 
 class ElgError(RuntimeError):
