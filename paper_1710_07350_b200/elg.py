@@ -219,8 +219,8 @@ class Beamline:
         return any(e["type"] in ("RCOL", "ECOL") for e in self.elements)
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().elg_beamline_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:       # (module globals are gone at interpreter exit)
+            _lib.elg_beamline_destroy(self._h)
             self._h = None
 
 
@@ -261,8 +261,8 @@ class Bunch:
             self.upload(coords, ids)
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().elg_bunch_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.elg_bunch_destroy(self._h)
             self._h = None
 
     # -- data movement -------------------------------------------------------------------------

@@ -1,0 +1,137 @@
+"""Parity at BASELINE.json's full size (1e8 particles), in the launch configuration bench.py times.
+
+The oracle cannot track 1e8 particles through 200 elements in test time, so (task statement, parity at full
+size): per-particle results are checked on SAMPLED particles the oracle computes one by one, the collective
+stages (window, histogram, convolution, moments) are checked by feeding the oracle's stage functions the
+coordinates the CUDA path produced (bit-equal to the oracle's own on the samples), and the compaction by
+sampled membership plus the properties that hold at any size (order, partition of the ID set).
+"""
+import numpy as np
+import pytest
+
+from elg_inputs import make_workload
+
+pytestmark = pytest.mark.gpu
+
+N_FULL = 100_000_000
+N_SAMPLE = 8192
+
+
+@pytest.fixture(scope="module")
+def elg():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1710_07350_b200 import elg as mod
+    mod.lib()
+    return mod
+
+
+def _pinned_particles(w, n):
+    import torch
+    h = torch.empty((6, n), dtype=torch.float64, pin_memory=True)
+    w.particles(n, out=h.numpy())
+    return h
+
+
+def _sample(n, seed):
+    rng = np.random.default_rng(seed)
+    idx = np.unique(np.concatenate([rng.integers(0, n, N_SAMPLE), [0, 1, 511, 512, 1535, 1536, n - 2, n - 1]]))
+    return idx.astype(np.int64)
+
+
+def test_cfg3_one_turn_at_1e8(elg, elgo):
+    """One turn of cfg3 (bench.py's step): 3 long-run launches, window, histogram, wake, kick, moments."""
+    import torch
+    w = make_workload("cfg3", n=N_FULL)
+    h = _pinned_particles(w, N_FULL)
+    v0 = h.numpy()
+    gbl = elg.Beamline(w.elements, ring=True)
+    gb = elg.Bunch(None, w.p0c_eV, w.charge_C, beamline=gbl, n0=N_FULL, lost_capacity=0)
+    gb.upload(h)
+    go = gb.track(gbl, 1, moments_every="turn", want_stage_outputs=True)
+    assert gb.n_alive == N_FULL
+
+    # (i) per-particle maps on samples: 200 MATRIX + RFKICK, x x' y y' s bit-identical
+    idx = _sample(N_FULL, 3)
+    maps = [e for e in w.elements if e["type"] != "WAKE"]
+    assert len(maps) == 201 and w.elements[-1]["type"] == "WAKE"
+    ob = elgo.Bunch(np.ascontiguousarray(v0[:, idx]), w.p0c_eV, w.charge_C)
+    ob.track(elgo.Beamline(maps, ring=True), 1)
+    ov, _ = ob.read()
+    t_idx = torch.as_tensor(idx, device="cuda")
+    gv = np.stack([gb.device_array(c)[t_idx].cpu().numpy() for c in range(6)])
+    assert np.array_equal(gv[:5], ov[:5])
+
+    # (ii) window and histogram from the CUDA path's s (bit-equal to the oracle's on the samples)
+    s_full = gb.device_array(4)[:N_FULL].cpu().numpy()
+    b0 = elgo.beta0(w.p0c_eV)
+    inv_bc = elgo.inv_bc(b0)
+    wake = w.elements[-1]
+    t_lo, dt, inv_dt = elgo.window(s_full, inv_bc, 1, wake["nb"])                    # AUTO_MINMAX
+    assert np.array_equal(go["window"][0], [t_lo, dt, inv_dt])
+    counts, binned = elgo.histogram(s_full, inv_bc, t_lo, inv_dt, wake["nb"])
+    assert np.array_equal(go["hist"], counts) and int(counts.sum()) == N_FULL == binned
+
+    # (iii) wake voltage from the oracle's samples and convolution
+    W = elgo.wake_samples(0, wake["nb"], dt, f=wake["f"], Q=wake["Q"], Rs=wake["Rs"])
+    V = elgo.convolve(counts, W, w.charge_C / N_FULL)
+    assert np.max(np.abs(go["V"] - V)) <= 1e-10 * np.max(np.abs(V))
+
+    # (iv) delta of the samples: RF kick (oracle) + interpolated wake kick (oracle's kick on the oracle's V)
+    d_exp = ov[5].copy()
+    elgo.kick(ov[4], d_exp, inv_bc, t_lo, inv_dt, wake["nb"], V, elgo.inv_E(b0, w.p0c_eV), True)
+    sig = np.std(d_exp)
+    assert np.max(np.abs(gv[5] - d_exp) / np.maximum(np.abs(d_exp), sig)) <= 1e-12
+
+    # (v) moments record against the oracle's two-pass moments of the same coordinates
+    full = np.empty((6, N_FULL))
+    full[4] = s_full
+    for c in (0, 1, 2, 3, 5):
+        full[c] = gb.device_array(c)[:N_FULL].cpu().numpy()
+    cen, sig6 = elgo.moments(full)
+    rec = go["records"][0]
+    assert rec[0] == N_FULL
+    S = np.asarray(sig6).reshape(6, 6)
+    assert np.max(np.abs(rec[7:].reshape(6, 6) - S)) <= 1e-10 * np.max(np.abs(S))
+    assert np.all(np.abs(rec[1:7] - cen) <= 1e-10 * np.maximum(np.abs(cen).max(), np.sqrt(np.diag(S))))
+
+
+def test_compaction_at_1e8(elg, elgo):
+    """DRIFT + MATRIX + RCOL on 1e8 particles (bench.py's p2 probe): stable order, exact partition of the ID
+    set, sampled particles where the oracle puts them."""
+    w = make_workload("p2-chain-rcol", n=N_FULL)
+    h = _pinned_particles(w, N_FULL)
+    v0 = h.numpy()
+    gbl = elg.Beamline(w.elements)
+    gb = elg.Bunch(None, w.p0c_eV, w.charge_C, beamline=gbl, n0=N_FULL, lost_capacity=2_000_000)
+    gb.upload(h)
+    gb.track(gbl, 1)
+    n_alive = gb.n_alive
+    gid = gb.device_array(6)[:n_alive].cpu().numpy()
+    lid, lturn, lelem, lco = gb.lost()
+    assert n_alive + lid.size == N_FULL and 0 < lid.size < 2_000_000
+    assert np.all(np.diff(gid) > 0), "survivors keep their original order"
+    assert np.all(np.diff(lid) > 0), "lost particles are logged in position order"
+    seen = np.zeros(N_FULL, dtype=np.bool_)
+    seen[gid] = True
+    assert not seen[lid].any()
+    seen[lid] = True
+    assert seen.all(), "survivors and lost partition the ID set"
+    assert np.all(lturn == 0) and np.all(lelem == 2)
+
+    # sampled particles, plus every 64th lost one: the oracle tracks them one by one
+    idx = np.unique(np.concatenate([_sample(N_FULL, 5), lid[::64]]))
+    ob = elgo.Bunch(np.ascontiguousarray(v0[:, idx]), w.p0c_eV, w.charge_C, ids=idx)
+    ob.track(elgo.Beamline(w.elements), 1)
+    ov, oid = ob.read()
+    olid, _, _, olco = ob.lost()
+    assert np.array_equal(np.sort(np.concatenate([oid, olid])), idx)
+    pos = np.searchsorted(gid, oid)
+    assert np.array_equal(gid[pos], oid), "oracle survivors are CUDA survivors"
+    import torch
+    t_pos = torch.as_tensor(pos, device="cuda")
+    gv = np.stack([gb.device_array(c)[t_pos].cpu().numpy() for c in range(6)])
+    assert np.array_equal(gv, ov)
+    lpos = np.searchsorted(lid, olid)
+    assert np.array_equal(lid[lpos], olid), "oracle lost are CUDA lost"
+    assert np.array_equal(lco[lpos], olco)
