@@ -9,10 +9,11 @@ SURVEY.md section 8c, restated in DESIGN.md).  Both sides receive the same bytes
 from .rng import uniform01, normal01, SEED_BASE
 from .configs import (
     ELECTRON_MC2_EV, C_LIGHT, Workload, make_workload, WORKLOAD_NAMES,
-    drift_matrix, thin_quad_matrix, compose,
+    drift_matrix, thin_quad_matrix, compose, pair_index, second_order_drift, thin_quad_sextupole,
 )
 
 __all__ = [
     "uniform01", "normal01", "SEED_BASE", "ELECTRON_MC2_EV", "C_LIGHT", "Workload",
     "make_workload", "WORKLOAD_NAMES", "drift_matrix", "thin_quad_matrix", "compose",
+    "pair_index", "second_order_drift", "thin_quad_sextupole",
 ]

@@ -17,6 +17,7 @@ readings it encodes (restated in DESIGN.md "Readings"):
 Element dictionaries (keys are the paper's/BASELINE.json's names):
   DRIFT  {L}                         exact drift, PAPER.md:68-79 (Listing 1)
   MATRIX {R (6,6), C (6,)}           first-order transport matrix
+  MATRIX2 {R, C, T (6,21)}           second-order transport map, PAPER.md:156 (G31)
   RFKICK {V, f, phi}                 thin RF cavity, PAPER.md:154,175
   RCOL   {ax, ay}  ECOL {a, b}       collimators, PAPER.md:149,153
   WAKE   {nb, window, wake, ...}     longitudinal wake, PAPER.md:165
@@ -36,7 +37,7 @@ C_LIGHT = 299792458.0
 
 WORKLOAD_NAMES = (
     "cfg0", "cfg1", "cfg2", "cfg3", "cfg3-literal", "cfg4",
-    "p1-chain", "p2-chain-rcol", "p3-matrices",
+    "p1-chain", "p2-chain-rcol", "p3-matrices", "p4-second-order",
 )
 
 
@@ -57,6 +58,37 @@ def thin_quad_matrix(k1L: float):
     R[1, 0] = -k1L
     R[3, 2] = +k1L
     return R, np.zeros(6)
+
+
+def pair_index(j: int, k: int) -> int:
+    """Position of the pair (j, k), j <= k, in the order (0,0) (0,1) .. (0,5) (1,1) .. (5,5) (G31)."""
+    if j > k:
+        j, k = k, j
+    return j * 6 - j * (j - 1) // 2 + (k - j)
+
+
+def second_order_drift(L: float):
+    """Drift to second order: the linear drift plus the path-length terms s += L/2 (x'^2 + y'^2)."""
+    R, C = drift_matrix(L)
+    T = np.zeros((6, 21))
+    T[4, pair_index(1, 1)] = 0.5 * L
+    T[4, pair_index(3, 3)] = 0.5 * L
+    return R, C, T
+
+
+def thin_quad_sextupole(k1L: float, k2L: float):
+    """Thin quadrupole + sextupole kick (G5 signs): x' -= k1L x + k2L/2 (x^2 - y^2);  y' += k1L y + k2L x y."""
+    R, C = thin_quad_matrix(k1L)
+    T = np.zeros((6, 21))
+    T[1, pair_index(0, 0)] = -0.5 * k2L
+    T[1, pair_index(2, 2)] = +0.5 * k2L
+    T[3, pair_index(0, 2)] = +k2L
+    return R, C, T
+
+
+def _matrix2_elem(R, C, T):
+    return {"type": "MATRIX2", "R": np.ascontiguousarray(R, dtype=np.float64),
+            "C": np.ascontiguousarray(C, dtype=np.float64), "T": np.ascontiguousarray(T, dtype=np.float64)}
 
 
 def compose(*maps):
@@ -286,11 +318,26 @@ def _p3(n, n_matrices=8):
                     c3.elements[:n_matrices], "gauss6", notes=f"{n_matrices} cfg3 matrices")
 
 
+def _p4(n, n_cells=100, n_turns=1):
+    """Second-order ring (track_particles M2): n_cells x [second-order drift 1 m,
+    thin quadrupole + sextupole], quadrupole strengths of the stabilised cfg3 ring, k2L = +-2 m^-2."""
+    seed = SEED_BASE + 3
+    u = uniform01(seed, 300, n_cells) - 0.5
+    elems = []
+    for i in range(n_cells):
+        k1L = (1.0 if i % 2 == 0 else -1.0) * 0.4 * (1.0 + 0.1 * u[i])
+        k2L = (2.0 if i % 2 == 0 else -2.0)
+        elems.append(_matrix2_elem(*second_order_drift(1.0)))
+        elems.append(_matrix2_elem(*thin_quad_sextupole(k1L, k2L)))
+    return Workload("p4-second-order", 3, n or 100_000_000, 3e9, 1e-9, True, n_turns, "none",
+                    elems, "gauss6", notes=f"{2 * n_cells} second-order maps per turn")
+
+
 def make_workload(name: str, n: Optional[int] = None, **kw) -> Workload:
     """name in WORKLOAD_NAMES; n overrides the particle count (reduced-size parity cases)."""
     table = {
         "cfg0": _cfg0, "cfg1": _cfg1, "cfg2": _cfg2, "cfg3": _cfg3, "cfg3-literal": _cfg3_literal,
-        "cfg4": _cfg4, "p1-chain": _p1, "p2-chain-rcol": _p2, "p3-matrices": _p3,
+        "cfg4": _cfg4, "p1-chain": _p1, "p2-chain-rcol": _p2, "p3-matrices": _p3, "p4-second-order": _p4,
     }
     if name not in table:
         raise KeyError(f"unknown workload {name!r}; known: {WORKLOAD_NAMES}")

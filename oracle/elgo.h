@@ -10,6 +10,8 @@
  * Parity status of each function (what pins it, see tests/test_oracle_pins.py):
  *   elgo_drift        pinned  - Listing 1 exact cases, literal re-evaluation
  *   elgo_matrix       pinned  - closed forms, identity, inverse, symplectic invariants
+ *   elgo_matrix2      pinned  - T = 0 equals elgo_matrix bitwise, one-entry index pins, thin sextupole and
+ *                               second-order drift closed forms (exact drift to O(x'^4))
  *   elgo_rfkick       pinned  - crest/zero-crossing/periodicity/slope closed forms
  *   elgo_aperture     pinned  - hand-placed particles, brute-force stable partition, erf fractions
  *   elgo_window/histogram  pinned - hand-placed bins, edge rule, sum of counts
@@ -36,7 +38,7 @@ enum { ELGO_OK = 0, ELGO_EINVAL = -1, ELGO_ENOMEM = -2, ELGO_ESTATE = -4, ELGO_E
 
 /* element types (names: PAPER.md:175 glossary; north_star) */
 enum { ELGO_DRIFT = 1, ELGO_MATRIX = 2, ELGO_RFKICK = 3, ELGO_RCOL = 4, ELGO_ECOL = 5,
-       ELGO_WAKE = 6, ELGO_HISTO = 7 };
+       ELGO_WAKE = 6, ELGO_HISTO = 7, ELGO_MATRIX2 = 8 };
 /* histogram window modes (G10) */
 enum { ELGO_WIN_EXPLICIT = 0, ELGO_WIN_AUTO_MINMAX = 1, ELGO_WIN_AUTO_TABLE = 2 };
 /* wake kinds (G12) */
@@ -47,6 +49,8 @@ enum { ELGO_MOM_NONE = 0, ELGO_MOM_TURN = 1, ELGO_MOM_ELEMENT = 2 };
 /* One beamline element.  Unused fields are ignored.
  *   DRIFT : L
  *   MATRIX: R (36, row-major R[6*r+c]), C (6, may be NULL = 0)
+ *   MATRIX2: R, C as MATRIX, T (126 = 6 x 21, T[21*i + q], q numbers the pairs (j,k), j <= k, in the order
+ *           (0,0) (0,1) .. (0,5) (1,1) .. (5,5)): second-order transport map (G31)
  *   RFKICK: V [V], f [Hz], phi [rad]
  *   RCOL  : ax, ay [m]      ECOL: ax=a, ay=b [m]
  *   WAKE  : nb, window, (t_lo_rel, dt if EXPLICIT), wake kind, (f, Q, Rs) or (table, n_table, dt_table), interp
@@ -68,6 +72,7 @@ typedef struct {
     const double* C;
     const double* table;
     int64_t n_table;
+    const double* T;
 } elgo_element;
 
 typedef struct elgo_bunch elgo_bunch;
@@ -76,6 +81,8 @@ typedef struct elgo_beamline elgo_beamline;
 /* ---- stage functions on plain arrays (used stage by stage in the parity protocol) ---- */
 void   elgo_drift(double* x, const double* xp, double* y, const double* yp, double* s, int64_t n, double L);
 void   elgo_matrix(double* const v[6], int64_t n, const double* R36, const double* C6);
+/* second-order map: v_i <- C_i + sum_j R_ij v_j + sum_{j<=k} T_ijk v_j v_k (G31) */
+void   elgo_matrix2(double* const v[6], int64_t n, const double* R36, const double* C6, const double* T126);
 void   elgo_rfkick(const double* s, double* delta, int64_t n, double A, double omega, double phi0,
                    double s_ref, double inv_bc);
 /* survive[i] = 1/0.  kind = ELGO_RCOL or ELGO_ECOL. */

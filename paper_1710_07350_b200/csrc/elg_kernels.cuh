@@ -26,7 +26,9 @@ constexpr int kTile = kBlock * kP;     // particles per tile
 constexpr int kHistSmemBins = 16384;   // 64 KB of privatised bins per block
 constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
 
-enum : uint8_t { OP_DRIFT = 1, OP_MATRIX = 2, OP_RFKICK = 3, OP_KICK = 4 };
+enum : uint8_t { OP_DRIFT = 1, OP_MATRIX = 2, OP_RFKICK = 3, OP_KICK = 4,
+                 OP_MATRIX2 = 5,      // second-order map: this slot holds R, C; the next three hold T (OP_CONT)
+                 OP_CONT = 6 };
 enum { AP_NONE = 0, AP_RCOL = 1, AP_ECOL = 2 };
 
 // Device-resident tracking state (first bytes of the workspace).  Nothing here is read by the host
@@ -73,8 +75,8 @@ template <int MAXOPS>
 struct ChainArgs {
     ChainCommon c;
     uint8_t type[MAXOPS];
-    double coef[MAXOPS][42];   // MATRIX: R[36], C[6].  DRIFT: L.  RFKICK: A, omega, phi0, s_ref, inv_bc.
-                               // KICK: inv_bc, inv_E
+    alignas(16) double coef[MAXOPS][42];   // MATRIX: R[36], C[6].  DRIFT: L.  RFKICK: A, omega, phi0, s_ref, inv_bc.
+                               // KICK: inv_bc, inv_E.  MATRIX2: R[36], C[6], then 3 slots = Tt[21][6] (pair-major)
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -149,6 +151,30 @@ __device__ __forceinline__ void matrix_map_s128(const double* c, const double (&
     }
 }
 
+// second-order terms of MATRIX2 (G31): w[p][r] += sum over the pairs q = (j,k), j <= k, of T[r][q] (v_j v_k),
+// q ascending, continuing row r's FMA chain after the six first-order terms.  tt = Tt[21][6] (pair-major), so
+// one pair costs P products and three 128-bit coefficient fetches for 6 P DFMA.
+template <int P>
+__device__ __forceinline__ void matrix2_terms(const double* __restrict__ tt, const double (&v)[P][6], double (&w)[P][6]) {
+    const double2* t2 = reinterpret_cast<const double2*>(tt);
+    int q = 0;
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+#pragma unroll
+        for (int k = j; k < 6; k++) {
+            const double2 t01 = t2[3 * q], t23 = t2[3 * q + 1], t45 = t2[3 * q + 2];
+            const double t[6] = {t01.x, t01.y, t23.x, t23.y, t45.x, t45.y};
+#pragma unroll
+            for (int p = 0; p < P; p++) {
+                const double pr = v[p][j] * v[p][k];            // rounded product (-fmad=false: never contracted)
+#pragma unroll
+                for (int r = 0; r < 6; r++) w[p][r] = fma(t[r], pr, w[p][r]);
+            }
+            q++;
+        }
+    }
+}
+
 // DRIFT, RFKICK and the wake KICK, in place
 template <int P>
 __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, const ChainCommon& cm, double (&v)[P][6]) {
@@ -204,9 +230,10 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
     for (int op = 0; op < a.c.n_ops; op++) {
         const double* c = a.coef[op];
         const int ty = a.type[op];
-        if (ty == OP_MATRIX) {
+        if (ty == OP_MATRIX || ty == OP_MATRIX2) {
             double w[P][6];
             matrix_map<P>(c, v, w);
+            if (ty == OP_MATRIX2) { matrix2_terms<P>(c + 42, v, w); op += 3; }
 #pragma unroll
             for (int p = 0; p < P; p++)
 #pragma unroll
@@ -230,14 +257,15 @@ __device__ __forceinline__ void apply_ops_smem(const ChainArgs<MAXOPS>& a, const
             matrix_map_s128<P>(s_coef + 42 * op, v, w);
             matrix_map_s128<P>(s_coef + 42 * (op + 1), w, v);
             op += 2;
-        } else if (ty == OP_MATRIX) {
+        } else if (ty == OP_MATRIX || ty == OP_MATRIX2) {
             double w[P][6];
             matrix_map_s128<P>(s_coef + 42 * op, v, w);
+            if (ty == OP_MATRIX2) matrix2_terms<P>(s_coef + 42 * (op + 1), v, w);
 #pragma unroll
             for (int p = 0; p < P; p++)
 #pragma unroll
                 for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
-            op++;
+            op += (ty == OP_MATRIX2) ? 4 : 1;
         } else {
             other_map<P>(ty, s_coef + 42 * op, c, v);
             op++;

@@ -155,6 +155,35 @@ def test_long_run_ending_in_aperture(elg, elgo):
     check_lost(ob, gb)
 
 
+@pytest.mark.parametrize("n,n_cells", [(1, 1), (513, 1), (1537, 2), (100_003, 3), (40_001, 30)])
+def test_second_order_maps_bitexact(elg, elgo, n, n_cells):
+    """MATRIX2 (second-order transport map, G31) in short runs (parameter-bank kernel, 4 slots per map) and in
+    long runs (chain_long_kernel): bit-identical to the oracle, two turns."""
+    w = make_workload("p4-second-order", n=n, n_cells=n_cells, n_turns=2)
+    ob, oo, gb, go = both(elg, elgo, w, stage=False)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid)
+    assert np.array_equal(gv, ov)
+
+
+def test_second_order_mixed_with_other_maps(elg, elgo):
+    """MATRIX2 between MATRIX, DRIFT and RFKICK, then a collimator: slot accounting of the planner."""
+    from elg_inputs import second_order_drift, thin_quad_sextupole
+    m2 = lambda t: {"type": "MATRIX2", "R": t[0], "C": t[1], "T": t[2]}
+    lin = _long_line(23, {})[:5]
+    elems = [lin[0], m2(thin_quad_sextupole(0.3, 40.0)), {"type": "DRIFT", "L": 0.5}, m2(second_order_drift(0.7)),
+             lin[1], lin[2], {"type": "RFKICK", "V": 1e6, "f": 1.3e9, "phi": 0.4}, m2(thin_quad_sextupole(-0.3, -40.0)),
+             lin[3], m2(second_order_drift(1.1)), lin[4], {"type": "RCOL", "ax": 500e-6, "ay": 450e-6},
+             m2(thin_quad_sextupole(0.2, 10.0)), {"type": "DRIFT", "L": 0.3}]
+    v0 = make_workload("cfg0", n=60_001).particles()
+    ob = elgo.Bunch(v0, 1e9, 1e-9); ob.track(elgo.Beamline(elems), 1)
+    gbl = elg.Beamline(elems); gb = elg.Bunch(v0, 1e9, 1e-9, beamline=gbl); gb.track(gbl, 1)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert 0 < gid.size < 60_001 and np.array_equal(gid, oid)
+    assert np.array_equal(gv[:5], ov[:5]) and rel_err(gv, ov) <= 1e-12
+    check_lost(ob, gb)
+
+
 # ------------------------------------------------------------------------------------ (ii) loss
 def test_compaction_hand_placed(elg, elgo):
     """Edge-inclusive, NaN lost, Fig. 2 shape (20 particles, 4 lost)."""

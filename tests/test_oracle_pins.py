@@ -568,3 +568,67 @@ def test_track_loss_sequence_cfg4_small(elgo):
     # every lost record violates its aperture, at the recorded coordinates
     hw = np.array([0.9e-3 + (0.2e-3 - 0.9e-3) * (e // 3) / 19.0 for e in le])
     assert np.all((np.abs(lc[:, 0]) > hw) | (np.abs(lc[:, 2]) > hw))
+
+
+# ------------------------------------------------------------------------------------ MATRIX2 (G31)
+def test_matrix2_reduces_to_matrix_and_index_convention(elgo):
+    """T = 0 is elgo_matrix bit for bit; a single T entry (i; j,k) gives out_i = R-part + T v_j v_k, for every
+    (i, j <= k): catches a transposed or mis-ordered pair index."""
+    from elg_inputs import pair_index
+    rng = np.random.default_rng(5)
+    v0 = rng.normal(size=(6, 50)) * np.array([1e-3, 1e-4, 1e-3, 1e-4, 1e-2, 1e-3])[:, None]
+    R = np.eye(6) + 0.1 * rng.normal(size=(6, 6)); Cv = rng.normal(size=6) * 1e-3
+    a = v0.copy(); b = v0.copy()
+    elgo.matrix(a, R, Cv); elgo.matrix2(b, R, np.zeros((6, 21)), Cv)
+    assert np.array_equal(a, b)
+    seen = set()
+    for i in range(6):
+        for j in range(6):
+            for k in range(j, 6):
+                q = pair_index(j, k); seen.add(q)
+                T = np.zeros((6, 21)); T[i, q] = 3.0
+                b = v0.copy(); elgo.matrix2(b, np.eye(6), T)
+                exp = v0.copy(); exp[i] = exp[i] + 3.0 * (v0[j] * v0[k])
+                assert np.allclose(b, exp, rtol=0, atol=1e-18), (i, j, k)
+                others = [r for r in range(6) if r != i]
+                assert np.array_equal(b[others], v0[others])
+    assert seen == set(range(21)) and pair_index(2, 0) == pair_index(0, 2) == 2 and pair_index(5, 5) == 20
+
+
+def test_matrix2_sextupole_and_drift_closed_forms(elgo):
+    """Thin quadrupole + sextupole kick against its definition; the second-order drift against Listing 1's
+    exact drift: the path lengths differ by the next term of the expansion, -L/8 (x'^2+y'^2)^2."""
+    from elg_inputs import second_order_drift, thin_quad_sextupole
+    rng = np.random.default_rng(6)
+    v0 = rng.normal(size=(6, 200)) * np.array([1e-3, 1e-3, 1e-3, 1e-3, 1e-2, 1e-3])[:, None]
+    k1, k2 = 0.7, -35.0
+    R, Cv, T = thin_quad_sextupole(k1, k2)
+    a = v0.copy(); elgo.matrix2(a, R, T, Cv)
+    x, xp, y, yp = v0[:4]
+    assert np.array_equal(a[[0, 2, 4, 5]], v0[[0, 2, 4, 5]])
+    assert np.allclose(a[1], xp - k1 * x - 0.5 * k2 * (x * x - y * y), rtol=1e-15, atol=1e-20)
+    assert np.allclose(a[3], yp + k1 * y + k2 * x * y, rtol=1e-15, atol=1e-20)
+    L = 2.5
+    R, Cv, T = second_order_drift(L)
+    v1 = v0.copy(); v1[1] *= 10.0; v1[3] *= 10.0; v1[4] = 0.0                  # slopes ~1e-2: the O(x'^4) term is resolved
+    a = v1.copy(); elgo.matrix2(a, R, T, Cv)
+    e = v1.copy(); elgo.drift(e, L)
+    assert np.allclose(a[[0, 2]], e[[0, 2]], rtol=1e-15, atol=1e-20)
+    u = v1[1] * v1[1] + v1[3] * v1[3]
+    # sqrt(1 + u) = 1 + u/2 - u^2/8 + ...: the second-order map keeps L (1 + u/2), the exact drift has the rest
+    assert np.allclose(a[4] - e[4], L / 8.0 * u * u, rtol=2e-3, atol=1e-15)
+    assert np.allclose(a[4], L * (1.0 + 0.5 * u), rtol=1e-15, atol=0)
+
+
+def test_matrix2_in_track(elgo):
+    """elgo_track applies MATRIX2 elements in order and counts C[4] into the design path length (G8)."""
+    w = make_workload("p4-second-order", n=300, n_cells=3)
+    v0 = w.particles()
+    ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C); bl = elgo.Beamline(w.elements, ring=True)
+    ob.track(bl, 2)
+    ref = v0.copy()
+    for _ in range(2):
+        for e in w.elements:
+            elgo.matrix2(ref, e["R"], e["T"], e["C"])
+    assert np.array_equal(ob.read()[0], ref)
+    assert bl.length == 3.0
