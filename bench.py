@@ -438,6 +438,26 @@ def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
                         "peak": hbm_peak, "frac": ach / hbm_peak, "frac_of_8TBs": ach / NOMINAL_HBM_GBS})
         out.append({"workload": name, "kernel": "whole pass", "ms_per_pass": ms_total / k,
                     "value": passes / (ms_total / k * 1e-3) / 1e6, "unit": UNIT, "n_alive_after": int(n_alive)})
+    # fp64-bound probe of the NEXT row: second-order maps in the long-run kernel
+    w = make_workload("p4-second-order", n=n0, n_cells=20)
+    bl = elg.Beamline(w.elements, ring=True)
+    for _ in range(3):
+        restore(); gb.track(bl, 1, moments_every="none", records=False)
+    gb.synchronize()
+    gb.profile(True); gb.profile_read()
+    for _ in range(args.probe_steps):
+        restore(); gb.track(bl, 1, moments_every="none", records=False)
+    gb.synchronize()
+    prof = gb.profile_read()
+    gb.profile(False)
+    n_l, ms = prof["chain_long"]
+    if n_l:
+        fl = flops_per_particle_turn(w.elements) * float(n0) * args.probe_steps
+        ach = fl / (ms * 1e-3) / 1e12
+        out.append({"workload": w.name, "kernel": "chain_long_kernel", "bound": "alu", "particles": int(n0),
+                    "maps_per_turn": len(w.elements), "avg_launch_ms": ms / n_l, "achieved": ach, "unit": "TFLOP/s",
+                    "peak": FP64_PEAK_TFLOPS, "frac": ach / FP64_PEAK_TFLOPS,
+                    "value": float(n0) * len(w.elements) * args.probe_steps / (ms * 1e-3) / 1e6, "value_unit": UNIT})
     return out
 
 
