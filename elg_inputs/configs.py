@@ -22,6 +22,7 @@ Element dictionaries (keys are the paper's/BASELINE.json's names):
   RCOL   {ax, ay}  ECOL {a, b}       collimators, PAPER.md:149,153
   WAKE   {nb, window, wake, ...}     longitudinal wake, PAPER.md:165
   HISTO  {nb, window, ...}           diagnostic time histogram only, PAPER.md:111
+  TRWAKE {nb, window, wake, ...}     transverse (dipole) wake, PAPER.md:164 (G32-G34)
 """
 from __future__ import annotations
 
@@ -37,7 +38,7 @@ C_LIGHT = 299792458.0
 
 WORKLOAD_NAMES = (
     "cfg0", "cfg1", "cfg2", "cfg3", "cfg3-literal", "cfg4",
-    "p1-chain", "p2-chain-rcol", "p3-matrices", "p4-second-order",
+    "p1-chain", "p2-chain-rcol", "p3-matrices", "p4-second-order", "p5-trwake",
 )
 
 
@@ -333,11 +334,33 @@ def _p4(n, n_cells=100, n_turns=1):
                     elems, "gauss6", notes=f"{2 * n_cells} second-order maps per turn")
 
 
+def _p5(n, n_turns=1):
+    """Transverse wake line (track_through_trwake): an offset bunch through two TRWAKE
+    elements (transverse resonator, tabulated dipole wake) and a WAKE, drifts in between (readings G32-G34)."""
+    off = np.zeros(6); off[0] = 2e-4; off[2] = -1e-4
+    tt = np.arange(1024) * 0.02e-12
+    table = 1e17 * np.sin(2 * np.pi * 5e9 * tt) * np.exp(-tt / 8e-12)          # V/C/m, W_T(0) = 0
+    elems = [
+        _matrix_elem(np.eye(6), off),
+        {"type": "DRIFT", "L": 1.0},
+        {"type": "TRWAKE", "nb": 512, "window": "AUTO_MINMAX", "wake": "RESONATOR_T", "f": 3e9, "Q": 20.0, "Rs": 1e6,
+         "interp": True},
+        {"type": "DRIFT", "L": 0.5},
+        {"type": "TRWAKE", "nb": 2048, "window": "AUTO_TABLE", "wake": "TABLE", "table": table, "dt_table": 0.02e-12,
+         "interp": True},
+        {"type": "WAKE", "nb": 512, "window": "AUTO_MINMAX", "wake": "RESONATOR", "f": 1e9, "Q": 1.0, "Rs": 1e3,
+         "interp": True},
+        {"type": "DRIFT", "L": 0.25},
+    ]
+    return Workload("p5-trwake", 0, n or 100_000_000, 1e9, 1e-9, False, n_turns, "none", elems, "gauss6",
+                    notes="offset bunch, TRWAKE resonator + TRWAKE table + WAKE")
+
+
 def make_workload(name: str, n: Optional[int] = None, **kw) -> Workload:
     """name in WORKLOAD_NAMES; n overrides the particle count (reduced-size parity cases)."""
     table = {
         "cfg0": _cfg0, "cfg1": _cfg1, "cfg2": _cfg2, "cfg3": _cfg3, "cfg3-literal": _cfg3_literal,
-        "cfg4": _cfg4, "p1-chain": _p1, "p2-chain-rcol": _p2, "p3-matrices": _p3, "p4-second-order": _p4,
+        "cfg4": _cfg4, "p1-chain": _p1, "p2-chain-rcol": _p2, "p3-matrices": _p3, "p4-second-order": _p4, "p5-trwake": _p5,
     }
     if name not in table:
         raise KeyError(f"unknown workload {name!r}; known: {WORKLOAD_NAMES}")

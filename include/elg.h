@@ -39,11 +39,11 @@ enum { ELG_OK = 0, ELG_EINVAL = -1, ELG_ENOMEM = -2, ELG_ECUDA = -3, ELG_ESTATE 
 
 /* element types (glossary PAPER.md:175; Table I rows PAPER.md:143-165) */
 enum { ELG_DRIFT = 1, ELG_MATRIX = 2, ELG_RFKICK = 3, ELG_RCOL = 4, ELG_ECOL = 5, ELG_WAKE = 6, ELG_HISTO = 7,
-       ELG_MATRIX2 = 8 };
+       ELG_MATRIX2 = 8, ELG_TRWAKE = 9 };
 /* histogram window modes (G10) */
 enum { ELG_WIN_EXPLICIT = 0, ELG_WIN_AUTO_MINMAX = 1, ELG_WIN_AUTO_TABLE = 2 };
 /* wake kinds (G12) */
-enum { ELG_WAKE_RESONATOR = 0, ELG_WAKE_TABLE = 1 };
+enum { ELG_WAKE_RESONATOR = 0, ELG_WAKE_TABLE = 1, ELG_WAKE_RESONATOR_T = 2 /* transverse resonator, TRWAKE only */ };
 /* when elg_track records moments (G26) */
 enum { ELG_MOM_NONE = 0, ELG_MOM_TURN = 1, ELG_MOM_ELEMENT = 2 };
 
@@ -65,6 +65,11 @@ enum { ELG_MOM_NONE = 0, ELG_MOM_TURN = 1, ELG_MOM_ELEMENT = 2 };
  *                                   (f, Q, Rs) or (table, n_table, dt_table), interp (1 = linear between
  *                                   bin centres, 0 = own bin)
  *   HISTO: nb, window, t_lo_rel, dt: time histogram only (diagnostic), no kick
+ *   TRWAKE (track_through_trwake; G32-G34): fields as WAKE, wake kind RESONATOR_T (f, Q, Rs in
+ *                                   Ohm/m) or TABLE [V/C/m].  Per time bin the dipole sums Dx = sum x, Dy = sum y
+ *                                   (accumulated exactly in 64-bit fixed point, G33), Vx_i = q sum_{j<=i} Dx_j W_{i-j},
+ *                                   x' += Vx(t)/(beta0 p0c), y' += Vy(t)/(beta0 p0c), interpolated as for WAKE.
+ *                                   Stage outputs: counts -> hist_out; Dx, Dy, Vx, Vy (4 nb doubles) -> V_out
  */
 typedef struct {
     int32_t type;

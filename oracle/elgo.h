@@ -18,6 +18,8 @@
  *   elgo_wake_samples pinned  - beam-loading theorem, independent evaluation
  *   elgo_convolve     pinned  - brute-force double loop, numpy.convolve, continuous closed form
  *   elgo_kick         pinned  - bin-centre / midpoint / clamped cases
+ *   elgo_dipole_histogram, elgo_convolve_d, elgo_tkick (TRWAKE)  pinned - plain weighted sums, brute-force
+ *                               convolution, two-particle closed form, zero offset => zero kick, linearity
  *   elgo_moments      pinned  - symmetric hand sets, shift invariance, Gaussian statistics
  *   elgo_track on whole configs: PARITY UNPINNED by the paper (no published end-to-end values);
  *                     it is the composition of the pinned stages in the order of PAPER.md:51.
@@ -38,11 +40,11 @@ enum { ELGO_OK = 0, ELGO_EINVAL = -1, ELGO_ENOMEM = -2, ELGO_ESTATE = -4, ELGO_E
 
 /* element types (names: PAPER.md:175 glossary; north_star) */
 enum { ELGO_DRIFT = 1, ELGO_MATRIX = 2, ELGO_RFKICK = 3, ELGO_RCOL = 4, ELGO_ECOL = 5,
-       ELGO_WAKE = 6, ELGO_HISTO = 7, ELGO_MATRIX2 = 8 };
+       ELGO_WAKE = 6, ELGO_HISTO = 7, ELGO_MATRIX2 = 8, ELGO_TRWAKE = 9 };
 /* histogram window modes (G10) */
 enum { ELGO_WIN_EXPLICIT = 0, ELGO_WIN_AUTO_MINMAX = 1, ELGO_WIN_AUTO_TABLE = 2 };
 /* wake kinds (G12) */
-enum { ELGO_WAKE_RESONATOR = 0, ELGO_WAKE_TABLE = 1 };
+enum { ELGO_WAKE_RESONATOR = 0, ELGO_WAKE_TABLE = 1, ELGO_WAKE_RESONATOR_T = 2 /* transverse, G34 */ };
 /* when elgo_track records moments (G26) */
 enum { ELGO_MOM_NONE = 0, ELGO_MOM_TURN = 1, ELGO_MOM_ELEMENT = 2 };
 
@@ -55,6 +57,7 @@ enum { ELGO_MOM_NONE = 0, ELGO_MOM_TURN = 1, ELGO_MOM_ELEMENT = 2 };
  *   RCOL  : ax, ay [m]      ECOL: ax=a, ay=b [m]
  *   WAKE  : nb, window, (t_lo_rel, dt if EXPLICIT), wake kind, (f, Q, Rs) or (table, n_table, dt_table), interp
  *   HISTO : nb, window, t_lo_rel, dt   (histogram only, no kick)
+ *   TRWAKE: as WAKE, wake kind RESONATOR_T or TABLE [V/C/m]: transverse (dipole) wake, kicks x' and y' (G32-G34)
  */
 typedef struct {
     int32_t type;
@@ -101,6 +104,15 @@ int64_t elgo_histogram(const double* s, int64_t n, double inv_bc, double t_lo, d
 int32_t elgo_wake_samples(int32_t kind, int32_t nb, double dt, double f, double Q, double Rs,
                           const double* table, int64_t n_table, double dt_table, double* W);
 void   elgo_convolve(const uint32_t* counts, const double* W, int32_t nb, double q, double* Vout);
+/* TRWAKE (G32-G34): counts[nb] and the per-bin dipole sums Dx[nb], Dy[nb] = sum of x, y of the particles in the
+   bin, accumulated exactly in two 64-bit fixed-point words (G33), hence independent of the summation order */
+int64_t elgo_dipole_histogram(const double* s, const double* x, const double* y, int64_t n, double inv_bc, double t_lo,
+                              double inv_dt, int32_t nb, uint32_t* counts, double* Dx, double* Dy);
+/* V_i = q sum_{j<=i} D_j W_{i-j} (G13 with real weights) */
+void   elgo_convolve_d(const double* D, const double* W, int32_t nb, double q, double* Vout);
+/* x' += Vx(t)/(beta0 p0c), y' += Vy(t)/(beta0 p0c), interpolation as elgo_kick (G14) */
+void   elgo_tkick(const double* s, double* xp, double* yp, int64_t n, double inv_bc, double t_lo, double inv_dt,
+                  int32_t nb, const double* Vx, const double* Vy, double inv_E, int32_t interp);
 void   elgo_kick(const double* s, double* delta, int64_t n, double inv_bc, double t_lo, double inv_dt,
                  int32_t nb, const double* V, double inv_E, int32_t interp);
 /* n>0 required. centroid[6], sigma[36] row-major, population (1/n) central moments (G20). */
@@ -130,7 +142,7 @@ typedef struct {
     uint32_t* hist_out;          /* nullable; histograms of successive WAKE/HISTO executions, nb each */
     int64_t hist_capacity;       /* in uint32 entries */
     int64_t hist_written;        /* out */
-    double* V_out;               /* nullable; V arrays of successive WAKE executions */
+    double* V_out;               /* nullable; V arrays of successive WAKE executions; a TRWAKE appends Dx, Dy, Vx, Vy */
     int64_t V_capacity;
     int64_t V_written;           /* out */
     double* window_out;          /* nullable; (t_lo, dt, inv_dt) of successive WAKE/HISTO executions */

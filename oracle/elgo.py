@@ -25,9 +25,9 @@ _HDR = os.path.join(_HERE, "elgo.h")
 _LIB = os.path.join(_HERE, "libelgo.so")
 
 OK, EINVAL, ENOMEM, ESTATE, ECAPACITY = 0, -1, -2, -4, -5
-DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2 = 1, 2, 3, 4, 5, 6, 7, 8
+DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2, TRWAKE = 1, 2, 3, 4, 5, 6, 7, 8, 9
 WIN = {"EXPLICIT": 0, "AUTO_MINMAX": 1, "AUTO_TABLE": 2}
-WAKEKIND = {"RESONATOR": 0, "TABLE": 1}
+WAKEKIND = {"RESONATOR": 0, "TABLE": 1, "RESONATOR_T": 2}
 MOM = {"none": 0, "turn": 1, "element": 2}
 ELECTRON_MC2_EV = 0.51099895e6
 
@@ -104,6 +104,14 @@ def lib():
         L.elgo_kick.argtypes = [_dp, _dp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32,
                                 _dp, C.c_double, C.c_int32]
         L.elgo_kick.restype = None
+        L.elgo_dipole_histogram.argtypes = [_dp, _dp, _dp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32,
+                                            _u32p, _dp, _dp]
+        L.elgo_dipole_histogram.restype = C.c_int64
+        L.elgo_convolve_d.argtypes = [_dp, _dp, C.c_int32, C.c_double, _dp]
+        L.elgo_convolve_d.restype = None
+        L.elgo_tkick.argtypes = [_dp, _dp, _dp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32,
+                                 _dp, _dp, C.c_double, C.c_int32]
+        L.elgo_tkick.restype = None
         L.elgo_moments.argtypes = [v6, C.c_int64, _dp, _dp]
         L.elgo_moments.restype = C.c_int32
         for name in ("elgo_beta0",):
@@ -233,6 +241,28 @@ def kick(s: np.ndarray, delta: np.ndarray, inv_bc, t_lo, inv_dt, nb, V, inv_E, i
     lib().elgo_kick(_p(s), _p(delta), s.shape[0], inv_bc, t_lo, inv_dt, nb, _p(V), inv_E, 1 if interp else 0)
 
 
+def dipole_histogram(s, x, y, inv_bc: float, t_lo: float, inv_dt: float, nb: int):
+    """TRWAKE stage (G32, G33): counts and exact per-bin dipole sums.  Returns (counts, Dx, Dy, binned)."""
+    s = _f64(s); x = _f64(x); y = _f64(y)
+    counts = np.empty(nb, dtype=np.uint32); Dx = np.empty(nb); Dy = np.empty(nb)
+    binned = lib().elgo_dipole_histogram(_p(s), _p(x), _p(y), s.shape[0], inv_bc, t_lo, inv_dt, nb,
+                                         _p(counts, _u32p), _p(Dx), _p(Dy))
+    return counts, Dx, Dy, binned
+
+
+def convolve_d(D, W, q: float) -> np.ndarray:
+    D = _f64(D); W = _f64(W)
+    V = np.empty(D.shape[0], dtype=np.float64)
+    lib().elgo_convolve_d(_p(D), _p(W), D.shape[0], q, _p(V))
+    return V
+
+
+def tkick(s, xp, yp, inv_bc, t_lo, inv_dt, nb, Vx, Vy, inv_E, interp=True) -> None:
+    Vx = _f64(Vx); Vy = _f64(Vy)
+    lib().elgo_tkick(_p(s), _p(xp), _p(yp), s.shape[0], inv_bc, t_lo, inv_dt, nb, _p(Vx), _p(Vy), inv_E,
+                     1 if interp else 0)
+
+
 def moments(v: np.ndarray):
     cen = np.empty(6); sig = np.empty(36)
     rc = lib().elgo_moments(_v6(v), v.shape[1], _p(cen), _p(sig))
@@ -279,16 +309,16 @@ def _elements_to_c(elements):
             e.type, e.ax, e.ay = RCOL, float(d["ax"]), float(d["ay"])
         elif t == "ECOL":
             e.type, e.ax, e.ay = ECOL, float(d["a"]), float(d["b"])
-        elif t in ("WAKE", "HISTO"):
-            e.type = WAKE if t == "WAKE" else HISTO
+        elif t in ("WAKE", "HISTO", "TRWAKE"):
+            e.type = {"WAKE": WAKE, "HISTO": HISTO, "TRWAKE": TRWAKE}[t]
             e.nb = int(d["nb"])
             e.window = WIN[d["window"]]
             e.t_lo_rel = float(d.get("t_lo_rel", 0.0))
             e.dt = float(d.get("dt", 0.0))
-            if t == "WAKE":
+            if t != "HISTO":
                 e.wake = WAKEKIND[d["wake"]]
                 e.interp = 1 if d.get("interp", True) else 0
-                if d["wake"] == "RESONATOR":
+                if d["wake"] in ("RESONATOR", "RESONATOR_T"):
                     e.f, e.Q, e.Rs = float(d["f"]), float(d["Q"]), float(d["Rs"])
                 else:
                     tb = _f64(d["table"]); keep.append(tb)
@@ -355,9 +385,9 @@ class Bunch:
         o.records, o.capacity_records = _p(rec), n_rec
         hist = V = win = None
         if want_stage_outputs:
-            nh = sum(e["nb"] for e in bl.elements if e["type"] in ("WAKE", "HISTO")) * n_turns
-            nv = sum(e["nb"] for e in bl.elements if e["type"] == "WAKE") * n_turns
-            nw = sum(1 for e in bl.elements if e["type"] in ("WAKE", "HISTO")) * n_turns
+            nh = sum(e["nb"] for e in bl.elements if e["type"] in ("WAKE", "HISTO", "TRWAKE")) * n_turns
+            nv = sum(e["nb"] * {"WAKE": 1, "TRWAKE": 4}[e["type"]] for e in bl.elements if e["type"] in ("WAKE", "TRWAKE")) * n_turns
+            nw = sum(1 for e in bl.elements if e["type"] in ("WAKE", "HISTO", "TRWAKE")) * n_turns
             hist = np.zeros(max(nh, 1), dtype=np.uint32)
             V = np.zeros(max(nv, 1), dtype=np.float64)
             win = np.zeros((max(nw, 1), 3), dtype=np.float64)

@@ -78,6 +78,9 @@ struct elg_bunch {
     unsigned int* counts = nullptr;
     double* W = nullptr;
     double* V = nullptr;
+    unsigned long long* dacc = nullptr;
+    double* D = nullptr;
+    double* Vt = nullptr;
     double* table = nullptr;
     long long nb_cap = 0, table_cap = 0;
     long long* lost_id = nullptr;
@@ -94,7 +97,7 @@ struct elg_bunch {
     int sms = 0;
     int grid_chain[3][2] = {{0, 0}, {0, 0}, {0, 0}};    // [variant][compact]; variants: <8 ops, P=2>, <8, P=4>, long run <80, P=6>
     int force_p = 0;                                    // ELG_CHAIN_P = 2 | 4 overrides the planner's choice
-    int grid_hist = 0, grid_mom = 0;
+    int grid_hist = 0, grid_mom = 0, grid_dipole = 0;
     int hist_aggregate = 0;
     // optional per-kernel event timing (elg_profile_*)
     bool prof_on = false;
@@ -150,7 +153,7 @@ struct ProfScope {
 
 // ------------------------------------------------------------------------------------- workspace
 struct WorkLayout {
-    long long off_state, off_soaB, off_status, off_mm, off_mom, off_rec, off_counts, off_W, off_V, off_table,
+    long long off_state, off_soaB, off_status, off_mm, off_mom, off_rec, off_counts, off_W, off_V, off_dacc, off_D, off_Vt, off_table,
         off_lost_id, off_lost_te, off_lost_v, total;
 };
 
@@ -167,6 +170,9 @@ WorkLayout layout(long long n0, long long nb_cap, long long table_cap, long long
     L.off_counts = o; o = align_up(o + nb_cap * 4, 256);
     L.off_W = o; o = align_up(o + nb_cap * 8, 256);
     L.off_V = o; o = align_up(o + nb_cap * 8, 256);
+    L.off_dacc = o; o = align_up(o + 4 * nb_cap * 8, 256);         // TRWAKE: fixed-point dipole accumulators
+    L.off_D = o; o = align_up(o + 2 * nb_cap * 8, 256);            //         Dx, Dy
+    L.off_Vt = o; o = align_up(o + 2 * nb_cap * 8, 256);           //         Vx, Vy
     L.off_table = o; o = align_up(o + table_cap * 8, 256);
     L.off_lost_id = o; o = align_up(o + lost_cap * 8, 256);
     L.off_lost_te = o; o = align_up(o + lost_cap * 8, 256);
@@ -212,6 +218,7 @@ int32_t hist_setup_once() {
     static bool done = false;
     if (!done) {
         ELG_CK(cudaFuncSetAttribute(hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kHistSmemBins * 4));
+        ELG_CK(cudaFuncSetAttribute(dipole_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDipoleSmemBins * 36));
         done = true;
     }
     return ELG_OK;
@@ -259,13 +266,24 @@ extern "C" int32_t elg_beamline_load(elg_beamline** out, const elg_element* elem
             case ELG_RCOL: case ELG_ECOL:
                 if (!(e.ax > 0.0) || !(e.ay > 0.0)) why = "aperture: ax, ay must be > 0";
                 break;
-            case ELG_WAKE: case ELG_HISTO:
+            case ELG_WAKE: case ELG_HISTO: case ELG_TRWAKE:
                 if (e.nb < 2) { why = "WAKE/HISTO: nb < 2"; break; }
                 if (e.nb > (1 << 24)) { why = "WAKE/HISTO: nb > 2^24"; break; }
                 if (e.window < ELG_WIN_EXPLICIT || e.window > ELG_WIN_AUTO_TABLE) { why = "WAKE/HISTO: bad window mode"; break; }
                 if (e.window == ELG_WIN_EXPLICIT && (!(e.dt > 0.0) || !std::isfinite(e.t_lo_rel))) { why = "EXPLICIT window: dt > 0 and finite t_lo_rel required"; break; }
                 if (e.nb > bl->nb_max) bl->nb_max = e.nb;
-                if (e.type == ELG_WAKE) {
+                if (e.type == ELG_TRWAKE && e.wake == ELG_WAKE_RESONATOR) { why = "TRWAKE: wake kind must be RESONATOR_T or TABLE"; break; }
+                if (e.type == ELG_WAKE && e.wake == ELG_WAKE_RESONATOR_T) { why = "WAKE: RESONATOR_T is a transverse wake"; break; }
+                if (e.type == ELG_TRWAKE && e.wake == ELG_WAKE_RESONATOR_T) {
+                    if (!(e.Q > 0.5) || !(e.f > 0.0) || !std::isfinite(e.Rs)) { why = "resonator: Q > 1/2, f > 0, finite Rs required"; break; }
+                    const double wr = kTwoPi * e.f;                      // G34, same expressions as the definition
+                    ResConst rc;
+                    rc.alpha = wr / (2.0 * e.Q);
+                    rc.wbar = std::sqrt(wr * wr - rc.alpha * rc.alpha);
+                    rc.kloss = (wr * e.Rs / e.Q) * (wr / rc.wbar);       // amplitude
+                    rc.ratio = 0.0;
+                    bl->res[k] = rc;
+                } else if (e.type == ELG_WAKE || e.type == ELG_TRWAKE) {
                     if (e.wake == ELG_WAKE_RESONATOR) {
                         if (!(e.Q > 0.5) || !(e.f > 0.0) || !std::isfinite(e.Rs)) { why = "resonator: Q > 1/2, f > 0, finite Rs required"; break; }
                         // G12, same expressions as the definition, evaluated once here
@@ -282,8 +300,8 @@ extern "C" int32_t elg_beamline_load(elg_beamline** out, const elg_element* elem
                         bl->table_off[k] = bl->table_total;
                         bl->table_total += e.n_table;
                     } else { why = "WAKE: bad wake kind"; break; }
-                    if (e.window == ELG_WIN_AUTO_TABLE && e.wake != ELG_WAKE_TABLE) why = "AUTO_TABLE window needs a table wake";
                 }
+                if (!why && e.type != ELG_HISTO && e.window == ELG_WIN_AUTO_TABLE && e.wake != ELG_WAKE_TABLE) why = "AUTO_TABLE window needs a table wake";
                 break;
             default: why = "unknown element type";
         }
@@ -360,6 +378,9 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     b->counts = (unsigned int*)(w + L.off_counts);
     b->W = (double*)(w + L.off_W);
     b->V = (double*)(w + L.off_V);
+    b->dacc = (unsigned long long*)(w + L.off_dacc);
+    b->D = (double*)(w + L.off_D);
+    b->Vt = (double*)(w + L.off_Vt);
     b->table = (double*)(w + L.off_table);
     b->lost_id = (long long*)(w + L.off_lost_id);
     b->lost_te = (long long*)(w + L.off_lost_te);
@@ -377,6 +398,7 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     if (rc == ELG_OK) rc = hist_setup_once();
     if (rc == ELG_OK) rc = grid_for(hist_kernel, sms, kHistSmemBins * 4, kBlock, &b->grid_hist);
     if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, kBlock, &b->grid_mom);
+    if (rc == ELG_OK) rc = grid_for(dipole_hist_kernel, sms, kDipoleSmemBins * 36, kBlock, &b->grid_dipole);
     if (rc != ELG_OK) { delete b; return rc; }
     const char* agg = std::getenv("ELG_HIST_AGGREGATE");
     b->hist_aggregate = agg ? std::atoi(agg) : -1;                 // -1: automatic
@@ -446,6 +468,7 @@ struct Tracker {
     elg_track_opts* o;
     std::vector<HostOp> pending;
     int kick_nb = 0, kick_interp = 0;
+    int tk_nb = 0, tk_interp = 0;
     bool mm_valid = false;
     long long launches = 0;
     int32_t rc = ELG_OK;
@@ -481,6 +504,7 @@ struct Tracker {
         c.epoch = b->epoch;
         c.want_minmax = want_mm ? 1 : 0; c.mm_partial = b->mm_partial;
         c.V = b->V; c.nb = kick_nb; c.interp = kick_interp;
+        c.Vx = b->Vt; c.Vy = b->Vt + tk_nb; c.t_nb = tk_nb; c.t_interp = tk_interp;
         for (size_t k = 0; k < pending.size(); k++) {
             a.type[k] = pending[k].type;
             std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
@@ -517,6 +541,7 @@ struct Tracker {
                 case OP_DRIFT: rmask |= 0x1F; wmask |= 0x15; break;           // reads x x' y y' s, writes x y s
                 case OP_MATRIX: case OP_MATRIX2: rmask |= 0x3F; wmask |= 0x3F; break;
                 case OP_RFKICK: case OP_KICK: rmask |= 0x30; wmask |= 0x20; break;   // reads s delta, writes delta
+                case OP_TKICK: rmask |= 0x1A; wmask |= 0x0A; break;                  // reads x' y' s, writes x' y'
             }
         }
         if (want_mm) rmask |= 0x10;
@@ -592,25 +617,71 @@ struct Tracker {
             w.mode = e.window; w.nb = e.nb; w.t_lo_rel = e.t_lo_rel;
             w.dt_in = (e.window == ELG_WIN_AUTO_TABLE) ? e.dt_table : e.dt;
             w.t_design = s_here * b->inv_bc; w.inv_bc = b->inv_bc; w.counts = b->counts;
+            w.dacc = (e.type == ELG_TRWAKE) ? reinterpret_cast<long long*>(b->dacc) : nullptr;
             {
                 ProfScope ps(b, ELG_K_WINDOW);
                 window_kernel<<<(e.nb + 4 * kBlock - 1) / (4 * kBlock), kBlock, 0, b->stream>>>(w);
             }
             check(cudaGetLastError(), "window_kernel launch");
-            HistArgs h;
-            h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1;
-            h.inv_bc = b->inv_bc; h.t_lo = 0; h.inv_dt = 0; h.nb = e.nb; h.counts = b->counts;
-            h.aggregate = b->hist_aggregate < 0 ? 0 : b->hist_aggregate;
-            {
+            if (e.type == ELG_TRWAKE) {                               // counts + exact dipole sums (G33)
+                DipoleArgs d;
+                d.s = b->coord(b->cur_buf, 4); d.x = b->coord(b->cur_buf, 0); d.y = b->coord(b->cur_buf, 2);
+                d.st = b->st; d.cur = b->cur_slot; d.inv_bc = b->inv_bc; d.nb = e.nb; d.counts = b->counts; d.dacc = b->dacc;
+                ProfScope ps(b, ELG_K_HIST);
+                dipole_hist_kernel<<<b->grid_dipole, kBlock, kDipoleSmemBins * 36, b->stream>>>(d);
+            } else {
+                HistArgs h;
+                h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1;
+                h.inv_bc = b->inv_bc; h.t_lo = 0; h.inv_dt = 0; h.nb = e.nb; h.counts = b->counts;
+                h.aggregate = b->hist_aggregate < 0 ? 0 : b->hist_aggregate;
                 ProfScope ps(b, ELG_K_HIST);
                 hist_kernel<<<b->grid_hist, kBlock, kHistSmemBins * 4, b->stream>>>(h);
             }
             check(cudaGetLastError(), "hist_kernel launch");
             stage_out_hist(e.nb);
         } else if (o) { o->window_written++; o->hist_written += e.nb; }
-        if (e.type != ELG_WAKE) return;
+        if (e.type == ELG_HISTO) return;
         count();                                                      // wake samples
         count();                                                      // convolution
+        if (e.type == ELG_TRWAKE) {
+            count(); count();                                         // dipole sums -> doubles; second convolution
+            if (b) {
+                WakeArgs wa;
+                wa.st = b->st; wa.dt_fixed = 0.0; wa.kind = e.wake; wa.nb = e.nb;
+                const ResConst& r = bl->res[k];
+                wa.kloss = r.kloss; wa.alpha = r.alpha; wa.wbar = r.wbar; wa.ratio = r.ratio;
+                wa.table = b->table + bl->table_off[k]; wa.n_table = e.n_table; wa.dt_table = e.dt_table; wa.W = b->W;
+                {
+                    ProfScope ps(b, ELG_K_WAKE_SAMPLES);
+                    wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
+                }
+                check(cudaGetLastError(), "wake_samples_kernel launch");
+                {
+                    ProfScope ps(b, ELG_K_CONV);
+                    dipole_finalize_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(b->dacc, e.nb, b->D);
+                }
+                check(cudaGetLastError(), "dipole_finalize_kernel launch");
+                for (int plane = 0; plane < 2; plane++) {
+                    ConvArgs<double> cv;
+                    cv.counts = b->D + (size_t)plane * e.nb; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro;
+                    cv.V = b->Vt + (size_t)plane * e.nb;
+                    ProfScope ps(b, ELG_K_CONV);
+                    conv_kernel<double><<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
+                }
+                check(cudaGetLastError(), "conv_kernel launch");
+                if (o && o->V_out && o->V_written + 4LL * e.nb <= o->V_capacity) {
+                    check(cudaMemcpyAsync(o->V_out + o->V_written, b->D, (size_t)e.nb * 16, cudaMemcpyDeviceToHost, b->stream), "D D2H");
+                    check(cudaMemcpyAsync(o->V_out + o->V_written + 2LL * e.nb, b->Vt, (size_t)e.nb * 16, cudaMemcpyDeviceToHost, b->stream), "Vt D2H");
+                }
+            }
+            if (o) o->V_written += 4LL * e.nb;
+            HostOp op{};
+            op.type = OP_TKICK;
+            op.coef[0] = b ? b->inv_bc : 0.0; op.coef[1] = b ? b->inv_E : 0.0;
+            pending.push_back(op);
+            tk_nb = e.nb; tk_interp = e.interp;
+            return;
+        }
         if (b) {
             WakeArgs wa;
             wa.st = b->st; wa.dt_fixed = 0.0; wa.kind = e.wake; wa.nb = e.nb;
@@ -622,11 +693,11 @@ struct Tracker {
                 wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
             }
             check(cudaGetLastError(), "wake_samples_kernel launch");
-            ConvArgs cv;
+            ConvArgs<unsigned int> cv;
             cv.counts = b->counts; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro; cv.V = b->V;
             {
                 ProfScope ps(b, ELG_K_CONV);
-                conv_kernel<<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
+                conv_kernel<unsigned int><<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
             }
             check(cudaGetLastError(), "conv_kernel launch");
             if (o && o->V_out && o->V_written + e.nb <= o->V_capacity)
@@ -693,14 +764,14 @@ struct Tracker {
                           (turn << 32) | k, next_is_hist(k, ne));
                     break;
                 }
-                case ELG_WAKE: case ELG_HISTO: wake_or_histo(k, s_here); break;
+                case ELG_WAKE: case ELG_HISTO: case ELG_TRWAKE: wake_or_histo(k, s_here); break;
             }
             if (mom == ELG_MOM_ELEMENT) moments_record();                                    // G26
         }
         if (mom == ELG_MOM_TURN) moments_record();
     }
     bool next_is_hist(long long k, long long ne) const {
-        return (k + 1 < ne) && (bl->e[k + 1].type == ELG_WAKE || bl->e[k + 1].type == ELG_HISTO);
+        return (k + 1 < ne) && (bl->e[k + 1].type == ELG_WAKE || bl->e[k + 1].type == ELG_HISTO || bl->e[k + 1].type == ELG_TRWAKE);
     }
 };
 
@@ -886,9 +957,9 @@ extern "C" int32_t elg_dbg_wake_samples(int32_t kind, int32_t nb, double dt, dou
 extern "C" int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W, int32_t nb, double q, double* d_V,
                                     void* stream) {
     if (nb < 1 || !d_counts || !d_W || !d_V) return fail(ELG_EINVAL, "elg_dbg_convolve: bad arguments");
-    ConvArgs cv;
+    ConvArgs<unsigned int> cv;
     cv.counts = d_counts; cv.W = d_W; cv.st = nullptr; cv.nb = nb; cv.q = q; cv.V = d_V;
-    conv_kernel<<<(nb + kWarps - 1) / kWarps, kBlock, 0, (cudaStream_t)stream>>>(cv);
+    conv_kernel<unsigned int><<<(nb + kWarps - 1) / kWarps, kBlock, 0, (cudaStream_t)stream>>>(cv);
     g_launches++;
     ELG_CK(cudaGetLastError());
     return ELG_OK;

@@ -28,7 +28,8 @@ constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
 
 enum : uint8_t { OP_DRIFT = 1, OP_MATRIX = 2, OP_RFKICK = 3, OP_KICK = 4,
                  OP_MATRIX2 = 5,      // second-order map: this slot holds R, C; the next three hold T (OP_CONT)
-                 OP_CONT = 6 };
+                 OP_CONT = 6,
+                 OP_TKICK = 7 };      // transverse wake kick of the preceding TRWAKE (G32)
 enum { AP_NONE = 0, AP_RCOL = 1, AP_ECOL = 2 };
 
 // Device-resident tracking state (first bytes of the workspace).  Nothing here is read by the host
@@ -69,6 +70,10 @@ struct ChainCommon {
     const double* V;           // OP_KICK operands
     int nb;
     int interp;
+    const double* Vx;          // OP_TKICK operands
+    const double* Vy;
+    int t_nb;
+    int t_interp;
 };
 
 template <int MAXOPS>
@@ -221,6 +226,35 @@ __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, 
                 Vt = fma(fr, V1 - V0, V0);
             }
             v[p][5] = fma(-Vt, inv_E, v[p][5]);
+        }
+    } else if (ty == OP_TKICK) {                                 // G32: x' += Vx(t) / (beta0 p0c), y' likewise
+        const double inv_bc = c[0], inv_E = c[1];
+        const double t_lo = cm.st->win[0], inv_dt = cm.st->win[2];
+        const int nb = cm.t_nb;
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            double u0;
+            const int b = bin_of(v[p][4], inv_bc, t_lo, inv_dt, nb, &u0);
+            if (b < 0) continue;
+            double vx, vy;
+            if (!cm.t_interp || nb < 2) {
+                vx = __ldg(cm.Vx + b); vy = __ldg(cm.Vy + b);
+            } else {
+                const double u = u0 - 0.5;
+                double k = floor(u);
+                if (k < 0.0) k = 0.0;
+                if (k > (double)(nb - 2)) k = (double)(nb - 2);
+                double fr = u - k;
+                if (fr < 0.0) fr = 0.0;
+                if (fr > 1.0) fr = 1.0;
+                const int ki = (int)k;
+                const double x0 = __ldg(cm.Vx + ki), x1 = __ldg(cm.Vx + ki + 1);
+                const double y0 = __ldg(cm.Vy + ki), y1 = __ldg(cm.Vy + ki + 1);
+                vx = fma(fr, x1 - x0, x0);
+                vy = fma(fr, y1 - y0, y0);
+            }
+            v[p][1] = fma(vx, inv_E, v[p][1]);
+            v[p][3] = fma(vy, inv_E, v[p][3]);
         }
     }
 }
@@ -701,10 +735,13 @@ struct WindowArgs {
     int nb;
     double t_lo_rel, dt_in, t_design, inv_bc;
     unsigned int* counts;
+    long long* dacc;     // TRWAKE: 4 * nb fixed-point dipole accumulators to zero as well (or NULL)
 };
 
 __global__ void __launch_bounds__(kBlock) window_kernel(const WindowArgs a) {
     for (int i = blockIdx.x * kBlock + threadIdx.x; i < a.nb; i += gridDim.x * kBlock) a.counts[i] = 0u;   // all blocks
+    if (a.dacc)
+        for (int i = blockIdx.x * kBlock + threadIdx.x; i < 4 * a.nb; i += gridDim.x * kBlock) a.dacc[i] = 0;
     if (blockIdx.x != 0) return;                                 // block 0 derives the window
     __shared__ double s_mn[kWarps], s_mx[kWarps];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -831,6 +868,108 @@ __global__ void __launch_bounds__(kBlock) hist_kernel(const HistArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// dipole_hist_kernel (TRWAKE, G32-G33): bin counts and per-bin dipole sums of x and y.  A sum of doubles
+// accumulated with atomics would depend on the order of arrival; here every coordinate is split exactly into
+// two integers (hi = rint(x 2^32), lo = rint((x - hi 2^-32) 2^64)) which are summed with 64-bit INTEGER
+// atomics: exact, order-independent, run-to-run reproducible, and bit-identical to the sequential CPU sum.
+// Shared-memory privatisation of the occupied bin range as in hist_kernel (36 bytes per bin).
+// ---------------------------------------------------------------------------------------------------
+constexpr int kDipoleSmemBins = 1792;                   // 1792 x 36 B = 63 KB
+
+struct DipoleArgs {
+    const double* s;
+    const double* x;
+    const double* y;
+    const DevState* st;
+    int cur;
+    double inv_bc;
+    int nb;
+    unsigned int* counts;
+    unsigned long long* dacc;      // [nb][4]: x hi, x lo, y hi, y lo
+};
+
+__device__ __forceinline__ bool fixed_split(double x, long long* hi, long long* lo) {
+    if (!(fabs(x) < 1048576.0)) return false;
+    const double h = rint(x * 4294967296.0);
+    const double r = x - h * (1.0 / 4294967296.0);               // exact
+    *hi = (long long)h;
+    *lo = (long long)rint(r * 18446744073709551616.0);
+    return true;
+}
+
+__global__ void __launch_bounds__(kBlock) dipole_hist_kernel(const DipoleArgs a) {
+    extern __shared__ __align__(8) unsigned char sh_raw[];
+    const long long n = a.st->n_alive[a.cur];
+    const long long blo = a.st->bin_lo, bhi = a.st->bin_hi;
+    const double t_lo = a.st->win[0], inv_dt = a.st->win[2];
+    long long span = bhi - blo + 1;
+    if (span < 1) span = 1;
+    const int S = (int)(span < kDipoleSmemBins ? span : kDipoleSmemBins);
+    unsigned long long* sd = reinterpret_cast<unsigned long long*>(sh_raw);          // [S][4]
+    unsigned int* sc = reinterpret_cast<unsigned int*>(sh_raw + (size_t)S * 32);      // [S]
+    for (int i = threadIdx.x; i < S * 4; i += kBlock) sd[i] = 0ull;
+    for (int i = threadIdx.x; i < S; i += kBlock) sc[i] = 0u;
+    __syncthreads();
+    const long long stride = (long long)gridDim.x * kBlock * 2;
+    for (long long i0 = ((long long)blockIdx.x * kBlock + threadIdx.x) * 2; i0 < n; i0 += stride) {
+        double sv[2], xv[2], yv[2];
+        const bool two = i0 + 2 <= n;
+        if (two) {
+            const double2 ts = ld_stream2(a.s + i0), tx = ld_stream2(a.x + i0), ty = ld_stream2(a.y + i0);
+            sv[0] = ts.x; sv[1] = ts.y; xv[0] = tx.x; xv[1] = tx.y; yv[0] = ty.x; yv[1] = ty.y;
+        } else {
+            sv[0] = ld_stream1(a.s + i0); xv[0] = ld_stream1(a.x + i0); yv[0] = ld_stream1(a.y + i0);
+            sv[1] = 0.0; xv[1] = 0.0; yv[1] = 0.0;
+        }
+#pragma unroll
+        for (int p = 0; p < 2; p++) {
+            if (p == 1 && !two) break;
+            double u;
+            const int b = bin_of(sv[p], a.inv_bc, t_lo, inv_dt, a.nb, &u);
+            if (b < 0) continue;
+            long long xh, xl, yh, yl;
+            const bool ok = fixed_split(xv[p], &xh, &xl) & fixed_split(yv[p], &yh, &yl);
+            const long long rel = (long long)b - blo;
+            if (rel < S) {
+                atomicAdd(sc + rel, 1u);
+                if (ok) {
+                    atomicAdd(sd + 4 * rel + 0, (unsigned long long)xh); atomicAdd(sd + 4 * rel + 1, (unsigned long long)xl);
+                    atomicAdd(sd + 4 * rel + 2, (unsigned long long)yh); atomicAdd(sd + 4 * rel + 3, (unsigned long long)yl);
+                }
+            } else {
+                atomicAdd(a.counts + b, 1u);
+                if (ok) {
+                    atomicAdd(a.dacc + 4 * (long long)b + 0, (unsigned long long)xh); atomicAdd(a.dacc + 4 * (long long)b + 1, (unsigned long long)xl);
+                    atomicAdd(a.dacc + 4 * (long long)b + 2, (unsigned long long)yh); atomicAdd(a.dacc + 4 * (long long)b + 3, (unsigned long long)yl);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < S; i += kBlock) {
+        const unsigned int cnt = sc[i];
+        if (cnt) {
+            atomicAdd(a.counts + blo + i, cnt);
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                const unsigned long long v = sd[4 * i + k];
+                if (v) atomicAdd(a.dacc + 4 * (blo + i) + k, v);
+            }
+        }
+    }
+}
+
+// D = fma((double)H, 2^-32, (double)L 2^-64) (G33), Dx then Dy
+__global__ void __launch_bounds__(kBlock) dipole_finalize_kernel(const unsigned long long* dacc, int nb, double* D) {
+    const int k = blockIdx.x * kBlock + threadIdx.x;
+    if (k >= nb) return;
+    const long long xh = (long long)dacc[4 * k + 0], xl = (long long)dacc[4 * k + 1];
+    const long long yh = (long long)dacc[4 * k + 2], yl = (long long)dacc[4 * k + 3];
+    D[k] = fma((double)xh, 1.0 / 4294967296.0, (double)xl * (1.0 / 18446744073709551616.0));
+    D[nb + k] = fma((double)yh, 1.0 / 4294967296.0, (double)yl * (1.0 / 18446744073709551616.0));
+}
+
+// ---------------------------------------------------------------------------------------------------
 // wake_samples_kernel (a10; G11, G12): W_k = W(k dt), k < nb, in V/C.
 // ---------------------------------------------------------------------------------------------------
 struct WakeArgs {
@@ -850,7 +989,13 @@ __global__ void __launch_bounds__(kBlock) wake_samples_kernel(const WakeArgs a) 
     if (k >= a.nb) return;
     const double dt = (a.dt_fixed > 0.0) ? a.dt_fixed : a.st->win[1];
     double w;
-    if (a.kind == 0) {
+    if (a.kind == 2) {                                                       // transverse resonator (G34)
+        if (k == 0) w = 0.0;
+        else {
+            const double tau = (double)k * dt;
+            w = a.kloss * exp(-a.alpha * tau) * sin(a.wbar * tau);          // kloss holds (w_r Rs / Q)(w_r / wbar)
+        }
+    } else if (a.kind == 0) {
         if (k == 0) w = a.kloss;                                             // beam-loading theorem (G11)
         else {
             const double tau = (double)k * dt;
@@ -881,8 +1026,9 @@ __global__ void __launch_bounds__(kBlock) wake_samples_kernel(const WakeArgs a) 
 // so the result is run-to-run deterministic.  Empty bins outside the occupied range are skipped
 // (they contribute exact zeros).
 // ---------------------------------------------------------------------------------------------------
+template <class T>
 struct ConvArgs {
-    const unsigned int* counts;
+    const T* counts;       // weights: bin counts (WAKE) or dipole sums (TRWAKE)
     const double* W;
     const DevState* st;    // occupied range; NULL: whole range
     int nb;
@@ -890,7 +1036,8 @@ struct ConvArgs {
     double* V;
 };
 
-__global__ void __launch_bounds__(kBlock) conv_kernel(const ConvArgs a) {
+template <class T>
+__global__ void __launch_bounds__(kBlock) conv_kernel(const ConvArgs<T> a) {
     const int lane = threadIdx.x & 31;
     const int i = blockIdx.x * kWarps + (threadIdx.x >> 5);
     if (i >= a.nb) return;

@@ -15,9 +15,9 @@ import numpy as np
 from .build import LIB, build
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ECAPACITY = 0, -1, -2, -3, -4, -5
-DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2 = 1, 2, 3, 4, 5, 6, 7, 8
+DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2, TRWAKE = 1, 2, 3, 4, 5, 6, 7, 8, 9
 WIN = {"EXPLICIT": 0, "AUTO_MINMAX": 1, "AUTO_TABLE": 2}
-WAKEKIND = {"RESONATOR": 0, "TABLE": 1}
+WAKEKIND = {"RESONATOR": 0, "TABLE": 1, "RESONATOR_T": 2}
 MOM = {"none": 0, "turn": 1, "element": 2}
 ELECTRON_MC2_EV = 0.51099895e6
 
@@ -178,16 +178,16 @@ def _elements_to_c(elements):
             e.type, e.ax, e.ay = RCOL, float(d["ax"]), float(d["ay"])
         elif t == "ECOL":
             e.type, e.ax, e.ay = ECOL, float(d["a"]), float(d["b"])
-        elif t in ("WAKE", "HISTO"):
-            e.type = WAKE if t == "WAKE" else HISTO
+        elif t in ("WAKE", "HISTO", "TRWAKE"):
+            e.type = {"WAKE": WAKE, "HISTO": HISTO, "TRWAKE": TRWAKE}[t]
             e.nb = int(d["nb"])
             e.window = WIN[d["window"]]
             e.t_lo_rel = float(d.get("t_lo_rel", 0.0))
             e.dt = float(d.get("dt", 0.0))
-            if t == "WAKE":
+            if t != "HISTO":
                 e.wake = WAKEKIND[d["wake"]]
                 e.interp = 1 if d.get("interp", True) else 0
-                if d["wake"] == "RESONATOR":
+                if d["wake"] in ("RESONATOR", "RESONATOR_T"):
                     e.f, e.Q, e.Rs = float(d["f"]), float(d["Q"]), float(d["Rs"])
                 else:
                     tb = _f64(d["table"]); keep.append(tb)
@@ -310,9 +310,9 @@ class Bunch:
             o.records, o.capacity_records = _p(rec), n_rec
         hist = V = win = None
         if want_stage_outputs:
-            nh = sum(e["nb"] for e in bl.elements if e["type"] in ("WAKE", "HISTO")) * n_turns
-            nv = sum(e["nb"] for e in bl.elements if e["type"] == "WAKE") * n_turns
-            nw = sum(1 for e in bl.elements if e["type"] in ("WAKE", "HISTO")) * n_turns
+            nh = sum(e["nb"] for e in bl.elements if e["type"] in ("WAKE", "HISTO", "TRWAKE")) * n_turns
+            nv = sum(e["nb"] * {"WAKE": 1, "TRWAKE": 4}[e["type"]] for e in bl.elements if e["type"] in ("WAKE", "TRWAKE")) * n_turns
+            nw = sum(1 for e in bl.elements if e["type"] in ("WAKE", "HISTO", "TRWAKE")) * n_turns
             hist = np.zeros(max(nh, 1), dtype=np.uint32)
             V = np.zeros(max(nv, 1), dtype=np.float64)
             win = np.zeros((max(nw, 1), 3), dtype=np.float64)

@@ -421,6 +421,49 @@ def test_cfg4_end_to_end(elg, elgo):
     assert nl + gid.size == w.n0 and nl / w.n0 > 0.9
 
 
+@pytest.mark.parametrize("n", [1, 2, 1000, 300_007])
+def test_trwake_end_to_end(elg, elgo, n):
+    """TRWAKE (G32-G34): counts and the exact fixed-point dipole sums bit-identical, Vx / Vy to 1e-10 of their
+    maximum, coordinates to 1e-12 (the transverse kicks feed x, y and s through the following drifts)."""
+    w = make_workload("p5-trwake", n=n)
+    ob, oo, gb, go = both(elg, elgo, w)
+    nb1, nb2 = w.elements[2]["nb"], w.elements[4]["nb"]
+    assert np.array_equal(go["window"][0], oo["window"][0])
+    assert np.array_equal(go["hist"][:nb1], oo["hist"][:nb1])
+    Vo, Vg = oo["V"], go["V"]
+    assert Vg.size == Vo.size == 4 * nb1 + 4 * nb2 + w.elements[5]["nb"]
+    assert np.array_equal(Vg[:2 * nb1], Vo[:2 * nb1]), "dipole sums of the first TRWAKE"
+    for lo, hi in ((2 * nb1, 3 * nb1), (3 * nb1, 4 * nb1)):
+        m = np.max(np.abs(Vo[lo:hi]))
+        assert np.max(np.abs(Vg[lo:hi] - Vo[lo:hi])) <= 1e-10 * m + 1e-300
+    if n > 2:
+        assert np.max(np.abs(Vo[2 * nb1:3 * nb1])) > 0
+    # later stages see coordinates that agree to ~1e-15 only: relative to their maximum
+    o2 = 4 * nb1
+    for k in range(4):
+        a, b_ = Vg[o2 + k * nb2: o2 + (k + 1) * nb2], Vo[o2 + k * nb2: o2 + (k + 1) * nb2]
+        assert np.max(np.abs(a - b_)) <= 1e-9 * np.max(np.abs(b_)) + 1e-300
+    assert int(go["hist"][nb1:nb1 + nb2].sum()) == int(oo["hist"][nb1:nb1 + nb2].sum())
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid)
+    if n > 2:
+        assert rel_err(gv, ov) <= 1e-12
+
+
+def test_trwake_run_to_run_deterministic(elg):
+    """Integer atomics: two runs give the same bits (a sum of doubles accumulated with atomics would not)."""
+    w = make_workload("p5-trwake", n=200_003)
+    v0 = w.particles()
+    outs = []
+    for _ in range(2):
+        bl = elg.Beamline(w.elements)
+        b = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=bl)
+        o = b.track(bl, 1, want_stage_outputs=True)
+        outs.append((b.read()[0], o["V"], o["hist"]))
+    for a, b_ in zip(outs[0], outs[1]):
+        assert np.array_equal(a, b_)
+
+
 def test_track_in_two_calls_equals_one(elg, elgo):
     """Turn counter, RF reference and lost log carry across elg_track calls."""
     w = make_workload("cfg3", n=5000, n_matrices=10, n_turns=6)

@@ -632,3 +632,100 @@ def test_matrix2_in_track(elgo):
             elgo.matrix2(ref, e["R"], e["T"], e["C"])
     assert np.array_equal(ob.read()[0], ref)
     assert bl.length == 3.0
+
+
+# ------------------------------------------------------------------------------------ TRWAKE (G32-G34)
+def test_dipole_histogram_is_the_plain_weighted_sum_and_order_free(elgo):
+    """G33: the fixed-point dipole sums equal the plain per-bin sums of x and y (<= 1e-14 of the largest), do not
+    depend on the particle order (bit for bit), and the counts are elgo_histogram's."""
+    rng = np.random.default_rng(11)
+    n, nb = 200_000, 97
+    s = rng.normal(size=n) * 1e-3
+    x = rng.normal(size=n) * 1e-4 + 3e-5
+    y = rng.normal(size=n) * 2e-4 - 1e-5
+    inv_bc = elgo.inv_bc(elgo.beta0(1e9))
+    t_lo, dt, inv_dt = elgo.window(s, inv_bc, 1, nb)
+    c, Dx, Dy, binned = elgo.dipole_histogram(s, x, y, inv_bc, t_lo, inv_dt, nb)
+    c0, b0, bins = elgo.histogram(s, inv_bc, t_lo, inv_dt, nb, want_bins=True)
+    assert np.array_equal(c, c0) and binned == b0 == n
+    import math
+    for D, w in ((Dx, x), (Dy, y)):
+        ref = np.array([math.fsum(w[bins == k]) for k in range(nb)])              # exactly rounded sums
+        assert np.max(np.abs(D - ref)) <= 1e-14 * np.max(np.abs(ref))
+    p = rng.permutation(n)
+    c2, Dx2, Dy2, _ = elgo.dipole_histogram(s[p], x[p], y[p], inv_bc, t_lo, inv_dt, nb)
+    assert np.array_equal(Dx, Dx2) and np.array_equal(Dy, Dy2) and np.array_equal(c, c2)
+    # exactly representable offsets give exact sums; out-of-range / NaN offsets are counted but not summed
+    s3 = np.zeros(5); x3 = np.array([0.5, 0.25, -0.125, np.nan, 4.0e6]); y3 = np.ones(5)
+    c3, Dx3, Dy3, _ = elgo.dipole_histogram(s3, x3, y3, 1.0, -0.5, 1.0, 2)
+    assert c3.tolist() == [5, 0] and Dx3[0] == 0.625 and Dy3[0] == 3.0
+
+
+def test_convolve_d_bruteforce(elgo):
+    rng = np.random.default_rng(12)
+    D = rng.normal(size=40); W = rng.normal(size=40)
+    V = elgo.convolve_d(D, W, 2.5)
+    ref = np.array([2.5 * sum(D[j] * W[i - j] for j in range(i + 1)) for i in range(40)])
+    assert np.allclose(V, ref, rtol=1e-13, atol=1e-15)
+    assert np.allclose(V, 2.5 * np.convolve(D, W)[:40], rtol=1e-12, atol=1e-14)
+    assert V[0] == 2.5 * D[0] * W[0]                                              # causality
+
+
+def test_transverse_resonator_samples(elgo):
+    """G34 by independent evaluation: W_T(0) = 0, W_T(tau) = (w Rs/Q)(w/wbar) exp(-alpha tau) sin(wbar tau)."""
+    f, Q, Rs, dt = 3e9, 20.0, 1e6, 0.1e-12
+    W = elgo.wake_samples(2, 64, dt, f=f, Q=Q, Rs=Rs)
+    w = 2 * np.pi * f; al = w / (2 * Q); wb = np.sqrt(w * w - al * al)
+    tau = np.arange(64) * dt
+    ref = (w * Rs / Q) * (w / wb) * np.exp(-al * tau) * np.sin(wb * tau)
+    assert W[0] == 0.0 and np.allclose(W, ref, rtol=1e-13, atol=0)
+    assert W[1] > 0 and abs(W[1] / (w * Rs / Q * w * dt) - 1) < 1e-2              # initial slope w^2 Rs/Q
+
+
+def test_trwake_two_particle_closed_form_and_linearity(elgo):
+    """A leading particle with offset (x0, y0) kicks a trailing one m bins behind by q W_T(m dt) x0 / (beta0 p0c); the
+    leading one is not kicked (W_T(0) = 0); zero offsets give zero kicks; the kick is linear in the offsets."""
+    p0c, Qb = 1e9, 2e-9
+    b0 = elgo.beta0(p0c); inv_bc = elgo.inv_bc(b0); inv_E = elgo.inv_E(b0, p0c)
+    nb, dt, m = 64, 0.2e-12, 7
+    f, Q, Rs = 3e9, 20.0, 1e6
+    el = [{"type": "TRWAKE", "nb": nb, "window": "EXPLICIT", "t_lo_rel": -0.5 * dt, "dt": dt, "wake": "RESONATOR_T",
+           "f": f, "Q": Q, "Rs": Rs, "interp": True}]
+    def run(x0, y0, x1=0.0):
+        v = np.zeros((6, 2)); v[0] = [x0, x1]; v[2] = [y0, 0.0]
+        v[4, 1] = m * dt / inv_bc                                                  # bin centres 0 and m
+        ob = elgo.Bunch(v, p0c, Qb); ob.track(elgo.Beamline(el), 1)
+        return ob.read()[0]
+    W = elgo.wake_samples(2, nb, dt, f=f, Q=Q, Rs=Rs)
+    q = Qb / 2
+    out = run(1e-3, -2e-3)
+    assert out[1, 0] == 0.0 and out[3, 0] == 0.0
+    assert np.isclose(out[1, 1], q * W[m] * 1e-3 * inv_E, rtol=1e-12) and out[1, 1] != 0.0
+    assert np.isclose(out[3, 1], q * W[m] * -2e-3 * inv_E, rtol=1e-12)
+    assert np.array_equal(out[[0, 2, 4, 5]], run(1e-3, -2e-3)[[0, 2, 4, 5]])
+    zero = run(0.0, 0.0)
+    assert not zero[1].any() and not zero[3].any()
+    twice = run(2e-3, -4e-3)
+    assert np.allclose(twice[[1, 3]], 2 * out[[1, 3]], rtol=1e-13, atol=0)
+    # the trailing particle's own offset does not kick itself
+    assert np.array_equal(run(1e-3, -2e-3, x1=5e-3)[[1, 3]], out[[1, 3]])
+
+
+def test_trwake_track_is_the_composition_of_stages(elgo):
+    w = make_workload("p5-trwake", n=20_000)
+    v0 = w.particles()
+    ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
+    oo = ob.track(elgo.Beamline(w.elements), 1, want_stage_outputs=True)
+    b0 = elgo.beta0(w.p0c_eV); inv_bc = elgo.inv_bc(b0); inv_E = elgo.inv_E(b0, w.p0c_eV)
+    v = v0.copy()
+    elgo.matrix(v, w.elements[0]["R"], w.elements[0]["C"]); elgo.drift(v, 1.0)
+    e = w.elements[2]
+    t_lo, dt, inv_dt = elgo.window(v[4], inv_bc, 1, e["nb"])
+    c, Dx, Dy, _ = elgo.dipole_histogram(v[4], v[0], v[2], inv_bc, t_lo, inv_dt, e["nb"])
+    W = elgo.wake_samples(2, e["nb"], dt, f=e["f"], Q=e["Q"], Rs=e["Rs"])
+    q = w.charge_C / w.n0
+    Vx = elgo.convolve_d(Dx, W, q); Vy = elgo.convolve_d(Dy, W, q)
+    nb = e["nb"]
+    assert np.array_equal(oo["hist"][:nb], c)
+    assert np.array_equal(oo["V"][:4 * nb], np.concatenate([Dx, Dy, Vx, Vy]))
+    assert np.max(np.abs(Vx)) > 0 and abs(Dx.sum() / w.n0 - 2e-4) < 1e-5          # the bunch is offset by 200 um
