@@ -404,6 +404,8 @@ def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
         ("p1-chain", "none", {"chain": 96.0}),
         ("p2-chain-rcol", "none", {"chain_compact": 112.0}),
         ("cfg0", "turn", {"chain_compact": 112.0, "hist": 8.0, "moments": 48.0, "chain": 24.0}),
+        # NEXT row f1: two dipole histograms (s, x, y: 24 B) + one plain (8 B) = 56 B over 3 launches
+        ("p5-trwake", "none", {"hist": 56.0 / 3.0}),
     ]
     for name, mom, bytes_pp in cases:
         w = make_workload(name, n=n0)

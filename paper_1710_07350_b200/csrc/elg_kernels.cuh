@@ -897,6 +897,17 @@ __device__ __forceinline__ bool fixed_split(double x, long long* hi, long long* 
     return true;
 }
 
+// 64-bit integer add in shared memory from two native 32-bit atomics (a 64-bit shared atomicAdd compiles to a
+// compare-and-swap spin loop): add the low word, carry into the high word when the low word wrapped.  Addition
+// modulo 2^64 commutes, so the result does not depend on the interleaving.
+__device__ __forceinline__ void smem_add64(unsigned long long* p, unsigned long long v) {
+    unsigned int* w = reinterpret_cast<unsigned int*>(p);
+    const unsigned int lo = (unsigned int)v, hi = (unsigned int)(v >> 32);
+    const unsigned int old = atomicAdd(w, lo);
+    const unsigned int carry = (old + lo < old) ? 1u : 0u;
+    if (hi + carry) atomicAdd(w + 1, hi + carry);
+}
+
 __global__ void __launch_bounds__(kBlock) dipole_hist_kernel(const DipoleArgs a) {
     extern __shared__ __align__(8) unsigned char sh_raw[];
     const long long n = a.st->n_alive[a.cur];
@@ -933,8 +944,8 @@ __global__ void __launch_bounds__(kBlock) dipole_hist_kernel(const DipoleArgs a)
             if (rel < S) {
                 atomicAdd(sc + rel, 1u);
                 if (ok) {
-                    atomicAdd(sd + 4 * rel + 0, (unsigned long long)xh); atomicAdd(sd + 4 * rel + 1, (unsigned long long)xl);
-                    atomicAdd(sd + 4 * rel + 2, (unsigned long long)yh); atomicAdd(sd + 4 * rel + 3, (unsigned long long)yl);
+                    smem_add64(sd + 4 * rel + 0, (unsigned long long)xh); smem_add64(sd + 4 * rel + 1, (unsigned long long)xl);
+                    smem_add64(sd + 4 * rel + 2, (unsigned long long)yh); smem_add64(sd + 4 * rel + 3, (unsigned long long)yl);
                 }
             } else {
                 atomicAdd(a.counts + b, 1u);
