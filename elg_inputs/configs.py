@@ -38,7 +38,7 @@ C_LIGHT = 299792458.0
 
 WORKLOAD_NAMES = (
     "cfg0", "cfg1", "cfg2", "cfg3", "cfg3-literal", "cfg4",
-    "p1-chain", "p2-chain-rcol", "p3-matrices", "p4-second-order", "p5-trwake",
+    "p1-chain", "p2-chain-rcol", "p3-matrices", "p4-second-order", "p5-trwake", "p6-rfcw",
 )
 
 
@@ -356,11 +356,30 @@ def _p5(n, n_turns=1):
                     notes="offset bunch, TRWAKE resonator + TRWAKE table + WAKE")
 
 
+def _p6(n, n_cavities=8, n_turns=1):
+    """RFCW-style composite ("RFCW, which is a combination of RFCA, WAKE, TRWAKE ..."):
+    an offset bunch through n_cavities x [drift x quad MATRIX of the cfg3 ring, RFKICK, WAKE, TRWAKE], the two wakes
+    with the same 512-bin AUTO_MINMAX binning."""
+    ring = _cfg3(n, n_matrices=max(8, n_cavities))
+    mats = [e for e in ring.elements if e["type"] == "MATRIX"][:n_cavities]
+    off = np.zeros(6); off[0] = 2e-4; off[2] = -1e-4
+    elems = [_matrix_elem(np.eye(6), off)]
+    for m in mats:
+        elems += [m,
+                  {"type": "RFKICK", "V": 2e6, "f": 1.3e9, "phi": 1.2},
+                  {"type": "WAKE", "nb": 512, "window": "AUTO_MINMAX", "wake": "RESONATOR", "f": 1.3e9, "Q": 5.0,
+                   "Rs": 1e3, "interp": True},
+                  {"type": "TRWAKE", "nb": 512, "window": "AUTO_MINMAX", "wake": "RESONATOR_T", "f": 2.4e9, "Q": 10.0,
+                   "Rs": 1e6, "interp": True}]
+    return Workload("p6-rfcw", 3, n or 100_000_000, 3e9, 1e-9, False, n_turns, "none", elems, "gauss6",
+                    notes=f"{n_cavities} cavities of MATRIX + RFKICK + WAKE + TRWAKE")
+
+
 def make_workload(name: str, n: Optional[int] = None, **kw) -> Workload:
     """name in WORKLOAD_NAMES; n overrides the particle count (reduced-size parity cases)."""
     table = {
         "cfg0": _cfg0, "cfg1": _cfg1, "cfg2": _cfg2, "cfg3": _cfg3, "cfg3-literal": _cfg3_literal,
-        "cfg4": _cfg4, "p1-chain": _p1, "p2-chain-rcol": _p2, "p3-matrices": _p3, "p4-second-order": _p4, "p5-trwake": _p5,
+        "cfg4": _cfg4, "p1-chain": _p1, "p2-chain-rcol": _p2, "p3-matrices": _p3, "p4-second-order": _p4, "p5-trwake": _p5, "p6-rfcw": _p6,
     }
     if name not in table:
         raise KeyError(f"unknown workload {name!r}; known: {WORKLOAD_NAMES}")

@@ -601,7 +601,43 @@ struct Tracker {
         b->rec_count = 0;
     }
 
+    // WAKE / HISTO / TRWAKE.  A WAKE directly followed by a TRWAKE with the same binning (the RFCW composite of
+    // "RFCW, which is a combination of RFCA, WAKE, TRWAKE ...") shares ONE window and ONE histogram
+    // pass (the dipole histogram also yields the counts: 24 B per particle instead of 8 + 24), and both kicks
+    // wait in the pending list for the next fused run, so a cavity costs one pass over the particles.
+    bool skip_next = false;
+
+    bool mergeable(long long k) const {
+        if (k + 1 >= (long long)bl->e.size()) return false;
+        const elg_element& w = bl->e[k];
+        const elg_element& t = bl->e[k + 1];
+        if (w.type != ELG_WAKE || t.type != ELG_TRWAKE) return false;
+        if (o && o->moments_every == ELG_MOM_ELEMENT) return false;
+        if (w.nb != t.nb || w.window != t.window) return false;
+        if (w.window == ELG_WIN_EXPLICIT && (w.dt != t.dt || w.t_lo_rel != t.t_lo_rel)) return false;
+        if (w.window == ELG_WIN_AUTO_TABLE && w.dt_table != t.dt_table) return false;
+        return true;
+    }
+
     void wake_or_histo(long long k, double s_here) {
+        const elg_element& e = bl->e[k];
+        const bool merged = mergeable(k);
+        prepare_hist(k, s_here, e.type == ELG_TRWAKE || merged);
+        if (!ok() || e.type == ELG_HISTO) return;
+        if (e.type == ELG_WAKE) {
+            wake_part(k);
+            if (merged) {                                             // the TRWAKE's window and counts are the same
+                if (b) stage_out_hist(e.nb);
+                else if (o) { o->window_written++; o->hist_written += e.nb; }
+                trwake_part(k + 1);
+                skip_next = true;
+            }
+        } else {
+            trwake_part(k);
+        }
+    }
+
+    void prepare_hist(long long k, double s_here, bool dipole) {
         const elg_element& e = bl->e[k];
         bool writes_s = false;
         for (const HostOp& op : pending) writes_s = writes_s || op.type == OP_DRIFT || op.type == OP_MATRIX || op.type == OP_MATRIX2;
@@ -617,13 +653,13 @@ struct Tracker {
             w.mode = e.window; w.nb = e.nb; w.t_lo_rel = e.t_lo_rel;
             w.dt_in = (e.window == ELG_WIN_AUTO_TABLE) ? e.dt_table : e.dt;
             w.t_design = s_here * b->inv_bc; w.inv_bc = b->inv_bc; w.counts = b->counts;
-            w.dacc = (e.type == ELG_TRWAKE) ? reinterpret_cast<long long*>(b->dacc) : nullptr;
+            w.dacc = dipole ? reinterpret_cast<long long*>(b->dacc) : nullptr;
             {
                 ProfScope ps(b, ELG_K_WINDOW);
                 window_kernel<<<(e.nb + 4 * kBlock - 1) / (4 * kBlock), kBlock, 0, b->stream>>>(w);
             }
             check(cudaGetLastError(), "window_kernel launch");
-            if (e.type == ELG_TRWAKE) {                               // counts + exact dipole sums (G33)
+            if (dipole) {                                             // counts + exact dipole sums (G33)
                 DipoleArgs d;
                 d.s = b->coord(b->cur_buf, 4); d.x = b->coord(b->cur_buf, 0); d.y = b->coord(b->cur_buf, 2);
                 d.st = b->st; d.cur = b->cur_slot; d.inv_bc = b->inv_bc; d.nb = e.nb; d.counts = b->counts; d.dacc = b->dacc;
@@ -640,59 +676,27 @@ struct Tracker {
             check(cudaGetLastError(), "hist_kernel launch");
             stage_out_hist(e.nb);
         } else if (o) { o->window_written++; o->hist_written += e.nb; }
-        if (e.type == ELG_HISTO) return;
-        count();                                                      // wake samples
-        count();                                                      // convolution
-        if (e.type == ELG_TRWAKE) {
-            count(); count();                                         // dipole sums -> doubles; second convolution
-            if (b) {
-                WakeArgs wa;
-                wa.st = b->st; wa.dt_fixed = 0.0; wa.kind = e.wake; wa.nb = e.nb;
-                const ResConst& r = bl->res[k];
-                wa.kloss = r.kloss; wa.alpha = r.alpha; wa.wbar = r.wbar; wa.ratio = r.ratio;
-                wa.table = b->table + bl->table_off[k]; wa.n_table = e.n_table; wa.dt_table = e.dt_table; wa.W = b->W;
-                {
-                    ProfScope ps(b, ELG_K_WAKE_SAMPLES);
-                    wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
-                }
-                check(cudaGetLastError(), "wake_samples_kernel launch");
-                {
-                    ProfScope ps(b, ELG_K_CONV);
-                    dipole_finalize_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(b->dacc, e.nb, b->D);
-                }
-                check(cudaGetLastError(), "dipole_finalize_kernel launch");
-                for (int plane = 0; plane < 2; plane++) {
-                    ConvArgs<double> cv;
-                    cv.counts = b->D + (size_t)plane * e.nb; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro;
-                    cv.V = b->Vt + (size_t)plane * e.nb;
-                    ProfScope ps(b, ELG_K_CONV);
-                    conv_kernel<double><<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
-                }
-                check(cudaGetLastError(), "conv_kernel launch");
-                if (o && o->V_out && o->V_written + 4LL * e.nb <= o->V_capacity) {
-                    check(cudaMemcpyAsync(o->V_out + o->V_written, b->D, (size_t)e.nb * 16, cudaMemcpyDeviceToHost, b->stream), "D D2H");
-                    check(cudaMemcpyAsync(o->V_out + o->V_written + 2LL * e.nb, b->Vt, (size_t)e.nb * 16, cudaMemcpyDeviceToHost, b->stream), "Vt D2H");
-                }
-            }
-            if (o) o->V_written += 4LL * e.nb;
-            HostOp op{};
-            op.type = OP_TKICK;
-            op.coef[0] = b ? b->inv_bc : 0.0; op.coef[1] = b ? b->inv_E : 0.0;
-            pending.push_back(op);
-            tk_nb = e.nb; tk_interp = e.interp;
-            return;
+    }
+
+    void launch_samples(long long k) {
+        const elg_element& e = bl->e[k];
+        WakeArgs wa;
+        wa.st = b->st; wa.dt_fixed = 0.0; wa.kind = e.wake; wa.nb = e.nb;
+        const ResConst& r = bl->res[k];
+        wa.kloss = r.kloss; wa.alpha = r.alpha; wa.wbar = r.wbar; wa.ratio = r.ratio;
+        wa.table = b->table + bl->table_off[k]; wa.n_table = e.n_table; wa.dt_table = e.dt_table; wa.W = b->W;
+        {
+            ProfScope ps(b, ELG_K_WAKE_SAMPLES);
+            wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
         }
+        check(cudaGetLastError(), "wake_samples_kernel launch");
+    }
+
+    void wake_part(long long k) {                                     // samples, convolution, queue the kick
+        const elg_element& e = bl->e[k];
+        count(); count();
         if (b) {
-            WakeArgs wa;
-            wa.st = b->st; wa.dt_fixed = 0.0; wa.kind = e.wake; wa.nb = e.nb;
-            const ResConst& r = bl->res[k];
-            wa.kloss = r.kloss; wa.alpha = r.alpha; wa.wbar = r.wbar; wa.ratio = r.ratio;
-            wa.table = b->table + bl->table_off[k]; wa.n_table = e.n_table; wa.dt_table = e.dt_table; wa.W = b->W;
-            {
-                ProfScope ps(b, ELG_K_WAKE_SAMPLES);
-                wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
-            }
-            check(cudaGetLastError(), "wake_samples_kernel launch");
+            launch_samples(k);
             ConvArgs<unsigned int> cv;
             cv.counts = b->counts; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro; cv.V = b->V;
             {
@@ -711,6 +715,37 @@ struct Tracker {
         kick_nb = e.nb; kick_interp = e.interp;
     }
 
+    void trwake_part(long long k) {                                   // samples, dipole sums -> doubles, two convolutions
+        const elg_element& e = bl->e[k];
+        count(); count(); count(); count();
+        if (b) {
+            launch_samples(k);
+            {
+                ProfScope ps(b, ELG_K_CONV);
+                dipole_finalize_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(b->dacc, e.nb, b->D);
+            }
+            check(cudaGetLastError(), "dipole_finalize_kernel launch");
+            for (int plane = 0; plane < 2; plane++) {
+                ConvArgs<double> cv;
+                cv.counts = b->D + (size_t)plane * e.nb; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro;
+                cv.V = b->Vt + (size_t)plane * e.nb;
+                ProfScope ps(b, ELG_K_CONV);
+                conv_kernel<double><<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
+            }
+            check(cudaGetLastError(), "conv_kernel launch");
+            if (o && o->V_out && o->V_written + 4LL * e.nb <= o->V_capacity) {
+                check(cudaMemcpyAsync(o->V_out + o->V_written, b->D, (size_t)e.nb * 16, cudaMemcpyDeviceToHost, b->stream), "D D2H");
+                check(cudaMemcpyAsync(o->V_out + o->V_written + 2LL * e.nb, b->Vt, (size_t)e.nb * 16, cudaMemcpyDeviceToHost, b->stream), "Vt D2H");
+            }
+        }
+        if (o) o->V_written += 4LL * e.nb;
+        HostOp op{};
+        op.type = OP_TKICK;
+        op.coef[0] = b ? b->inv_bc : 0.0; op.coef[1] = b ? b->inv_E : 0.0;
+        pending.push_back(op);
+        tk_nb = e.nb; tk_interp = e.interp;
+    }
+
     void stage_out_hist(int nb) {
         if (!o) return;
         if (o->window_out && o->window_written < o->window_capacity)
@@ -725,6 +760,7 @@ struct Tracker {
         const long long ne = (long long)bl->e.size();
         const int mom = o ? o->moments_every : ELG_MOM_NONE;
         for (long long k = 0; k < ne && ok(); k++) {
+            if (skip_next) { skip_next = false; continue; }           // TRWAKE merged into the preceding WAKE
             const elg_element& e = bl->e[k];
             const double s_here = std::fma((double)turn, bl->length, bl->s_design[k]);      // G8
             HostOp op{};

@@ -108,3 +108,20 @@ def test_no_cpu_fallback():
     addr = (C.addressof(buf) + 255) & ~255
     rc = elg.lib().elg_bunch_create(C.byref(h), 0, addr, addr, 1 << 30, None, 0, 1e9, 0.511e6, 1e-9, None)
     assert rc == elg.ECUDA
+
+
+def test_rfcw_composite_shares_one_histogram_pass():
+    """WAKE directly followed by TRWAKE with the same binning: one window, one (dipole) histogram, both kicks wait
+    for the next fused run: 10 launches per cavity (chain, window, histogram, samples, conv, samples, finalize,
+    2 conv ... ) instead of 14."""
+    from elg_inputs import make_workload
+    w = make_workload("p6-rfcw", n=16, n_cavities=3)
+    bl = elg.Beamline(w.elements)
+    # per cavity: 1 fused run + window + histogram + (samples + conv) + (samples + finalize + 2 conv); + the last kicks
+    assert bl.launches_per_turn("none") == 3 * (1 + 2 + 2 + 4) + 1
+    # different binning: no sharing
+    e2 = [dict(e) for e in w.elements]
+    for e in e2:
+        if e["type"] == "TRWAKE":
+            e["nb"] = 256
+    assert elg.Beamline(e2).launches_per_turn("none") == 3 * (1 + 2 + 2 + 1 + 2 + 4) + 1

@@ -464,6 +464,29 @@ def test_trwake_run_to_run_deterministic(elg):
         assert np.array_equal(a, b_)
 
 
+@pytest.mark.parametrize("n", [3, 70_001])
+def test_rfcw_composite(elg, elgo, n):
+    """RFKICK + WAKE + TRWAKE per cavity with shared binning (one histogram pass on the CUDA side, two on the
+    oracle's): identical windows, counts and dipole sums at the first cavity, V to 1e-10, coordinates to 1e-12."""
+    w = make_workload("p6-rfcw", n=n, n_cavities=4)
+    ob, oo, gb, go = both(elg, elgo, w)
+    nb = 512
+    assert go["hist"].size == oo["hist"].size == 8 * nb and go["window"].shape == oo["window"].shape == (8, 3)
+    assert np.array_equal(go["window"][:2], oo["window"][:2]) and np.array_equal(go["window"][0], go["window"][1])
+    assert np.array_equal(go["hist"][:2 * nb], oo["hist"][:2 * nb])
+    assert np.array_equal(go["hist"][:nb], go["hist"][nb:2 * nb])
+    Vo, Vg = oo["V"], go["V"]
+    assert Vg.size == Vo.size == 4 * 5 * nb
+    assert np.array_equal(Vg[nb:3 * nb], Vo[nb:3 * nb]), "dipole sums of the first cavity"
+    for c in range(4):
+        for lo, hi in ((0, nb), (3 * nb, 4 * nb), (4 * nb, 5 * nb)):
+            a = Vg[5 * nb * c + lo: 5 * nb * c + hi]; r = Vo[5 * nb * c + lo: 5 * nb * c + hi]
+            assert np.max(np.abs(a - r)) <= (1e-10 if c == 0 else 1e-9) * np.max(np.abs(r)) + 1e-300
+        assert int(go["hist"][2 * nb * c: 2 * nb * c + nb].sum()) == n
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid) and rel_err(gv, ov) <= 1e-12
+
+
 def test_track_in_two_calls_equals_one(elg, elgo):
     """Turn counter, RF reference and lost log carry across elg_track calls."""
     w = make_workload("cfg3", n=5000, n_matrices=10, n_turns=6)
