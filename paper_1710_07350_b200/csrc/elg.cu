@@ -6,6 +6,7 @@
 #include "elg_kernels.cuh"
 
 #include <atomic>
+#include <map>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -95,7 +96,7 @@ struct elg_bunch {
     long long rec_count = 0;                            // records in the device ring
     // launch geometry
     int sms = 0;
-    int grid_chain[3][2] = {{0, 0}, {0, 0}, {0, 0}};    // [variant][compact]; variants: <8 ops, P=2>, <8, P=4>, long run <80, P=6>
+    std::map<const void*, int> grids;                   // persistent grid size per chain kernel instantiation
     int force_p = 0;                                    // ELG_CHAIN_P = 2 | 4 overrides the planner's choice
     int grid_hist = 0, grid_mom = 0, grid_dipole = 0;
     int hist_aggregate = 0;
@@ -388,13 +389,6 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     b->sms = sms;
     int32_t rc = ELG_OK;
     if (rc == ELG_OK) rc = long_setup_once();
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, 2>, sms, 0, kBlock, &b->grid_chain[0][0]);
-    if (rc == ELG_OK) rc = grid_for(chain_kernel<kMaxOpsSmall, 4>, sms, 0, kBlock, &b->grid_chain[1][0]);
-    if (rc == ELG_OK) rc = grid_for(compact_kernel<kMaxOpsSmall>, sms, 0, kBlock, &b->grid_chain[0][1]);
-    if (b->grid_chain[0][1] > kCompactMaxGrid) b->grid_chain[0][1] = kCompactMaxGrid;   // kPoll status words per thread
-    b->grid_chain[1][1] = b->grid_chain[0][1];
-    if (rc == ELG_OK) rc = grid_for(chain_long_kernel<kMaxOpsLarge>, sms, chain_long_smem_bytes<kMaxOpsLarge>(), kBlock, &b->grid_chain[2][0]);
-    b->grid_chain[2][1] = b->grid_chain[2][0];
     if (rc == ELG_OK) rc = hist_setup_once();
     if (rc == ELG_OK) rc = grid_for(hist_kernel, sms, kHistSmemBins * 4, kBlock, &b->grid_hist);
     if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, kBlock, &b->grid_mom);
@@ -482,7 +476,20 @@ struct Tracker {
         if (e != cudaSuccess && rc == ELG_OK) rc = fail(ELG_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
     }
 
-    template <int MAXOPS, bool COMPACT, int P>
+    // blocks of a persistent grid = resident blocks per SM x SMs, looked up once per kernel
+    int cached_grid(const void* kernel, int smem) {
+        auto it = b->grids.find(kernel);
+        if (it != b->grids.end()) return it->second;
+        int occ = 0;
+        check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kBlock, smem), "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+        if (occ < 1 && rc == ELG_OK) rc = fail(ELG_ECUDA, "kernel does not fit on an SM");
+        long long g = (long long)occ * b->sms;
+        if (g > kMaxGrid) g = kMaxGrid / b->sms * b->sms;
+        b->grids[kernel] = (int)g;
+        return (int)g;
+    }
+
+    template <int MAXOPS, bool COMPACT, int P, bool EXT>
     void launch_chain(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm, unsigned rmask, unsigned wmask) {
         count();
         if (!b) return;
@@ -509,7 +516,13 @@ struct Tracker {
             a.type[k] = pending[k].type;
             std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
         }
-        const int grid = b->grid_chain[MAXOPS == kMaxOpsLarge ? 2 : (P == 4 ? 1 : 0)][COMPACT ? 1 : 0];
+        int grid = 0;
+        if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS>, chain_long_smem_bytes<MAXOPS>());
+        else if constexpr (COMPACT) {
+            grid = cached_grid((const void*)compact_kernel<MAXOPS, EXT>, 0);
+            if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
+        } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, EXT>, 0);
+        if (!ok()) return;
         if (want_mm) mm_grid = grid;
         {
             ProfScope ps(b, MAXOPS == kMaxOpsLarge ? ELG_K_CHAIN_LONG : (COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN));
@@ -518,11 +531,11 @@ struct Tracker {
             else if constexpr (COMPACT)
             {
                 void* kargs[] = {(void*)&a};                     // cooperative: every block resident (static tiles)
-                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS>, dim3(grid), dim3(kBlock), kargs, 0, b->stream),
+                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS, EXT>, dim3(grid), dim3(kBlock), kargs, 0, b->stream),
                       "compact_kernel cooperative launch");
             }
             else
-                chain_kernel<MAXOPS, P><<<grid, kBlock, 0, b->stream>>>(a);
+                chain_kernel<MAXOPS, P, EXT><<<grid, kBlock, 0, b->stream>>>(a);
         }
         check(cudaGetLastError(), "chain_kernel launch");
         if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
@@ -554,11 +567,13 @@ struct Tracker {
         bool p4 = n_mat >= kMatricesForP4;
         if (b && b->force_p == 2) p4 = false;
         if (b && b->force_p == 4) p4 = true;
-#define ELG_LAUNCH(M, C, PP) launch_chain<M, C, PP>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
-        if (large)   { ELG_LAUNCH(kMaxOpsLarge, false, kPL); }
-        else if (compact) { ELG_LAUNCH(kMaxOpsSmall, true, 2); }
-        else if (p4) { ELG_LAUNCH(kMaxOpsSmall, false, 4); }
-        else         { ELG_LAUNCH(kMaxOpsSmall, false, 2); }
+        bool ext = false;                                             // rarely used maps: the EXT instantiations
+        for (const HostOp& op : pending) ext = ext || op.type == OP_MATRIX2 || op.type == OP_TKICK;
+#define ELG_LAUNCH(M, C, PP, E) launch_chain<M, C, PP, E>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
+        if (large)   { ELG_LAUNCH(kMaxOpsLarge, false, kPL, true); }
+        else if (compact) { if (ext) ELG_LAUNCH(kMaxOpsSmall, true, 2, true); else ELG_LAUNCH(kMaxOpsSmall, true, 2, false); }
+        else if (p4) { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 4, true); else ELG_LAUNCH(kMaxOpsSmall, false, 4, false); }
+        else         { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 2, true); else ELG_LAUNCH(kMaxOpsSmall, false, 2, false); }
 #undef ELG_LAUNCH
         if (compact || (wmask & 0x10)) mm_valid = want_mm;
         else mm_valid = mm_valid || want_mm;

@@ -181,7 +181,7 @@ __device__ __forceinline__ void matrix2_terms(const double* __restrict__ tt, con
 }
 
 // DRIFT, RFKICK and the wake KICK, in place
-template <int P>
+template <int P, bool EXT = true>
 __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, const ChainCommon& cm, double (&v)[P][6]) {
     if (ty == OP_DRIFT) {                                        // PAPER.md:75-77, G2
         const double L = c[0];
@@ -227,7 +227,7 @@ __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, 
             }
             v[p][5] = fma(-Vt, inv_E, v[p][5]);
         }
-    } else if (ty == OP_TKICK) {                                 // G32: x' += Vx(t) / (beta0 p0c), y' likewise
+    } else if (EXT && ty == OP_TKICK) {                          // G32: x' += Vx(t) / (beta0 p0c), y' likewise
         const double inv_bc = c[0], inv_E = c[1];
         const double t_lo = cm.st->win[0], inv_dt = cm.st->win[2];
         const int nb = cm.t_nb;
@@ -259,21 +259,23 @@ __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, 
     }
 }
 
-template <int MAXOPS, int P>
+// EXT = false leaves out the rarely used maps (MATRIX2, TKICK): the HBM-bound short kernels stay at 62 registers
+// (4 blocks per SM); the planner picks the EXT = true instantiation when a run holds one of them.
+template <int MAXOPS, int P, bool EXT>
 __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
     for (int op = 0; op < a.c.n_ops; op++) {
         const double* c = a.coef[op];
         const int ty = a.type[op];
-        if (ty == OP_MATRIX || ty == OP_MATRIX2) {
+        if (ty == OP_MATRIX || (EXT && ty == OP_MATRIX2)) {
             double w[P][6];
             matrix_map<P>(c, v, w);
-            if (ty == OP_MATRIX2) { matrix2_terms<P>(c + 42, v, w); op += 3; }
+            if (EXT && ty == OP_MATRIX2) { matrix2_terms<P>(c + 42, v, w); op += 3; }
 #pragma unroll
             for (int p = 0; p < P; p++)
 #pragma unroll
                 for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
         } else {
-            other_map<P>(ty, c, a.c, v);
+            other_map<P, EXT>(ty, c, a.c, v);
         }
     }
 }
@@ -330,7 +332,7 @@ __device__ __forceinline__ unsigned long long pack_status(unsigned int epoch, un
 // sub-tile, warp accesses are 512 contiguous bytes).  Only the coordinates the run reads / writes are
 // loaded / stored (accessor masks).
 // ---------------------------------------------------------------------------------------------------
-template <int MAXOPS, int P>
+template <int MAXOPS, int P, bool EXT>
 __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
     constexpr int H = P / 2;                    // sub-tiles per tile
     constexpr int kSub = 2 * kBlock;            // particles per sub-tile
@@ -362,7 +364,7 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
             }
         }
 
-        apply_ops<MAXOPS, P>(a, v);
+        apply_ops<MAXOPS, P, EXT>(a, v);
 
 #pragma unroll
         for (int h = 0; h < H; h++) {
@@ -544,7 +546,7 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
 constexpr int kPoll = 3;                                // status words per thread and tile: grids up to 3 * 256 + 1 blocks
 constexpr int kCompactMaxGrid = kPoll * kBlock + 1;
 
-template <int MAXOPS>
+template <int MAXOPS, bool EXT>
 __global__ void __launch_bounds__(kBlock, ELG_COMPACT_BLOCKS) compact_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
     const ChainCommon& c = a.c;
     const long long n = c.st->n_alive[c.cur];
@@ -610,7 +612,7 @@ __global__ void __launch_bounds__(kBlock, ELG_COMPACT_BLOCKS) compact_kernel(con
             }
             if (tile + gridDim.x < n_tiles) prefetch(tile + gridDim.x);   // streams in during this iteration
 
-            apply_ops<MAXOPS, 2>(a, v);       // short run: coefficients straight from the parameter bank
+            apply_ops<MAXOPS, 2, EXT>(a, v);  // short run: coefficients straight from the parameter bank
 
 #pragma unroll
             for (int q = 0; q < 2; q++) surv[q] = ok[q] && survives(c.ap_type, c.ap_x, c.ap_y, v[q][0], v[q][2]);
