@@ -36,7 +36,8 @@ UNIT = "Mpasses/s"
 # algorithmic fp64 flops per particle per element (MATRIX = 36 FMA, the constant C
 # rides as the accumulator's start value; DRIFT = 5 FMA + sqrt; RFKICK = sub, mul, 2 FMA (+ sin, not counted);
 # wake KICK = bin index and interpolation: mul, sub, mul, sub, sub, sub, FMA, FMA)
-FLOPS = {"MATRIX": 72.0, "DRIFT": 11.0, "RFKICK": 6.0, "WAKE": 10.0, "MATRIX2": 72.0 + 21.0 + 2.0 * 126.0}
+FLOPS = {"MATRIX": 72.0, "DRIFT": 11.0, "RFKICK": 6.0, "WAKE": 10.0, "MATRIX2": 72.0 + 21.0 + 2.0 * 126.0,
+         "MATRIX3": 72.0 + 21.0 + 2.0 * 126.0 + 56.0 + 2.0 * 336.0}
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x DFMA/clk/SM x 2 flop x clocks.max.sm
 NOMINAL_HBM_GBS = 8000.0                              # BASELINE.json: "vs 8 TB/s roofline"
 

@@ -10,10 +10,12 @@ from .rng import uniform01, normal01, SEED_BASE
 from .configs import (
     ELECTRON_MC2_EV, C_LIGHT, Workload, make_workload, WORKLOAD_NAMES,
     drift_matrix, thin_quad_matrix, compose, pair_index, second_order_drift, thin_quad_sextupole,
+    triple_index, thin_quad_sext_octupole, third_order_drift,
 )
 
 __all__ = [
     "uniform01", "normal01", "SEED_BASE", "ELECTRON_MC2_EV", "C_LIGHT", "Workload",
     "make_workload", "WORKLOAD_NAMES", "drift_matrix", "thin_quad_matrix", "compose",
     "pair_index", "second_order_drift", "thin_quad_sextupole",
+    "triple_index", "thin_quad_sext_octupole", "third_order_drift",
 ]

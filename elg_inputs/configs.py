@@ -38,7 +38,7 @@ C_LIGHT = 299792458.0
 
 WORKLOAD_NAMES = (
     "cfg0", "cfg1", "cfg2", "cfg3", "cfg3-literal", "cfg4",
-    "p1-chain", "p2-chain-rcol", "p3-matrices", "p4-second-order", "p5-trwake", "p6-rfcw",
+    "p1-chain", "p2-chain-rcol", "p3-matrices", "p4-second-order", "p5-trwake", "p6-rfcw", "p7-third-order",
 )
 
 
@@ -85,6 +85,44 @@ def thin_quad_sextupole(k1L: float, k2L: float):
     T[1, pair_index(2, 2)] = +0.5 * k2L
     T[3, pair_index(0, 2)] = +k2L
     return R, C, T
+
+
+def triple_index(j: int, k: int, l: int) -> int:
+    """Position of the triple j <= k <= l in lexicographic order (G35)."""
+    j, k, l = sorted((j, k, l))
+    t = 0
+    for a in range(6):
+        for b in range(a, 6):
+            for c in range(b, 6):
+                if (a, b, c) == (j, k, l):
+                    return t
+                t += 1
+    raise ValueError((j, k, l))
+
+
+def thin_quad_sext_octupole(k1L: float, k2L: float, k3L: float):
+    """Thin multipole kick to third order: quadrupole + sextupole (see thin_quad_sextupole) + octupole
+    x' -= k3L/6 (x^3 - 3 x y^2);  y' -= k3L/6 (y^3 - 3 x^2 y)."""
+    R, C, T = thin_quad_sextupole(k1L, k2L)
+    U = np.zeros((6, 56))
+    U[1, triple_index(0, 0, 0)] = -k3L / 6.0
+    U[1, triple_index(0, 2, 2)] = +k3L / 2.0
+    U[3, triple_index(2, 2, 2)] = -k3L / 6.0
+    U[3, triple_index(0, 0, 2)] = +k3L / 2.0
+    return R, C, T, U
+
+
+def third_order_drift(L: float):
+    """Drift to third order: second_order_drift (the cubic terms of x, y and s vanish for a drift in these
+    coordinates: x = x + L x' exactly, s gains L/2 (x'^2 + y'^2) and nothing cubic)."""
+    R, C, T = second_order_drift(L)
+    return R, C, T, np.zeros((6, 56))
+
+
+def _matrix3_elem(R, C, T, U):
+    return {"type": "MATRIX3", "R": np.ascontiguousarray(R, dtype=np.float64),
+            "C": np.ascontiguousarray(C, dtype=np.float64), "T": np.ascontiguousarray(T, dtype=np.float64),
+            "U": np.ascontiguousarray(U, dtype=np.float64)}
 
 
 def _matrix2_elem(R, C, T):
@@ -319,6 +357,20 @@ def _p3(n, n_matrices=8):
                     c3.elements[:n_matrices], "gauss6", notes=f"{n_matrices} cfg3 matrices")
 
 
+def _p7(n, n_cells=40, n_turns=1):
+    """Third-order ring (track_particles M3): n_cells x [third-order drift 1 m, thin quadrupole +
+    sextupole + octupole], strengths as p4 plus k3L = +-500 m^-3."""
+    seed = SEED_BASE + 3
+    u = uniform01(seed, 301, n_cells) - 0.5
+    elems = []
+    for i in range(n_cells):
+        sg = 1.0 if i % 2 == 0 else -1.0
+        elems.append(_matrix3_elem(*third_order_drift(1.0)))
+        elems.append(_matrix3_elem(*thin_quad_sext_octupole(sg * 0.4 * (1.0 + 0.1 * u[i]), sg * 2.0, sg * 500.0)))
+    return Workload("p7-third-order", 3, n or 100_000_000, 3e9, 1e-9, True, n_turns, "none",
+                    elems, "gauss6", notes=f"{2 * n_cells} third-order maps per turn")
+
+
 def _p4(n, n_cells=100, n_turns=1):
     """Second-order ring (track_particles M2): n_cells x [second-order drift 1 m,
     thin quadrupole + sextupole], quadrupole strengths of the stabilised cfg3 ring, k2L = +-2 m^-2."""
@@ -379,7 +431,7 @@ def make_workload(name: str, n: Optional[int] = None, **kw) -> Workload:
     """name in WORKLOAD_NAMES; n overrides the particle count (reduced-size parity cases)."""
     table = {
         "cfg0": _cfg0, "cfg1": _cfg1, "cfg2": _cfg2, "cfg3": _cfg3, "cfg3-literal": _cfg3_literal,
-        "cfg4": _cfg4, "p1-chain": _p1, "p2-chain-rcol": _p2, "p3-matrices": _p3, "p4-second-order": _p4, "p5-trwake": _p5, "p6-rfcw": _p6,
+        "cfg4": _cfg4, "p1-chain": _p1, "p2-chain-rcol": _p2, "p3-matrices": _p3, "p4-second-order": _p4, "p5-trwake": _p5, "p6-rfcw": _p6, "p7-third-order": _p7,
     }
     if name not in table:
         raise KeyError(f"unknown workload {name!r}; known: {WORKLOAD_NAMES}")

@@ -39,7 +39,7 @@ enum { ELG_OK = 0, ELG_EINVAL = -1, ELG_ENOMEM = -2, ELG_ECUDA = -3, ELG_ESTATE 
 
 /* element types (glossary PAPER.md:175; Table I rows PAPER.md:143-165) */
 enum { ELG_DRIFT = 1, ELG_MATRIX = 2, ELG_RFKICK = 3, ELG_RCOL = 4, ELG_ECOL = 5, ELG_WAKE = 6, ELG_HISTO = 7,
-       ELG_MATRIX2 = 8, ELG_TRWAKE = 9 };
+       ELG_MATRIX2 = 8, ELG_TRWAKE = 9, ELG_MATRIX3 = 10 };
 /* histogram window modes (G10) */
 enum { ELG_WIN_EXPLICIT = 0, ELG_WIN_AUTO_MINMAX = 1, ELG_WIN_AUTO_TABLE = 2 };
 /* wake kinds (G12) */
@@ -56,6 +56,10 @@ enum { ELG_MOM_NONE = 0, ELG_MOM_TURN = 1, ELG_MOM_ELEMENT = 2 };
  *                                   v_i <- C_i + sum_j R_ij v_j + sum_{j<=k} T_ijk v_j v_k; row i accumulated from
  *                                   C_i with FMAs, R terms first (j ascending), then T terms (q ascending) on the
  *                                   rounded products v_j v_k
+ *   MATRIX3 (track_particles M3; G35): MATRIX2 plus U (336 doubles, U[56 i + t], t numbering the
+ *                                   triples (j,k,l), j <= k <= l, lexicographically): + sum U_ijkl v_j v_k v_l, the
+ *                                   terms after the T terms, t ascending, on the products (v_j v_k) v_l.  Always runs
+ *                                   in the long-run kernel (12 parameter slots)
  *   RFKICK (G8): V [V], f [Hz], phi [rad].
  *                                   delta += V/(beta0 p0c) sin(phi + 2 pi f (s - s_ref)/(beta0 c)),
  *                                   s_ref = design path length in front of the element on this turn
@@ -88,6 +92,7 @@ typedef struct {
     const double* table;
     int64_t n_table;
     const double* T;
+    const double* U;
 } elg_element;
 
 typedef struct elg_bunch elg_bunch;
@@ -136,7 +141,7 @@ int64_t elg_soa_bytes(int64_t n0);
 /* Validates and copies n_elems elements (L finite, apertures > 0, nb >= 2, Q > 1/2, ...).  On a bad
  * element returns ELG_EINVAL and elg_last_error() names its index.  ring = 1: the line closes on itself,
  * RF phase references and EXPLICIT windows advance by the line length every turn (G8).  The design path
- * length is the sequential fp64 sum of L (DRIFT) and C[4] (MATRIX, MATRIX2) of the preceding elements. */
+ * length is the sequential fp64 sum of L (DRIFT) and C[4] (MATRIX, MATRIX2, MATRIX3) of the preceding elements. */
 int32_t elg_beamline_load(elg_beamline** out, const elg_element* h_elems, int64_t n_elems, int32_t ring);
 void    elg_beamline_destroy(elg_beamline*);
 int64_t elg_beamline_n_elements(const elg_beamline*);

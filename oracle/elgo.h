@@ -10,6 +10,8 @@
  * Parity status of each function (what pins it, see tests/test_oracle_pins.py):
  *   elgo_drift        pinned  - Listing 1 exact cases, literal re-evaluation
  *   elgo_matrix       pinned  - closed forms, identity, inverse, symplectic invariants
+ *   elgo_matrix3      pinned  - U = 0 equals elgo_matrix2 bitwise, one-entry index pins, thin octupole closed form,
+ *                               third-order path length of a drift
  *   elgo_matrix2      pinned  - T = 0 equals elgo_matrix bitwise, one-entry index pins, thin sextupole and
  *                               second-order drift closed forms (exact drift to O(x'^4))
  *   elgo_rfkick       pinned  - crest/zero-crossing/periodicity/slope closed forms
@@ -40,7 +42,7 @@ enum { ELGO_OK = 0, ELGO_EINVAL = -1, ELGO_ENOMEM = -2, ELGO_ESTATE = -4, ELGO_E
 
 /* element types (names: PAPER.md:175 glossary; north_star) */
 enum { ELGO_DRIFT = 1, ELGO_MATRIX = 2, ELGO_RFKICK = 3, ELGO_RCOL = 4, ELGO_ECOL = 5,
-       ELGO_WAKE = 6, ELGO_HISTO = 7, ELGO_MATRIX2 = 8, ELGO_TRWAKE = 9 };
+       ELGO_WAKE = 6, ELGO_HISTO = 7, ELGO_MATRIX2 = 8, ELGO_TRWAKE = 9, ELGO_MATRIX3 = 10 };
 /* histogram window modes (G10) */
 enum { ELGO_WIN_EXPLICIT = 0, ELGO_WIN_AUTO_MINMAX = 1, ELGO_WIN_AUTO_TABLE = 2 };
 /* wake kinds (G12) */
@@ -53,6 +55,8 @@ enum { ELGO_MOM_NONE = 0, ELGO_MOM_TURN = 1, ELGO_MOM_ELEMENT = 2 };
  *   MATRIX: R (36, row-major R[6*r+c]), C (6, may be NULL = 0)
  *   MATRIX2: R, C as MATRIX, T (126 = 6 x 21, T[21*i + q], q numbers the pairs (j,k), j <= k, in the order
  *           (0,0) (0,1) .. (0,5) (1,1) .. (5,5)): second-order transport map (G31)
+ *   MATRIX3: MATRIX2 plus U (336 = 6 x 56, U[56*i + t], t numbers the triples (j,k,l), j <= k <= l, in
+ *           lexicographic order): third-order transport map (G35)
  *   RFKICK: V [V], f [Hz], phi [rad]
  *   RCOL  : ax, ay [m]      ECOL: ax=a, ay=b [m]
  *   WAKE  : nb, window, (t_lo_rel, dt if EXPLICIT), wake kind, (f, Q, Rs) or (table, n_table, dt_table), interp
@@ -76,6 +80,7 @@ typedef struct {
     const double* table;
     int64_t n_table;
     const double* T;
+    const double* U;
 } elgo_element;
 
 typedef struct elgo_bunch elgo_bunch;
@@ -86,6 +91,9 @@ void   elgo_drift(double* x, const double* xp, double* y, const double* yp, doub
 void   elgo_matrix(double* const v[6], int64_t n, const double* R36, const double* C6);
 /* second-order map: v_i <- C_i + sum_j R_ij v_j + sum_{j<=k} T_ijk v_j v_k (G31) */
 void   elgo_matrix2(double* const v[6], int64_t n, const double* R36, const double* C6, const double* T126);
+/* third-order map (G35): ... + sum_{j<=k<=l} U_ijkl v_j v_k v_l */
+void   elgo_matrix3(double* const v[6], int64_t n, const double* R36, const double* C6, const double* T126,
+                    const double* U336);
 void   elgo_rfkick(const double* s, double* delta, int64_t n, double A, double omega, double phi0,
                    double s_ref, double inv_bc);
 /* survive[i] = 1/0.  kind = ELGO_RCOL or ELGO_ECOL. */

@@ -25,7 +25,7 @@ _HDR = os.path.join(_HERE, "elgo.h")
 _LIB = os.path.join(_HERE, "libelgo.so")
 
 OK, EINVAL, ENOMEM, ESTATE, ECAPACITY = 0, -1, -2, -4, -5
-DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2, TRWAKE = 1, 2, 3, 4, 5, 6, 7, 8, 9
+DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2, TRWAKE, MATRIX3 = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 WIN = {"EXPLICIT": 0, "AUTO_MINMAX": 1, "AUTO_TABLE": 2}
 WAKEKIND = {"RESONATOR": 0, "TABLE": 1, "RESONATOR_T": 2}
 MOM = {"none": 0, "turn": 1, "element": 2}
@@ -45,7 +45,7 @@ class Element(C.Structure):
         ("L", C.c_double), ("V", C.c_double), ("f", C.c_double), ("phi", C.c_double),
         ("ax", C.c_double), ("ay", C.c_double), ("Q", C.c_double), ("Rs", C.c_double),
         ("t_lo_rel", C.c_double), ("dt", C.c_double), ("dt_table", C.c_double),
-        ("R", _dp), ("C", _dp), ("table", _dp), ("n_table", C.c_int64), ("T", _dp),
+        ("R", _dp), ("C", _dp), ("table", _dp), ("n_table", C.c_int64), ("T", _dp), ("U", _dp),
     ]
 
 
@@ -84,6 +84,8 @@ def lib():
         L.elgo_matrix.restype = None
         L.elgo_matrix2.argtypes = [v6, C.c_int64, _dp, _dp, _dp]
         L.elgo_matrix2.restype = None
+        L.elgo_matrix3.argtypes = [v6, C.c_int64, _dp, _dp, _dp, _dp]
+        L.elgo_matrix3.restype = None
         L.elgo_rfkick.argtypes = [_dp, _dp, C.c_int64] + [C.c_double] * 5
         L.elgo_rfkick.restype = None
         L.elgo_aperture_flags.argtypes = [_dp, _dp, C.c_int64, C.c_int32, C.c_double, C.c_double, _u8p]
@@ -178,6 +180,12 @@ def matrix2(v: np.ndarray, R, T, Cvec=None) -> None:
     T = _f64(T).reshape(126)
     Cv = None if Cvec is None else _f64(Cvec)
     lib().elgo_matrix2(_v6(v), v.shape[1], _p(R), _p(Cv), _p(T))
+
+
+def matrix3(v: np.ndarray, R, T, U, Cvec=None) -> None:
+    R = _f64(R).reshape(36); T = _f64(T).reshape(126); U = _f64(U).reshape(336)
+    Cv = None if Cvec is None else _f64(Cvec)
+    lib().elgo_matrix3(_v6(v), v.shape[1], _p(R), _p(Cv), _p(T), _p(U))
 
 
 def rfkick(v: np.ndarray, A: float, omega: float, phi0: float, s_ref: float, inv_bc: float) -> None:
@@ -298,9 +306,11 @@ def _elements_to_c(elements):
             e.type, e.R = MATRIX, _p(R)
             if d.get("C") is not None:
                 Cv = _f64(d["C"]).reshape(6); keep.append(Cv); e.C = _p(Cv)
-        elif t == "MATRIX2":
+        elif t in ("MATRIX2", "MATRIX3"):
             R = _f64(d["R"]).reshape(36); T = _f64(d["T"]).reshape(126); keep += [R, T]
-            e.type, e.R, e.T = MATRIX2, _p(R), _p(T)
+            e.type, e.R, e.T = (MATRIX2 if t == "MATRIX2" else MATRIX3), _p(R), _p(T)
+            if t == "MATRIX3":
+                U = _f64(d["U"]).reshape(336); keep.append(U); e.U = _p(U)
             if d.get("C") is not None:
                 Cv = _f64(d["C"]).reshape(6); keep.append(Cv); e.C = _p(Cv)
         elif t == "RFKICK":

@@ -52,7 +52,7 @@ struct ResConst { double kloss, alpha, wbar, ratio; };
 
 struct elg_beamline {
     std::vector<elg_element> e;
-    std::vector<std::vector<double>> R, C, table, T;
+    std::vector<std::vector<double>> R, C, table, T, U;
     std::vector<ResConst> res;
     std::vector<double> s_design;
     double length = 0.0;
@@ -241,7 +241,7 @@ extern "C" int32_t elg_beamline_load(elg_beamline** out, const elg_element* elem
     if (!bl) return fail(ELG_ENOMEM, "elg_beamline_load: out of host memory");
     bl->ring = ring;
     bl->e.assign(elems, elems + n_elems);
-    bl->R.resize(n_elems); bl->C.resize(n_elems); bl->table.resize(n_elems); bl->T.resize(n_elems);
+    bl->R.resize(n_elems); bl->C.resize(n_elems); bl->table.resize(n_elems); bl->T.resize(n_elems); bl->U.resize(n_elems);
     bl->res.resize(n_elems); bl->table_off.assign(n_elems, 0);
     bl->s_design.resize(n_elems + 1);
     bl->serial = ++g_bl_serial;
@@ -254,12 +254,14 @@ extern "C" int32_t elg_beamline_load(elg_beamline** out, const elg_element* elem
             case ELG_DRIFT:
                 if (!std::isfinite(e.L)) why = "DRIFT: L not finite"; else s = s + e.L;
                 break;
-            case ELG_MATRIX: case ELG_MATRIX2:
+            case ELG_MATRIX: case ELG_MATRIX2: case ELG_MATRIX3:
                 if (!e.R) { why = "MATRIX: R is NULL"; break; }
-                if (e.type == ELG_MATRIX2 && !e.T) { why = "MATRIX2: T is NULL"; break; }
+                if (e.type != ELG_MATRIX && !e.T) { why = "MATRIX2/3: T is NULL"; break; }
+                if (e.type == ELG_MATRIX3 && !e.U) { why = "MATRIX3: U is NULL"; break; }
                 bl->R[k].assign(e.R, e.R + 36); e.R = bl->R[k].data();
                 if (e.C) { bl->C[k].assign(e.C, e.C + 6); e.C = bl->C[k].data(); s = s + e.C[4]; }
-                if (e.type == ELG_MATRIX2) { bl->T[k].assign(e.T, e.T + 126); e.T = bl->T[k].data(); }
+                if (e.type != ELG_MATRIX) { bl->T[k].assign(e.T, e.T + 126); e.T = bl->T[k].data(); }
+                if (e.type == ELG_MATRIX3) { bl->U[k].assign(e.U, e.U + 336); e.U = bl->U[k].data(); }
                 break;
             case ELG_RFKICK:
                 if (!std::isfinite(e.V) || !std::isfinite(e.f) || !std::isfinite(e.phi)) why = "RFKICK: V, f, phi must be finite";
@@ -552,7 +554,7 @@ struct Tracker {
         for (const HostOp& op : pending) {
             switch (op.type) {
                 case OP_DRIFT: rmask |= 0x1F; wmask |= 0x15; break;           // reads x x' y y' s, writes x y s
-                case OP_MATRIX: case OP_MATRIX2: rmask |= 0x3F; wmask |= 0x3F; break;
+                case OP_MATRIX: case OP_MATRIX2: case OP_MATRIX3: rmask |= 0x3F; wmask |= 0x3F; break;
                 case OP_RFKICK: case OP_KICK: rmask |= 0x30; wmask |= 0x20; break;   // reads s delta, writes delta
                 case OP_TKICK: rmask |= 0x1A; wmask |= 0x0A; break;                  // reads x' y' s, writes x' y'
             }
@@ -563,12 +565,12 @@ struct Tracker {
         // particles per thread: 2 while the run is HBM-bound; 4 once it holds enough MATRIX maps for the
         // coefficient fetches (one per 2 particles) to matter
         int n_mat = 0;
-        for (const HostOp& op : pending) n_mat += (op.type == OP_MATRIX) + 4 * (op.type == OP_MATRIX2);
+        for (const HostOp& op : pending) n_mat += (op.type == OP_MATRIX) + 4 * (op.type == OP_MATRIX2) + 12 * (op.type == OP_MATRIX3);
         bool p4 = n_mat >= kMatricesForP4;
         if (b && b->force_p == 2) p4 = false;
         if (b && b->force_p == 4) p4 = true;
         bool ext = false;                                             // rarely used maps: the EXT instantiations
-        for (const HostOp& op : pending) ext = ext || op.type == OP_MATRIX2 || op.type == OP_TKICK;
+        for (const HostOp& op : pending) ext = ext || op.type == OP_MATRIX2 || op.type == OP_MATRIX3 || op.type == OP_TKICK;
 #define ELG_LAUNCH(M, C, PP, E) launch_chain<M, C, PP, E>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
         if (large)   { ELG_LAUNCH(kMaxOpsLarge, false, kPL, true); }
         else if (compact) { if (ext) ELG_LAUNCH(kMaxOpsSmall, true, 2, true); else ELG_LAUNCH(kMaxOpsSmall, true, 2, false); }
@@ -655,7 +657,7 @@ struct Tracker {
     void prepare_hist(long long k, double s_here, bool dipole) {
         const elg_element& e = bl->e[k];
         bool writes_s = false;
-        for (const HostOp& op : pending) writes_s = writes_s || op.type == OP_DRIFT || op.type == OP_MATRIX || op.type == OP_MATRIX2;
+        for (const HostOp& op : pending) writes_s = writes_s || op.type == OP_DRIFT || op.type == OP_MATRIX || op.type == OP_MATRIX2 || op.type == OP_MATRIX3;
         const bool need_mm = !mm_valid || writes_s;
         if (!pending.empty() || need_mm) flush(AP_NONE, 0, 0, 0, need_mm);
         if (!ok()) return;
@@ -787,17 +789,27 @@ struct Tracker {
                     if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
                     push(op);
                     break;
-                case ELG_MATRIX2: {                                          // 4 slots: R, C | Tt[21][6] in three
-                    op.type = OP_MATRIX2;
+                case ELG_MATRIX2: case ELG_MATRIX3: {                        // 4 slots: R, C | Tt[21][6]; MATRIX3: + 8 slots Ut[56][6]
+                    const bool third = e.type == ELG_MATRIX3;
+                    op.type = third ? OP_MATRIX3 : OP_MATRIX2;
                     std::memcpy(op.coef, e.R, 36 * sizeof(double));
                     if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
-                    push(op, 4);
+                    push(op, third ? 12 : 4);
                     for (int part = 0; part < 3; part++) {
                         HostOp t{};
                         t.type = OP_CONT;
                         for (int j = 0; j < 42; j++) {                       // layout only: pair-major transpose of T
                             const int q = (42 * part + j) / 6, r = (42 * part + j) % 6;
                             t.coef[j] = e.T[21 * r + q];
+                        }
+                        pending.push_back(t);
+                    }
+                    for (int part = 0; third && part < 8; part++) {
+                        HostOp t{};
+                        t.type = OP_CONT;
+                        for (int j = 0; j < 42; j++) {                       // layout only: triple-major transpose of U
+                            const int q = (42 * part + j) / 6, r = (42 * part + j) % 6;
+                            t.coef[j] = e.U[56 * r + q];
                         }
                         pending.push_back(t);
                     }

@@ -29,7 +29,8 @@ constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
 enum : uint8_t { OP_DRIFT = 1, OP_MATRIX = 2, OP_RFKICK = 3, OP_KICK = 4,
                  OP_MATRIX2 = 5,      // second-order map: this slot holds R, C; the next three hold T (OP_CONT)
                  OP_CONT = 6,
-                 OP_TKICK = 7 };      // transverse wake kick of the preceding TRWAKE (G32)
+                 OP_TKICK = 7,        // transverse wake kick of the preceding TRWAKE (G32)
+                 OP_MATRIX3 = 8 };    // third-order map: R, C | 3 slots Tt[21][6] | 8 slots Ut[56][6] (12 slots, G35)
 enum { AP_NONE = 0, AP_RCOL = 1, AP_ECOL = 2 };
 
 // Device-resident tracking state (first bytes of the workspace).  Nothing here is read by the host
@@ -180,6 +181,35 @@ __device__ __forceinline__ void matrix2_terms(const double* __restrict__ tt, con
     }
 }
 
+// third-order terms of MATRIX3 (G35): w[p][r] += sum over the triples t = (j,k,l), j <= k <= l, lexicographic, of
+// U[r][t] ((v_j v_k) v_l), continuing row r's FMA chain after the second-order terms.  ut = Ut[56][6].
+template <int P>
+__device__ __forceinline__ void matrix3_terms(const double* __restrict__ ut, const double (&v)[P][6], double (&w)[P][6]) {
+    const double2* u2 = reinterpret_cast<const double2*>(ut);
+    int t = 0;
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+#pragma unroll
+        for (int k = j; k < 6; k++) {
+            double pjk[P];
+#pragma unroll
+            for (int p = 0; p < P; p++) pjk[p] = v[p][j] * v[p][k];
+#pragma unroll
+            for (int l = k; l < 6; l++) {
+                const double2 u01 = u2[3 * t], u23 = u2[3 * t + 1], u45 = u2[3 * t + 2];
+                const double u[6] = {u01.x, u01.y, u23.x, u23.y, u45.x, u45.y};
+#pragma unroll
+                for (int p = 0; p < P; p++) {
+                    const double pr = pjk[p] * v[p][l];
+#pragma unroll
+                    for (int r = 0; r < 6; r++) w[p][r] = fma(u[r], pr, w[p][r]);
+                }
+                t++;
+            }
+        }
+    }
+}
+
 // DRIFT, RFKICK and the wake KICK, in place
 template <int P, bool EXT = true>
 __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, const ChainCommon& cm, double (&v)[P][6]) {
@@ -293,15 +323,16 @@ __device__ __forceinline__ void apply_ops_smem(const ChainArgs<MAXOPS>& a, const
             matrix_map_s128<P>(s_coef + 42 * op, v, w);
             matrix_map_s128<P>(s_coef + 42 * (op + 1), w, v);
             op += 2;
-        } else if (ty == OP_MATRIX || ty == OP_MATRIX2) {
+        } else if (ty == OP_MATRIX || ty == OP_MATRIX2 || ty == OP_MATRIX3) {
             double w[P][6];
             matrix_map_s128<P>(s_coef + 42 * op, v, w);
-            if (ty == OP_MATRIX2) matrix2_terms<P>(s_coef + 42 * (op + 1), v, w);
+            if (ty != OP_MATRIX) matrix2_terms<P>(s_coef + 42 * (op + 1), v, w);
+            if (ty == OP_MATRIX3) matrix3_terms<P>(s_coef + 42 * (op + 4), v, w);
 #pragma unroll
             for (int p = 0; p < P; p++)
 #pragma unroll
                 for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
-            op += (ty == OP_MATRIX2) ? 4 : 1;
+            op += (ty == OP_MATRIX3) ? 12 : ((ty == OP_MATRIX2) ? 4 : 1);
         } else {
             other_map<P>(ty, s_coef + 42 * op, c, v);
             op++;

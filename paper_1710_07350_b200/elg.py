@@ -15,7 +15,7 @@ import numpy as np
 from .build import LIB, build
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ECAPACITY = 0, -1, -2, -3, -4, -5
-DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2, TRWAKE = 1, 2, 3, 4, 5, 6, 7, 8, 9
+DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2, TRWAKE, MATRIX3 = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 WIN = {"EXPLICIT": 0, "AUTO_MINMAX": 1, "AUTO_TABLE": 2}
 WAKEKIND = {"RESONATOR": 0, "TABLE": 1, "RESONATOR_T": 2}
 MOM = {"none": 0, "turn": 1, "element": 2}
@@ -51,7 +51,7 @@ class Element(C.Structure):
         ("L", C.c_double), ("V", C.c_double), ("f", C.c_double), ("phi", C.c_double),
         ("ax", C.c_double), ("ay", C.c_double), ("Q", C.c_double), ("Rs", C.c_double),
         ("t_lo_rel", C.c_double), ("dt", C.c_double), ("dt_table", C.c_double),
-        ("R", _dp), ("C", _dp), ("table", _dp), ("n_table", C.c_int64), ("T", _dp),
+        ("R", _dp), ("C", _dp), ("table", _dp), ("n_table", C.c_int64), ("T", _dp), ("U", _dp),
     ]
 
 
@@ -167,9 +167,11 @@ def _elements_to_c(elements):
             e.type, e.R = MATRIX, _p(R)
             if d.get("C") is not None:
                 Cv = _f64(d["C"]).reshape(6); keep.append(Cv); e.C = _p(Cv)
-        elif t == "MATRIX2":
+        elif t in ("MATRIX2", "MATRIX3"):
             R = _f64(d["R"]).reshape(36); T = _f64(d["T"]).reshape(126); keep += [R, T]
-            e.type, e.R, e.T = MATRIX2, _p(R), _p(T)
+            e.type, e.R, e.T = (MATRIX2 if t == "MATRIX2" else MATRIX3), _p(R), _p(T)
+            if t == "MATRIX3":
+                U = _f64(d["U"]).reshape(336); keep.append(U); e.U = _p(U)
             if d.get("C") is not None:
                 Cv = _f64(d["C"]).reshape(6); keep.append(Cv); e.C = _p(Cv)
         elif t == "RFKICK":

@@ -27,10 +27,10 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_element_struct_matches_header_layout():
-    # 6 int32 + 11 doubles + 3 pointers + int64 + 1 pointer = 24 + 88 + 24 + 8 + 8
-    assert C.sizeof(elg.Element) == 152
+    # 6 int32 + 11 doubles + 3 pointers + int64 + 2 pointers = 24 + 88 + 24 + 8 + 16
+    assert C.sizeof(elg.Element) == 160
     assert elg.Element.L.offset == 24 and elg.Element.R.offset == 112 and elg.Element.n_table.offset == 136
-    assert elg.Element.T.offset == 144
+    assert elg.Element.T.offset == 144 and elg.Element.U.offset == 152
     assert C.sizeof(elg.TrackOpts) == 8 + 3 * 8 + 3 * 8 * 3
 
 

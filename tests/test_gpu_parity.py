@@ -166,6 +166,28 @@ def test_second_order_maps_bitexact(elg, elgo, n, n_cells):
     assert np.array_equal(gv, ov)
 
 
+@pytest.mark.parametrize("n,n_cells", [(1, 1), (1537, 1), (50_001, 7)])
+def test_third_order_maps_bitexact(elg, elgo, n, n_cells):
+    """MATRIX3 (third-order transport map, G35; 12 parameter slots, long-run kernel): bit-identical, two turns."""
+    w = make_workload("p7-third-order", n=n, n_cells=n_cells, n_turns=2)
+    ob, oo, gb, go = both(elg, elgo, w, stage=False)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid) and np.array_equal(gv, ov)
+
+
+def test_third_order_then_aperture(elg, elgo):
+    from elg_inputs import thin_quad_sext_octupole, third_order_drift
+    m3 = lambda t: {"type": "MATRIX3", "R": t[0], "C": t[1], "T": t[2], "U": t[3]}
+    elems = [m3(third_order_drift(0.8)), m3(thin_quad_sext_octupole(0.3, 20.0, 4000.0)), {"type": "DRIFT", "L": 0.4},
+             {"type": "RCOL", "ax": 250e-6, "ay": 260e-6}, m3(third_order_drift(0.2))]
+    v0 = make_workload("cfg0", n=30_001).particles()
+    ob = elgo.Bunch(v0, 1e9, 1e-9); ob.track(elgo.Beamline(elems), 1)
+    gbl = elg.Beamline(elems); gb = elg.Bunch(v0, 1e9, 1e-9, beamline=gbl); gb.track(gbl, 1)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert 0 < gid.size < 30_001 and np.array_equal(gid, oid) and np.array_equal(gv, ov)
+    check_lost(ob, gb)
+
+
 def test_second_order_mixed_with_other_maps(elg, elgo):
     """MATRIX2 between MATRIX, DRIFT and RFKICK, then a collimator: slot accounting of the planner."""
     from elg_inputs import second_order_drift, thin_quad_sextupole

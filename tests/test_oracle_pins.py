@@ -729,3 +729,52 @@ def test_trwake_track_is_the_composition_of_stages(elgo):
     assert np.array_equal(oo["hist"][:nb], c)
     assert np.array_equal(oo["V"][:4 * nb], np.concatenate([Dx, Dy, Vx, Vy]))
     assert np.max(np.abs(Vx)) > 0 and abs(Dx.sum() / w.n0 - 2e-4) < 1e-5          # the bunch is offset by 200 um
+
+
+# ------------------------------------------------------------------------------------ MATRIX3 (G35)
+def test_matrix3_reduces_to_matrix2_and_index_convention(elgo):
+    from elg_inputs import triple_index
+    rng = np.random.default_rng(21)
+    v0 = rng.normal(size=(6, 40)) * np.array([1e-3, 1e-4, 1e-3, 1e-4, 1e-2, 1e-3])[:, None]
+    R = np.eye(6) + 0.1 * rng.normal(size=(6, 6)); Cv = rng.normal(size=6) * 1e-3; T = rng.normal(size=(6, 21))
+    a = v0.copy(); b = v0.copy()
+    elgo.matrix2(a, R, T, Cv); elgo.matrix3(b, R, T, np.zeros((6, 56)), Cv)
+    assert np.array_equal(a, b)
+    seen = set()
+    for i in (0, 3, 5):
+        for j in range(6):
+            for k in range(j, 6):
+                for l in range(k, 6):
+                    t = triple_index(j, k, l); seen.add(t)
+                    U = np.zeros((6, 56)); U[i, t] = 2.0
+                    b = v0.copy(); elgo.matrix3(b, np.eye(6), np.zeros((6, 21)), U)
+                    exp = v0.copy(); exp[i] = exp[i] + 2.0 * ((v0[j] * v0[k]) * v0[l])
+                    assert np.allclose(b, exp, rtol=0, atol=1e-20), (i, j, k, l)
+    assert seen == set(range(56)) and triple_index(5, 5, 5) == 55 and triple_index(2, 0, 1) == triple_index(0, 1, 2)
+
+
+def test_matrix3_octupole_closed_form(elgo):
+    """Thin quadrupole + sextupole + octupole kick against the multipole expansion Re/Im (x + i y)^n."""
+    from elg_inputs import thin_quad_sext_octupole
+    rng = np.random.default_rng(22)
+    v0 = rng.normal(size=(6, 300)) * 2e-3
+    k1, k2, k3 = 0.4, -30.0, 900.0
+    R, Cv, T, U = thin_quad_sext_octupole(k1, k2, k3)
+    a = v0.copy(); elgo.matrix3(a, R, T, U, Cv)
+    z = v0[0] + 1j * v0[2]
+    kick = k1 * z + k2 / 2 * z ** 2 + k3 / 6 * z ** 3            # sum_n knL/n! (x + i y)^n
+    assert np.array_equal(a[[0, 2, 4, 5]], v0[[0, 2, 4, 5]])
+    assert np.allclose(a[1], v0[1] - kick.real, rtol=1e-14, atol=1e-17)      # a few ulp of the 1e-3 slopes
+    assert np.allclose(a[3], v0[3] + kick.imag, rtol=1e-14, atol=1e-17)
+    assert np.max(np.abs(kick.real)) > 1e-4 and np.max(np.abs((k3 / 6 * z ** 3).real)) > 1e-7
+
+
+def test_matrix3_in_track(elgo):
+    w = make_workload("p7-third-order", n=200, n_cells=2)
+    v0 = w.particles()
+    ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C); ob.track(elgo.Beamline(w.elements, ring=True), 2)
+    ref = v0.copy()
+    for _ in range(2):
+        for e in w.elements:
+            elgo.matrix3(ref, e["R"], e["T"], e["U"], e["C"])
+    assert np.array_equal(ob.read()[0], ref)
