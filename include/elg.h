@@ -62,7 +62,9 @@ enum { ELG_MOM_NONE = 0, ELG_MOM_TURN = 1, ELG_MOM_ELEMENT = 2 };
  *                                   in the long-run kernel (12 parameter slots)
  *   RFKICK (G8): V [V], f [Hz], phi [rad].
  *                                   delta += V/(beta0 p0c) sin(phi + 2 pi f (s - s_ref)/(beta0 c)),
- *                                   s_ref = design path length in front of the element on this turn
+ *                                   s_ref = design path length in front of the element on this turn, or with
+ *                                   fiducial = 1 (the reduction of PAPER.md:154; G36) s_design + the exactly
+ *                                   accumulated mean of s - s_design over the live particles
  *   RCOL   (G17): ax, ay [m].  survive iff |x| <= ax and |y| <= ay
  *   ECOL   (G17): ax, ay [m] semi-axes.  survive iff (x/ax)^2 + (y/ay)^2 <= 1
  *   WAKE   (G9-G16): nb bins, window mode (+ t_lo_rel, dt if EXPLICIT), wake kind with
@@ -81,7 +83,7 @@ typedef struct {
     int32_t window;
     int32_t wake;
     int32_t interp;
-    int32_t reserved;
+    int32_t fiducial;   /* RFKICK: 1 = phase reference on the bunch's mean path length (G36), 0 = design orbit (G8) */
     double L;
     double V, f, phi;
     double ax, ay;

@@ -15,6 +15,7 @@
  *   elgo_matrix2      pinned  - T = 0 equals elgo_matrix bitwise, one-entry index pins, thin sextupole and
  *                               second-order drift closed forms (exact drift to O(x'^4))
  *   elgo_rfkick       pinned  - crest/zero-crossing/periodicity/slope closed forms
+ *   elgo_fiducial     pinned  - exact mean (math.fsum), order-free, kicks invariant under a common delay
  *   elgo_aperture     pinned  - hand-placed particles, brute-force stable partition, erf fractions
  *   elgo_window/histogram  pinned - hand-placed bins, edge rule, sum of counts
  *   elgo_wake_samples pinned  - beam-loading theorem, independent evaluation
@@ -57,7 +58,7 @@ enum { ELGO_MOM_NONE = 0, ELGO_MOM_TURN = 1, ELGO_MOM_ELEMENT = 2 };
  *           (0,0) (0,1) .. (0,5) (1,1) .. (5,5)): second-order transport map (G31)
  *   MATRIX3: MATRIX2 plus U (336 = 6 x 56, U[56*i + t], t numbers the triples (j,k,l), j <= k <= l, in
  *           lexicographic order): third-order transport map (G35)
- *   RFKICK: V [V], f [Hz], phi [rad]
+ *   RFKICK: V [V], f [Hz], phi [rad], fiducial
  *   RCOL  : ax, ay [m]      ECOL: ax=a, ay=b [m]
  *   WAKE  : nb, window, (t_lo_rel, dt if EXPLICIT), wake kind, (f, Q, Rs) or (table, n_table, dt_table), interp
  *   HISTO : nb, window, t_lo_rel, dt   (histogram only, no kick)
@@ -69,7 +70,7 @@ typedef struct {
     int32_t window;
     int32_t wake;
     int32_t interp;
-    int32_t reserved;
+    int32_t fiducial;   /* RFKICK: 1 = phase reference on the bunch's mean path length (G36), 0 = design (G8) */
     double L;
     double V, f, phi;
     double ax, ay;
@@ -94,6 +95,8 @@ void   elgo_matrix2(double* const v[6], int64_t n, const double* R36, const doub
 /* third-order map (G35): ... + sum_{j<=k<=l} U_ijkl v_j v_k v_l */
 void   elgo_matrix3(double* const v[6], int64_t n, const double* R36, const double* C6, const double* T126,
                     const double* U336);
+/* G36: s_design + (exact fixed-point sum of the rounded differences s_i - s_design, G33) / n; n = 0: s_design */
+double elgo_fiducial(const double* s, int64_t n, double s_design);
 void   elgo_rfkick(const double* s, double* delta, int64_t n, double A, double omega, double phi0,
                    double s_ref, double inv_bc);
 /* survive[i] = 1/0.  kind = ELGO_RCOL or ELGO_ECOL. */

@@ -41,7 +41,7 @@ _u8p = C.POINTER(C.c_uint8)
 class Element(C.Structure):
     _fields_ = [
         ("type", C.c_int32), ("nb", C.c_int32), ("window", C.c_int32), ("wake", C.c_int32),
-        ("interp", C.c_int32), ("reserved", C.c_int32),
+        ("interp", C.c_int32), ("fiducial", C.c_int32),
         ("L", C.c_double), ("V", C.c_double), ("f", C.c_double), ("phi", C.c_double),
         ("ax", C.c_double), ("ay", C.c_double), ("Q", C.c_double), ("Rs", C.c_double),
         ("t_lo_rel", C.c_double), ("dt", C.c_double), ("dt_table", C.c_double),
@@ -88,6 +88,8 @@ def lib():
         L.elgo_matrix3.restype = None
         L.elgo_rfkick.argtypes = [_dp, _dp, C.c_int64] + [C.c_double] * 5
         L.elgo_rfkick.restype = None
+        L.elgo_fiducial.argtypes = [_dp, C.c_int64, C.c_double]
+        L.elgo_fiducial.restype = C.c_double
         L.elgo_aperture_flags.argtypes = [_dp, _dp, C.c_int64, C.c_int32, C.c_double, C.c_double, _u8p]
         L.elgo_aperture_flags.restype = None
         L.elgo_compact.argtypes = [v6, _i64p, C.c_int64, _u8p, v6, _i64p]
@@ -190,6 +192,11 @@ def matrix3(v: np.ndarray, R, T, U, Cvec=None) -> None:
 
 def rfkick(v: np.ndarray, A: float, omega: float, phi0: float, s_ref: float, inv_bc: float) -> None:
     lib().elgo_rfkick(_p(v[4]), _p(v[5]), v.shape[1], A, omega, phi0, s_ref, inv_bc)
+
+
+def fiducial(s: np.ndarray, s_design: float) -> float:
+    s = _f64(s)
+    return lib().elgo_fiducial(_p(s), s.shape[0], s_design)
 
 
 def aperture_flags(x: np.ndarray, y: np.ndarray, kind: int, ax: float, ay: float) -> np.ndarray:
@@ -315,6 +322,7 @@ def _elements_to_c(elements):
                 Cv = _f64(d["C"]).reshape(6); keep.append(Cv); e.C = _p(Cv)
         elif t == "RFKICK":
             e.type, e.V, e.f, e.phi = RFKICK, float(d["V"]), float(d["f"]), float(d["phi"])
+            e.fiducial = 1 if d.get("fiducial", False) else 0
         elif t == "RCOL":
             e.type, e.ax, e.ay = RCOL, float(d["ax"]), float(d["ay"])
         elif t == "ECOL":

@@ -816,6 +816,16 @@ struct Tracker {
                     break;
                 }
                 case ELG_RFKICK:
+                    if (e.fiducial) {                                        // G36: needs the particles in memory
+                        flush(AP_NONE, 0, 0, 0, false);
+                        count();
+                        if (b && ok()) {
+                            ProfScope ps(b, ELG_K_MOMENTS);
+                            fiducial_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(b->coord(b->cur_buf, 4), b->st, b->cur_slot, s_here);
+                            check(cudaGetLastError(), "fiducial_kernel launch");
+                        }
+                        op.coef[5] = 1.0;
+                    }
                     op.type = OP_RFKICK;
                     op.coef[0] = e.V * (b ? b->inv_E : 0.0); op.coef[1] = kTwoPi * e.f; op.coef[2] = e.phi;
                     op.coef[3] = s_here; op.coef[4] = b ? b->inv_bc : 0.0;

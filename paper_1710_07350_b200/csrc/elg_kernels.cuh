@@ -45,7 +45,9 @@ struct DevState {
     unsigned int tile_counter; // dynamic tile ids for the look-back scan
     unsigned int done_counter;
     unsigned int mom_done;
-    unsigned int pad;
+    unsigned int fid_done;
+    unsigned long long fid_acc[2];   // exact fixed-point sum of s - s_design (G36)
+    double s_ref;              // fiducial path length of the bunch, read by RFKICK ops with the fiducial flag
 };
 
 struct ChainCommon {
@@ -224,7 +226,8 @@ __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, 
             v[p][4] = fma(L, sqrt(u), v[p][4]);
         }
     } else if (ty == OP_RFKICK) {                                // G8
-        const double A = c[0], omega = c[1], phi0 = c[2], s_ref = c[3], inv_bc = c[4];
+        const double A = c[0], omega = c[1], phi0 = c[2], inv_bc = c[4];
+        const double s_ref = (c[5] != 0.0) ? cm.st->s_ref : c[3];            // G36 (bunch fiducial) / G8 (design)
 #pragma unroll
         for (int p = 0; p < P; p++) {
             const double tau = (v[p][4] - s_ref) * inv_bc;
@@ -1014,6 +1017,50 @@ __global__ void __launch_bounds__(kBlock) dipole_finalize_kernel(const unsigned 
 }
 
 // ---------------------------------------------------------------------------------------------------
+// fiducial_kernel (G36; the reduction of simple_rf_cavity): s_ref = s_design + (exact fixed-point
+// sum of s_i - s_design) / n.  64-bit integer sums per thread, shuffle tree, one global integer atomic per block;
+// the last block to finish converts, publishes s_ref in the device state and re-arms the accumulators.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlock) fiducial_kernel(const double* s, DevState* st, int cur, double s_design) {
+    const long long n = st->n_alive[cur];
+    long long H = 0, L = 0;
+    const long long stride = (long long)gridDim.x * kBlock * 2;
+    for (long long i0 = ((long long)blockIdx.x * kBlock + threadIdx.x) * 2; i0 < n; i0 += stride) {
+        double a, b = 0.0;
+        const bool two = i0 + 2 <= n;
+        if (two) { const double2 t = ld_stream2(s + i0); a = t.x; b = t.y; }
+        else a = ld_stream1(s + i0);
+        long long h, l;
+        if (fixed_split(a - s_design, &h, &l)) { H += h; L += l; }
+        if (two && fixed_split(b - s_design, &h, &l)) { H += h; L += l; }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        H += __shfl_xor_sync(0xffffffffu, H, d);
+        L += __shfl_xor_sync(0xffffffffu, L, d);
+    }
+    __shared__ long long s_h[kWarps], s_l[kWarps];
+    __shared__ bool s_last;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { s_h[wid] = H; s_l[wid] = L; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < kWarps; w++) { H += s_h[w]; L += s_l[w]; }
+        atomicAdd(&st->fid_acc[0], (unsigned long long)H);
+        atomicAdd(&st->fid_acc[1], (unsigned long long)L);
+        __threadfence();
+        s_last = (atomicAdd(&st->fid_done, 1u) == gridDim.x - 1);
+        if (s_last) {
+            __threadfence();
+            const long long Ht = (long long)atomicAdd(&st->fid_acc[0], 0ull), Lt = (long long)atomicAdd(&st->fid_acc[1], 0ull);
+            const double sum = fma((double)Ht, 1.0 / 4294967296.0, (double)Lt * (1.0 / 18446744073709551616.0));
+            st->s_ref = (n > 0) ? s_design + sum / (double)n : s_design;
+            st->fid_acc[0] = 0ull; st->fid_acc[1] = 0ull; st->fid_done = 0;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // wake_samples_kernel (a10; G11, G12): W_k = W(k dt), k < nb, in V/C.
 // ---------------------------------------------------------------------------------------------------
 struct WakeArgs {
@@ -1241,7 +1288,8 @@ __global__ void init_state_kernel(DevState* st, long long n0) {
     st->win[0] = 0.0; st->win[1] = 1.0; st->win[2] = 1.0; st->win[3] = 0.0;
     st->smin = 0.0; st->smax = 0.0;
     st->bin_lo = 0; st->bin_hi = -1;
-    st->tile_counter = 0; st->done_counter = 0; st->mom_done = 0; st->pad = 0;
+    st->tile_counter = 0; st->done_counter = 0; st->mom_done = 0; st->fid_done = 0;
+    st->fid_acc[0] = 0ull; st->fid_acc[1] = 0ull; st->s_ref = 0.0;
 }
 
 }  // namespace elg

@@ -47,7 +47,7 @@ class ElgError(RuntimeError):
 class Element(C.Structure):
     _fields_ = [
         ("type", C.c_int32), ("nb", C.c_int32), ("window", C.c_int32), ("wake", C.c_int32),
-        ("interp", C.c_int32), ("reserved", C.c_int32),
+        ("interp", C.c_int32), ("fiducial", C.c_int32),
         ("L", C.c_double), ("V", C.c_double), ("f", C.c_double), ("phi", C.c_double),
         ("ax", C.c_double), ("ay", C.c_double), ("Q", C.c_double), ("Rs", C.c_double),
         ("t_lo_rel", C.c_double), ("dt", C.c_double), ("dt_table", C.c_double),
@@ -176,6 +176,7 @@ def _elements_to_c(elements):
                 Cv = _f64(d["C"]).reshape(6); keep.append(Cv); e.C = _p(Cv)
         elif t == "RFKICK":
             e.type, e.V, e.f, e.phi = RFKICK, float(d["V"]), float(d["f"]), float(d["phi"])
+            e.fiducial = 1 if d.get("fiducial", False) else 0
         elif t == "RCOL":
             e.type, e.ax, e.ay = RCOL, float(d["ax"]), float(d["ay"])
         elif t == "ECOL":

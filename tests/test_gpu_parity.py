@@ -206,6 +206,23 @@ def test_second_order_mixed_with_other_maps(elg, elgo):
     check_lost(ob, gb)
 
 
+@pytest.mark.parametrize("n", [1, 513, 150_001])
+def test_fiducial_rf_phase(elg, elgo, n):
+    """RFKICK with the phase reference on the bunch (G36): exact integer reduction, so s_ref is bit-identical and
+    delta differs by sin's 2 ulp only."""
+    ring = _long_line(23, {})
+    elems = [ring[0], {"type": "RFKICK", "V": 2e6, "f": 1.3e9, "phi": 0.9, "fiducial": True}, ring[1],
+             {"type": "DRIFT", "L": 0.5}, {"type": "RFKICK", "V": 1e6, "f": 2.856e9, "phi": 2.0, "fiducial": True},
+             {"type": "RFKICK", "V": 1e6, "f": 2.856e9, "phi": 0.1}, ring[2]]
+    v0 = make_workload("cfg0", n=n).particles()
+    v0[4] += 2.5e-4                                          # the bunch is late: fiducial and design phase differ
+    ob = elgo.Bunch(v0, 1e9, 1e-9); ob.track(elgo.Beamline(elems, ring=True), 3)
+    gbl = elg.Beamline(elems, ring=True); gb = elg.Bunch(v0, 1e9, 1e-9, beamline=gbl); gb.track(gbl, 3)
+    ov, _ = ob.read(); gv, _ = gb.read()
+    assert np.array_equal(gv[:5], ov[:5])
+    assert rel_err(gv, ov) <= 1e-12
+
+
 # ------------------------------------------------------------------------------------ (ii) loss
 def test_compaction_hand_placed(elg, elgo):
     """Edge-inclusive, NaN lost, Fig. 2 shape (20 particles, 4 lost)."""

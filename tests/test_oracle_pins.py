@@ -778,3 +778,31 @@ def test_matrix3_in_track(elgo):
         for e in w.elements:
             elgo.matrix3(ref, e["R"], e["T"], e["U"], e["C"])
     assert np.array_equal(ob.read()[0], ref)
+
+
+# ------------------------------------------------------------------------------------ fiducial RF phase (G36)
+def test_fiducial_is_the_exact_mean_and_makes_kicks_delay_invariant(elgo):
+    import math
+    rng = np.random.default_rng(31)
+    s0 = 271.25
+    s = s0 + rng.normal(size=50_000) * 1e-3 + 3e-4
+    f = elgo.fiducial(s, s0)
+    assert abs(f - (s0 + math.fsum(s - s0) / s.size)) <= 1e-15 * s0
+    assert elgo.fiducial(s[rng.permutation(s.size)], s0) == f                 # order-free
+    assert elgo.fiducial(s[:0], s0) == s0
+    # a common delay of the whole bunch changes the design-orbit kick but not the fiducial one
+    w = make_workload("cfg0", n=2000)
+    v0 = w.particles()
+    def kicks(fid, shift):
+        v = v0.copy(); v[4] += shift
+        ob = elgo.Bunch(v, 1e9, 1e-9)
+        ob.track(elgo.Beamline([{"type": "DRIFT", "L": 1.0}, {"type": "RFKICK", "V": 1e6, "f": 2.856e9, "phi": 0.3,
+                                                          "fiducial": fid}]), 1)
+        return ob.read()[0][5] - v0[5]
+    a, b_ = kicks(True, 0.0), kicks(True, 7e-3)
+    assert np.max(np.abs(a - b_)) <= 1e-9 * np.max(np.abs(a))                 # s + shift rounds at 1e-16 relative
+    c, d = kicks(False, 0.0), kicks(False, 7e-3)
+    assert np.max(np.abs(c - d)) > 0.1 * np.max(np.abs(c))
+    # with the fiducial the mean phase is phi exactly: the mean kick is A sin(phi) <cos> ~ A sin(phi)
+    A = 1e6 * elgo.inv_E(elgo.beta0(1e9), 1e9)
+    assert abs(a.mean() / (A * math.sin(0.3)) - 1.0) < 2e-3
