@@ -208,8 +208,12 @@ int32_t device_sms(int* sms) {
 int32_t long_setup_once() {
     static bool done = false;
     if (!done) {
-        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    chain_long_smem_bytes<kMaxOpsLarge>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    chain_long_smem_bytes<kMaxOpsLarge, 0>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    chain_long_smem_bytes<kMaxOpsLarge, 1>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    chain_long_smem_bytes<kMaxOpsLarge, 2>()));
         done = true;
     }
     return ELG_OK;
@@ -491,7 +495,7 @@ struct Tracker {
         return (int)g;
     }
 
-    template <int MAXOPS, bool COMPACT, int P, bool EXT>
+    template <int MAXOPS, bool COMPACT, int P, int EXT>                // EXT: 0 basic maps, 1 + MATRIX2 / TKICK, 2 + MATRIX3
     void launch_chain(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm, unsigned rmask, unsigned wmask) {
         count();
         if (!b) return;
@@ -519,25 +523,25 @@ struct Tracker {
             std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
         }
         int grid = 0;
-        if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS>, chain_long_smem_bytes<MAXOPS>());
+        if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS, EXT>, chain_long_smem_bytes<MAXOPS, EXT>());
         else if constexpr (COMPACT) {
-            grid = cached_grid((const void*)compact_kernel<MAXOPS, EXT>, 0);
+            grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0)>, 0);
             if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
-        } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, EXT>, 0);
+        } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, (EXT != 0)>, 0);
         if (!ok()) return;
         if (want_mm) mm_grid = grid;
         {
             ProfScope ps(b, MAXOPS == kMaxOpsLarge ? ELG_K_CHAIN_LONG : (COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN));
             if constexpr (MAXOPS == kMaxOpsLarge)
-                chain_long_kernel<MAXOPS><<<grid, kBlock, chain_long_smem_bytes<MAXOPS>(), b->stream>>>(a);
+                chain_long_kernel<MAXOPS, EXT><<<grid, kBlock, chain_long_smem_bytes<MAXOPS, EXT>(), b->stream>>>(a);
             else if constexpr (COMPACT)
             {
                 void* kargs[] = {(void*)&a};                     // cooperative: every block resident (static tiles)
-                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS, EXT>, dim3(grid), dim3(kBlock), kargs, 0, b->stream),
+                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS, (EXT != 0)>, dim3(grid), dim3(kBlock), kargs, 0, b->stream),
                       "compact_kernel cooperative launch");
             }
             else
-                chain_kernel<MAXOPS, P, EXT><<<grid, kBlock, 0, b->stream>>>(a);
+                chain_kernel<MAXOPS, P, (EXT != 0)><<<grid, kBlock, 0, b->stream>>>(a);
         }
         check(cudaGetLastError(), "chain_kernel launch");
         if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
@@ -569,13 +573,20 @@ struct Tracker {
         bool p4 = n_mat >= kMatricesForP4;
         if (b && b->force_p == 2) p4 = false;
         if (b && b->force_p == 4) p4 = true;
-        bool ext = false;                                             // rarely used maps: the EXT instantiations
-        for (const HostOp& op : pending) ext = ext || op.type == OP_MATRIX2 || op.type == OP_MATRIX3 || op.type == OP_TKICK;
+        int ext = 0;                                                  // rarely used maps: higher EXT instantiations
+        for (const HostOp& op : pending) {
+            if (op.type == OP_MATRIX2 || op.type == OP_TKICK) ext = ext < 1 ? 1 : ext;
+            if (op.type == OP_MATRIX3) ext = 2;
+        }
 #define ELG_LAUNCH(M, C, PP, E) launch_chain<M, C, PP, E>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
-        if (large)   { ELG_LAUNCH(kMaxOpsLarge, false, kPL, true); }
-        else if (compact) { if (ext) ELG_LAUNCH(kMaxOpsSmall, true, 2, true); else ELG_LAUNCH(kMaxOpsSmall, true, 2, false); }
-        else if (p4) { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 4, true); else ELG_LAUNCH(kMaxOpsSmall, false, 4, false); }
-        else         { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 2, true); else ELG_LAUNCH(kMaxOpsSmall, false, 2, false); }
+        if (large) {
+            if (ext == 2) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 2);
+            else if (ext == 1) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 1);
+            else ELG_LAUNCH(kMaxOpsLarge, false, kPL, 0);
+        }
+        else if (compact) { if (ext) ELG_LAUNCH(kMaxOpsSmall, true, 2, 1); else ELG_LAUNCH(kMaxOpsSmall, true, 2, 0); }
+        else if (p4) { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 4, 1); else ELG_LAUNCH(kMaxOpsSmall, false, 4, 0); }
+        else         { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 2, 1); else ELG_LAUNCH(kMaxOpsSmall, false, 2, 0); }
 #undef ELG_LAUNCH
         if (compact || (wmask & 0x10)) mm_valid = want_mm;
         else mm_valid = mm_valid || want_mm;

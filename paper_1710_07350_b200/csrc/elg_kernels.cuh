@@ -315,7 +315,9 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
 
 // the run's maps with the coefficients in shared memory (copied there once per block): 128-bit fetches, and
 // consecutive MATRIX maps applied in pairs (v -> w -> v) so that no register copy-back is needed
-template <int MAXOPS, int P>
+// LEVEL 0: MATRIX, DRIFT, RFKICK, KICK; 1: + MATRIX2, TKICK; 2: + MATRIX3.  The planner picks the lowest level a run
+// needs: the higher-order code costs the 200-matrix cfg3 kernel registers and 30 % of its speed when compiled in.
+template <int MAXOPS, int P, int LEVEL>
 __device__ __forceinline__ void apply_ops_smem(const ChainArgs<MAXOPS>& a, const double* s_coef, double (&v)[P][6]) {
     const ChainCommon& c = a.c;
     int op = 0;
@@ -326,18 +328,18 @@ __device__ __forceinline__ void apply_ops_smem(const ChainArgs<MAXOPS>& a, const
             matrix_map_s128<P>(s_coef + 42 * op, v, w);
             matrix_map_s128<P>(s_coef + 42 * (op + 1), w, v);
             op += 2;
-        } else if (ty == OP_MATRIX || ty == OP_MATRIX2 || ty == OP_MATRIX3) {
+        } else if (ty == OP_MATRIX || (LEVEL >= 1 && ty == OP_MATRIX2) || (LEVEL >= 2 && ty == OP_MATRIX3)) {
             double w[P][6];
             matrix_map_s128<P>(s_coef + 42 * op, v, w);
-            if (ty != OP_MATRIX) matrix2_terms<P>(s_coef + 42 * (op + 1), v, w);
-            if (ty == OP_MATRIX3) matrix3_terms<P>(s_coef + 42 * (op + 4), v, w);
+            if (LEVEL >= 1 && ty != OP_MATRIX) matrix2_terms<P>(s_coef + 42 * (op + 1), v, w);
+            if (LEVEL >= 2 && ty == OP_MATRIX3) matrix3_terms<P>(s_coef + 42 * (op + 4), v, w);
 #pragma unroll
             for (int p = 0; p < P; p++)
 #pragma unroll
                 for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
             op += (ty == OP_MATRIX3) ? 12 : ((ty == OP_MATRIX2) ? 4 : 1);
         } else {
-            other_map<P>(ty, s_coef + 42 * op, c, v);
+            other_map<P, (LEVEL >= 1)>(ty, s_coef + 42 * op, c, v);
             op++;
         }
     }
@@ -449,8 +451,9 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
 //     the 16-byte chunks it will read itself (no block-wide barrier in the tile loop).
 // Same arithmetic, in the same order, as chain_kernel.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kPL = 6;
-constexpr int kTileL = kBlock * kPL;
+constexpr int kPL = 6;                                  // particles per thread of the long-run kernel (levels 0, 1)
+constexpr int kPL3 = 4;                                 // with third-order maps (level 2): 6 would spill
+__host__ __device__ constexpr int long_pl(int level) { return level >= 2 ? kPL3 : kPL; }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
     const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
@@ -465,12 +468,14 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-template <int MAXOPS>
-constexpr int chain_long_smem_bytes() { return MAXOPS * 42 * 8 + 6 * kTileL * 8; }
+template <int MAXOPS, int LEVEL>
+constexpr int chain_long_smem_bytes() { return MAXOPS * 42 * 8 + 6 * kBlock * long_pl(LEVEL) * 8; }
 
-template <int MAXOPS>
+template <int MAXOPS, int LEVEL>
 __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
-    constexpr int H = kPL / 2;
+    constexpr int PL = long_pl(LEVEL);
+    constexpr int kTileL = kBlock * PL;
+    constexpr int H = PL / 2;
     constexpr int kSub = 2 * kBlock;
     extern __shared__ __align__(16) double sm_long[];
     double* s_coef = sm_long;                                    // [n_ops][42]
@@ -502,7 +507,7 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
     if (tile < n_tiles) prefetch(tile);
     __syncthreads();                                             // s_coef complete
     while (tile < n_tiles) {
-        double v[kPL][6];
+        double v[PL][6];
         cp_async_wait_all();
 #pragma unroll
         for (int h = 0; h < H; h++)
@@ -515,7 +520,7 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
         const long long next = tile + gridDim.x;
         if (next < n_tiles) prefetch(next);                      // own slots only: already in registers
 
-        apply_ops_smem<MAXOPS, kPL>(a, s_coef, v);
+        apply_ops_smem<MAXOPS, PL, LEVEL>(a, s_coef, v);
 
         const long long t0 = tile * kTileL + (long long)threadIdx.x * 2;
 #pragma unroll
