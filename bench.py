@@ -441,6 +441,61 @@ def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
                         "peak": hbm_peak, "frac": ach / hbm_peak, "frac_of_8TBs": ach / NOMINAL_HBM_GBS})
         out.append({"workload": name, "kernel": "whole pass", "ms_per_pass": ms_total / k,
                     "value": passes / (ms_total / k * 1e-3) / 1e6, "unit": UNIT, "n_alive_after": int(n_alive)})
+    # P3: chain-length sweep over k cfg3 matrices in one fused run: the HBM -> fp64 crossover
+    for k in (1, 2, 4, 8, 16, 40, 80):
+        w = make_workload("p3-matrices", n=n0, n_matrices=k)
+        bl = elg.Beamline(w.elements, ring=True)
+        for _ in range(2):
+            gb.track(bl, 1, moments_every="none", records=False)
+        gb.synchronize()
+        ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(3):
+            gb.track(bl, 1, moments_every="none", records=False)
+        ev1.record(stream)
+        torch.cuda.synchronize(dev)
+        ms = ev0.elapsed_time(ev1) / 3
+        out.append({"workload": "p3-matrices", "matrices": k, "ms_per_run": ms, "hbm_gbs": 96.0 * n0 / (ms * 1e-3) / 1e9,
+                    "fp64_tflops": 72.0 * k * n0 / (ms * 1e-3) / 1e12, "value": float(n0) * k / (ms * 1e-3) / 1e6,
+                    "unit": UNIT})
+    restore()
+
+    # P0: single-element launches at the paper's Table I size (3.2 M particles), beside its V100 / K20c /
+    # one-CPU-core times (other hardware: context only).  179 MB of particle data is partly
+    # L2-resident on B200, so these are not HBM-clean numbers.
+    n_t1 = min(3_200_000, n0)
+    cfg0 = make_workload("cfg0", n=n_t1)
+    cfg1 = make_workload("cfg1", n=n_t1)
+    t1_elems = [
+        ("exactDrift", {"type": "DRIFT", "L": 1.0}, "none", (0.17, 0.835, 17.8)),
+        ("track_particles (M1)", cfg0.elements[1], "none", (0.42, 1.98, 69.9)),
+        ("simple_rf_cavity", {"type": "RFKICK", "V": 1e6, "f": 2.856e9, "phi": 1.0, "fiducial": True}, "none", (0.75, 3.51, 164.0)),
+        ("rectangular_collimator", cfg0.elements[2], "none", (0.27, 1.23, 59.3)),
+        ("elliptical_collimator", cfg1.elements[1], "none", (0.31, 2.63, 78.9)),
+        ("track_through_wake", cfg0.elements[3], "none", (0.34, 1.33, 25.6)),
+        ("accumulate_beam_sums", None, "turn", (4.08, 24.8, 696.0)),
+    ]
+    small = elg.Bunch(None, w_main.p0c_eV, w_main.charge_C, beamline=None, n0=n_t1, device=str(dev), lost_capacity=n_t1)
+    hp = torch.empty((6, n_t1), dtype=torch.float64, pin_memory=True)
+    cfg0.particles(n_t1, out=hp.numpy())
+    small.upload(hp); small.synchronize()
+    keep = small.soa.clone()
+    for name, el, mom, paper in t1_elems:
+        bl = elg.Beamline([el] if el is not None else [], ring=False)
+        times = []
+        for rep in range(8):
+            small.soa.copy_(keep); small.rewind(); small.synchronize()
+            ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+            ev0.record(stream)
+            small.track(bl, 1, moments_every=mom, records=False)
+            ev1.record(stream)
+            torch.cuda.synchronize(dev)
+            if rep >= 3:
+                times.append(ev0.elapsed_time(ev1))
+        out.append({"workload": "table1", "function": name, "particles": n_t1, "ms": float(np.median(times)),
+                    "paper_ms": {"V100": paper[0], "K20c": paper[1], "i7-3770K 1 core": paper[2]}})
+    del small
+
     # fp64-bound probe of the NEXT row: second-order maps in the long-run kernel
     w = make_workload("p4-second-order", n=n0, n_cells=20)
     bl = elg.Beamline(w.elements, ring=True)

@@ -35,6 +35,7 @@ constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr int kMaxOpsSmall = 8;
 constexpr int kMaxOpsLarge = 80;                        // 80 x 42 x 8 B = 26.9 KB of kernel parameters
 constexpr int kMatricesForP4 = 3;                       // runs with >= 3 MATRIX maps use 4 particles per thread
+constexpr int kMatricesForLong = 5;                     // runs with >= 5 use the long-run kernel
 constexpr int kMaxGrid = 4096;
 constexpr long long kRecCap = 2048;                     // device ring of moment records
 constexpr int kNbDefault = 65536;
@@ -564,7 +565,11 @@ struct Tracker {
             }
         }
         if (want_mm) rmask |= 0x10;
-        const bool large = pending.size() > (size_t)kMaxOpsSmall;
+        // the long-run kernel (coefficients in shared memory, 6 particles per thread) also takes the short runs that
+        // are already fp64-bound: from 5 matrices on it beats the parameter-bank kernel (bench.py p3 sweep)
+        int n_mat_run = 0;
+        for (const HostOp& op : pending) n_mat_run += (op.type == OP_MATRIX) + 4 * (op.type == OP_MATRIX2);
+        const bool large = pending.size() > (size_t)kMaxOpsSmall || (ap_type == AP_NONE && n_mat_run >= kMatricesForLong);
         const bool compact = ap_type != AP_NONE;
         // particles per thread: 2 while the run is HBM-bound; 4 once it holds enough MATRIX maps for the
         // coefficient fetches (one per 2 particles) to matter
