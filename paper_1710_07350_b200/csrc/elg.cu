@@ -97,6 +97,7 @@ struct elg_bunch {
     long long rec_count = 0;                            // records in the device ring
     // launch geometry
     int sms = 0;
+    std::map<int, int> hist_grids;                      // hist_kernel grid per shared-memory size
     std::map<const void*, int> grids;                   // persistent grid size per chain kernel instantiation
     int force_p = 0;                                    // ELG_CHAIN_P = 2 | 4 overrides the planner's choice
     int grid_hist = 0, grid_mom = 0, grid_dipole = 0;
@@ -483,6 +484,17 @@ struct Tracker {
         if (e != cudaSuccess && rc == ELG_OK) rc = fail(ELG_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
     }
 
+    int hist_grid(int smem_bins) {                                    // resident blocks of hist_kernel for this much shared memory
+        auto it = b->hist_grids.find(smem_bins);
+        if (it != b->hist_grids.end()) return it->second;
+        int occ = 0;
+        check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_kernel, kBlock, (size_t)smem_bins * 4), "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+        if (occ < 1) occ = 1;
+        const int g = occ * b->sms;
+        b->hist_grids[smem_bins] = g;
+        return g;
+    }
+
     // blocks of a persistent grid = resident blocks per SM x SMs, looked up once per kernel
     int cached_grid(const void* kernel, int smem) {
         auto it = b->grids.find(kernel);
@@ -703,8 +715,12 @@ struct Tracker {
                 h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1;
                 h.inv_bc = b->inv_bc; h.t_lo = 0; h.inv_dt = 0; h.nb = e.nb; h.counts = b->counts;
                 h.aggregate = b->hist_aggregate < 0 ? 0 : b->hist_aggregate;
+                // one private copy per warp needs 8 nb bins: small histograms take less shared memory and get more
+                // resident blocks (more loads in flight)
+                h.smem_bins = (8LL * e.nb < kHistSmemBins) ? 8 * e.nb : kHistSmemBins;
                 ProfScope ps(b, ELG_K_HIST);
-                hist_kernel<<<b->grid_hist, kBlock, kHistSmemBins * 4, b->stream>>>(h);
+                hist_kernel<<<hist_grid(h.smem_bins), kBlock, h.smem_bins * 4, b->stream>>>(h);
+
             }
             check(cudaGetLastError(), "hist_kernel launch");
             stage_out_hist(e.nb);
@@ -1015,6 +1031,7 @@ extern "C" int32_t elg_dbg_histogram(const double* d_s, int64_t n, double inv_bc
     const char* agg = std::getenv("ELG_HIST_AGGREGATE");
     h.aggregate = agg ? std::atoi(agg) : 0;
     h.counts = d_counts;
+    h.smem_bins = kHistSmemBins;
     hist_kernel<<<grid * sms, kBlock, kHistSmemBins * 4, (cudaStream_t)stream>>>(h);
     g_launches++;
     ELG_CK(cudaGetLastError());

@@ -844,6 +844,7 @@ struct HistArgs {
     double inv_bc, t_lo, inv_dt;
     int nb;
     int aggregate;         // 1: warp-aggregate equal bins with match.any before the shared atomic
+    int smem_bins;         // bins of dynamic shared memory this launch was given (<= kHistSmemBins)
     unsigned int* counts;
 };
 
@@ -855,8 +856,8 @@ __global__ void __launch_bounds__(kBlock) hist_kernel(const HistArgs a) {
     else { n = a.st->n_alive[a.cur]; blo = a.st->bin_lo; bhi = a.st->bin_hi; t_lo = a.st->win[0]; inv_dt = a.st->win[2]; }
     long long span = bhi - blo + 1;
     if (span < 1) span = 1;
-    const int S = (int)(span < kHistSmemBins ? span : kHistSmemBins);
-    int R = kHistSmemBins / S;
+    const int S = (int)(span < a.smem_bins ? span : a.smem_bins);
+    int R = a.smem_bins / S;
     if (R > kWarps) R = kWarps;
     const int wid = threadIdx.x >> 5;
     unsigned int* mine = sh + (wid % R) * S;
