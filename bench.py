@@ -332,7 +332,7 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         k_e2e = max(1, min(args.steps, args.e2e_steps))
-        gb.upload(h_pinned); gb.track(gbl, 1, moments_every="turn"); gb.synchronize()      # warm-up
+        gb.upload_and_track(h_pinned, gbl, 1, moments_every="turn", n_chunks=args.e2e_chunks); gb.synchronize()   # warm-up
         pdist.barrier(); torch.cuda.synchronize(dev)
         ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
         t0 = time.perf_counter()
@@ -340,8 +340,9 @@ def run_ours(args):
         e_passes = 0.0
         rec = None
         for _ in range(k_e2e):
-            gb.upload(h_pinned)                                   # elg_bunch_upload: 6 x n0 x 8 B from pinned host
-            out = gb.track(gbl, 1, moments_every="turn")          # elg_track with a HOST record buffer (syncs)
+            # elg_upload_and_track: 6 x n0 x 8 B from pinned host memory, pipelined in chunks against the turn's
+            # leading maps; HOST record buffer (the call synchronises)
+            out = gb.upload_and_track(h_pinned, gbl, 1, moments_every="turn", n_chunks=args.e2e_chunks)
             rec = out["records"]
             e_passes += float(n0) * per_turn if w.ring else line_passes(gb, w)
         ev1.record(stream)
@@ -350,7 +351,9 @@ def run_ours(args):
         e_max, e_all = pdist.aggregate(e_ms, e_passes, dev if world > 1 else None)
         e2e = {"value": e_all / (e_max * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 6 * n0 * 8,
                "d2h_bytes_per_step": int(rec.size * 8), "steps": k_e2e, "ms_per_step": e_max / k_e2e,
-               "what": "elg_bunch_upload from pinned host memory + elg_track(1 turn, host moments record)"}
+               "chunks": args.e2e_chunks,
+               "what": "elg_upload_and_track: pinned host arrays -> device in chunks, overlapped with the turn's leading maps; "
+                       "1 turn, host moments record"}
 
     # ---- HBM-bound probes at the same particle count (north_star target kernels)
     probes = []
@@ -529,6 +532,7 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="particles per GPU (default: the workload's own count)")
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="particles of the oracle's bounded sample")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-chunks", type=int, default=16, help="particle ranges of the pipelined upload (1: no overlap)")
     ap.add_argument("--probe-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -174,6 +174,16 @@ int32_t elg_bunch_rewind(elg_bunch*);
 /* Track n_turns passes through the beamline.  opts nullable. */
 int32_t elg_track(elg_bunch*, const elg_beamline*, int64_t n_turns, elg_track_opts* opts);
 
+/* elg_bunch_upload followed by elg_track in ONE call with the upload pipelined against the tracking: the bunch is
+ * cut into n_chunks particle ranges (n_chunks <= 1: no pipelining); each range is copied from the HOST arrays on a
+ * copy stream owned by the bunch and, as soon as it has landed, the leading per-particle maps of the first turn
+ * (everything in front of the first WAKE / HISTO / TRWAKE, aperture, bunch-fiducial RFKICK or per-element record)
+ * run on that range while the following ranges are still being copied.  Results are identical to
+ * elg_bunch_upload + elg_track.  Host arrays as for elg_bunch_upload (pinned memory for real overlap); they must
+ * stay valid until the bunch's stream has been synchronised. */
+int32_t elg_upload_and_track(elg_bunch*, const elg_beamline*, const double* const h_coords[6], const int64_t* h_ids,
+                             int64_t n_turns, elg_track_opts* opts, int32_t n_chunks);
+
 /* Moments of the live particles now (north_star part 4).  n_alive == 0: ELG_ESTATE, outputs untouched. */
 int32_t elg_moments(elg_bunch*, int64_t* n_alive, double h_centroid[6], double h_sigma[36]);
 /* Lost-particle log in canonical order (G18): chronological (turn, element index), then original array

@@ -37,6 +37,7 @@ constexpr int kMaxOpsLarge = 80;                        // 80 x 42 x 8 B = 26.9 
 constexpr int kMatricesForP4 = 3;                       // runs with >= 3 MATRIX maps use 4 particles per thread
 constexpr int kMatricesForLong = 5;                     // runs with >= 5 use the long-run kernel
 constexpr int kMaxGrid = 4096;
+constexpr int kMmPartials = 16384;                      // min/max partial pairs: blocks x chunks of a pipelined upload
 constexpr long long kRecCap = 2048;                     // device ring of moment records
 constexpr int kNbDefault = 65536;
 
@@ -102,6 +103,10 @@ struct elg_bunch {
     int force_p = 0;                                    // ELG_CHAIN_P = 2 | 4 overrides the planner's choice
     int grid_hist = 0, grid_mom = 0, grid_dipole = 0;
     int hist_aggregate = 0;
+    // pipelined upload (elg_upload_and_track): the library's own copy stream and one event per chunk
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t entry_ev = nullptr;
+    std::vector<cudaEvent_t> chunk_ev;
     // optional per-kernel event timing (elg_profile_*)
     bool prof_on = false;
     struct ProfRec { int kind; cudaEvent_t t0, t1; };
@@ -167,7 +172,7 @@ WorkLayout layout(long long n0, long long nb_cap, long long table_cap, long long
     L.off_state = o; o = align_up(o + (long long)sizeof(DevState), 256);
     L.off_soaB = o; o = align_up(o + 7 * stride * 8, 256);
     L.off_status = o; o = align_up(o + (stride / kTile + 2) * 8, 256);
-    L.off_mm = o; o = align_up(o + 2LL * kMaxGrid * 8, 256);
+    L.off_mm = o; o = align_up(o + 2LL * kMmPartials * 8, 256);
     L.off_mom = o; o = align_up(o + (long long)kNMom * kMaxGrid * 8, 256);
     L.off_rec = o; o = align_up(o + (kRecCap + 1) * 43 * 8, 256);   // + 1: elg_moments' own slot
     L.off_counts = o; o = align_up(o + nb_cap * 4, 256);
@@ -418,6 +423,9 @@ extern "C" void elg_bunch_destroy(elg_bunch* b) {
         cudaStreamSynchronize(b->stream);
         b->prof_drain();
         for (cudaEvent_t e : b->prof_pool) cudaEventDestroy(e);
+        for (cudaEvent_t e : b->chunk_ev) cudaEventDestroy(e);
+        if (b->entry_ev) cudaEventDestroy(b->entry_ev);
+        if (b->copy_stream) cudaStreamDestroy(b->copy_stream);
     }
     delete b;
 }
@@ -471,6 +479,8 @@ struct Tracker {
     std::vector<HostOp> pending;
     int kick_nb = 0, kick_interp = 0;
     int tk_nb = 0, tk_interp = 0;
+    long long range_lo = 0, range_hi = -1;   // particle range of the chain launches (pipelined upload), -1: all live
+    int mm_slot = 0;                         // min/max partials of chunk c go to slot c of the partial array
     bool mm_valid = false;
     long long launches = 0;
     int32_t rc = ELG_OK;
@@ -528,7 +538,8 @@ struct Tracker {
             b->epoch = 1;
         }
         c.epoch = b->epoch;
-        c.want_minmax = want_mm ? 1 : 0; c.mm_partial = b->mm_partial;
+        c.want_minmax = want_mm ? 1 : 0;
+        c.range_lo = range_lo; c.range_hi = range_hi;
         c.V = b->V; c.nb = kick_nb; c.interp = kick_interp;
         c.Vx = b->Vt; c.Vy = b->Vt + tk_nb; c.t_nb = tk_nb; c.t_interp = tk_interp;
         for (size_t k = 0; k < pending.size(); k++) {
@@ -542,7 +553,8 @@ struct Tracker {
             if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
         } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, (EXT != 0)>, 0);
         if (!ok()) return;
-        if (want_mm) mm_grid = grid;
+        c.mm_partial = b->mm_partial + 2LL * mm_slot * grid;          // one slot of partials per chunk
+        if (want_mm) mm_grid = (mm_slot + 1) * grid;
         {
             ProfScope ps(b, MAXOPS == kMaxOpsLarge ? ELG_K_CHAIN_LONG : (COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN));
             if constexpr (MAXOPS == kMaxOpsLarge)
@@ -613,6 +625,33 @@ struct Tracker {
     void push(const HostOp& op, int slots = 1) {           // slots: parameter-block slots the op and its continuation take
         if (pending.size() + slots > (size_t)kMaxOpsLarge) flush(AP_NONE, 0, 0, 0, false);
         pending.push_back(op);
+    }
+
+    void push_higher_order(const elg_element& e) {                    // 4 slots: R, C | Tt[21][6]; MATRIX3: + 8 slots Ut[56][6]
+        HostOp op{};
+        const bool third = e.type == ELG_MATRIX3;
+        op.type = third ? OP_MATRIX3 : OP_MATRIX2;
+        std::memcpy(op.coef, e.R, 36 * sizeof(double));
+        if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
+        push(op, third ? 12 : 4);
+        for (int part = 0; part < 3; part++) {
+            HostOp t{};
+            t.type = OP_CONT;
+            for (int j = 0; j < 42; j++) {                           // layout only: pair-major transpose of T
+                const int q = (42 * part + j) / 6, r = (42 * part + j) % 6;
+                t.coef[j] = e.T[21 * r + q];
+            }
+            pending.push_back(t);
+        }
+        for (int part = 0; third && part < 8; part++) {
+            HostOp t{};
+            t.type = OP_CONT;
+            for (int j = 0; j < 42; j++) {                           // layout only: triple-major transpose of U
+                const int q = (42 * part + j) / 6, r = (42 * part + j) % 6;
+                t.coef[j] = e.U[56 * r + q];
+            }
+            pending.push_back(t);
+        }
     }
 
     void moments_record() {
@@ -805,10 +844,10 @@ struct Tracker {
         o->hist_written += nb;
     }
 
-    void run_turn(long long turn) {
+    void run_turn(long long turn, long long k_begin = 0) {
         const long long ne = (long long)bl->e.size();
         const int mom = o ? o->moments_every : ELG_MOM_NONE;
-        for (long long k = 0; k < ne && ok(); k++) {
+        for (long long k = k_begin; k < ne && ok(); k++) {
             if (skip_next) { skip_next = false; continue; }           // TRWAKE merged into the preceding WAKE
             const elg_element& e = bl->e[k];
             const double s_here = std::fma((double)turn, bl->length, bl->s_design[k]);      // G8
@@ -821,32 +860,7 @@ struct Tracker {
                     if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
                     push(op);
                     break;
-                case ELG_MATRIX2: case ELG_MATRIX3: {                        // 4 slots: R, C | Tt[21][6]; MATRIX3: + 8 slots Ut[56][6]
-                    const bool third = e.type == ELG_MATRIX3;
-                    op.type = third ? OP_MATRIX3 : OP_MATRIX2;
-                    std::memcpy(op.coef, e.R, 36 * sizeof(double));
-                    if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
-                    push(op, third ? 12 : 4);
-                    for (int part = 0; part < 3; part++) {
-                        HostOp t{};
-                        t.type = OP_CONT;
-                        for (int j = 0; j < 42; j++) {                       // layout only: pair-major transpose of T
-                            const int q = (42 * part + j) / 6, r = (42 * part + j) % 6;
-                            t.coef[j] = e.T[21 * r + q];
-                        }
-                        pending.push_back(t);
-                    }
-                    for (int part = 0; third && part < 8; part++) {
-                        HostOp t{};
-                        t.type = OP_CONT;
-                        for (int j = 0; j < 42; j++) {                       // layout only: triple-major transpose of U
-                            const int q = (42 * part + j) / 6, r = (42 * part + j) % 6;
-                            t.coef[j] = e.U[56 * r + q];
-                        }
-                        pending.push_back(t);
-                    }
-                    break;
-                }
+                case ELG_MATRIX2: case ELG_MATRIX3: push_higher_order(e); break;
                 case ELG_RFKICK:
                     if (e.fiducial) {                                        // G36: needs the particles in memory
                         flush(AP_NONE, 0, 0, 0, false);
@@ -875,6 +889,55 @@ struct Tracker {
         }
         if (mom == ELG_MOM_TURN) moments_record();
     }
+    // leading elements of the beamline that are plain per-particle maps (no collective step, aperture or record):
+    // they can run chunk by chunk while later chunks are still being uploaded
+    long long map_prefix() const {
+        const long long ne = (long long)bl->e.size();
+        if (o && o->moments_every == ELG_MOM_ELEMENT) return 0;
+        long long k = 0;
+        for (; k < ne; k++) {
+            const elg_element& e = bl->e[k];
+            const bool map = e.type == ELG_DRIFT || e.type == ELG_MATRIX || e.type == ELG_MATRIX2 || e.type == ELG_MATRIX3 ||
+                             (e.type == ELG_RFKICK && !e.fiducial);
+            if (!map) break;
+        }
+        return k;
+    }
+
+    // the map prefix of one turn on particles [lo, hi); the pending list is flushed with the min/max epilogue the next
+    // element wants (slot = chunk index)
+    void run_prefix_on_range(long long turn, long long k_end, long long lo, long long hi, int slot) {
+        range_lo = lo; range_hi = hi; mm_slot = slot;
+        const long long ne = (long long)bl->e.size();
+        run_turn_range(turn, 0, k_end);
+        flush(AP_NONE, 0, 0, 0, next_is_hist(k_end - 1, ne));
+        range_lo = 0; range_hi = -1; mm_slot = 0;
+    }
+    void run_turn_range(long long turn, long long k_begin, long long k_end) {       // maps only (no records)
+        for (long long k = k_begin; k < k_end && ok(); k++) {
+            const elg_element& e = bl->e[k];
+            const double s_here = std::fma((double)turn, bl->length, bl->s_design[k]);
+            HostOp op{};
+            switch (e.type) {
+                case ELG_DRIFT: op.type = OP_DRIFT; op.coef[0] = e.L; push(op); break;
+                case ELG_MATRIX:
+                    op.type = OP_MATRIX;
+                    std::memcpy(op.coef, e.R, 36 * sizeof(double));
+                    if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
+                    push(op);
+                    break;
+                case ELG_MATRIX2: case ELG_MATRIX3: push_higher_order(e); break;
+                case ELG_RFKICK:
+                    op.type = OP_RFKICK;
+                    op.coef[0] = e.V * b->inv_E; op.coef[1] = kTwoPi * e.f; op.coef[2] = e.phi;
+                    op.coef[3] = s_here; op.coef[4] = b->inv_bc;
+                    push(op);
+                    break;
+                default: break;
+            }
+        }
+    }
+
     bool next_is_hist(long long k, long long ne) const {
         return (k + 1 < ne) && (bl->e[k + 1].type == ELG_WAKE || bl->e[k + 1].type == ELG_HISTO || bl->e[k + 1].type == ELG_TRWAKE);
     }
@@ -910,6 +973,70 @@ extern "C" int32_t elg_track(elg_bunch* b, const elg_beamline* bl, int64_t n_tur
     Tracker t{b, bl, o};
     b->rec_count = 0;
     for (int64_t it = 0; it < n_turns && t.ok(); it++) {
+        t.run_turn(b->turn);
+        b->turn++;
+    }
+    t.flush(AP_NONE, 0, 0, 0, false);
+    if (t.ok()) t.flush_records();
+    if (o) o->n_records = t.rec_total;
+    if (t.ok() && o && (o->records || o->hist_out || o->V_out || o->window_out)) {
+        cudaError_t e = cudaStreamSynchronize(b->stream);
+        if (e != cudaSuccess) return fail(ELG_ECUDA, std::string("cudaStreamSynchronize: ") + cudaGetErrorString(e));
+    }
+    return t.rc;
+}
+
+// elg_bunch_upload + elg_track in one call, with the upload pipelined against the tracking: the bunch is cut into
+// n_chunks particle ranges, each range is copied on the library's own copy stream and, as soon as it has landed, the
+// leading per-particle maps of the first turn (everything in front of the first collective element, aperture or
+// record) run on it while the next ranges are still crossing PCIe.  Results are identical to upload followed by track.
+extern "C" int32_t elg_upload_and_track(elg_bunch* b, const elg_beamline* bl, const double* const h_coords[6],
+                                        const int64_t* h_ids, int64_t n_turns, elg_track_opts* o, int32_t n_chunks) {
+    if (!b || !bl || !h_coords || n_turns < 0) return fail(ELG_EINVAL, "elg_upload_and_track: bad arguments");
+    for (int c = 0; c < 6; c++) if (!h_coords[c]) return fail(ELG_EINVAL, "elg_upload_and_track: NULL coordinate array");
+    Tracker probe{b, bl, o};
+    const long long k_split = probe.map_prefix();
+    if (n_turns < 1 || k_split == 0 || n_chunks <= 1 || b->n0 < 4 * 3072) {       // nothing to overlap
+        int32_t rc = elg_bunch_upload(b, h_coords, h_ids);
+        return rc != ELG_OK ? rc : elg_track(b, bl, n_turns, o);
+    }
+    if (o) { o->n_records = 0; o->hist_written = 0; o->V_written = 0; o->window_written = 0; }
+    if (!b->copy_stream) {
+        ELG_CK(cudaStreamCreateWithFlags(&b->copy_stream, cudaStreamNonBlocking));
+        ELG_CK(cudaEventCreateWithFlags(&b->entry_ev, cudaEventDisableTiming));
+    }
+    if (n_chunks > 24) n_chunks = 24;                               // min/max partial slots (kMmPartials)
+    while ((int)b->chunk_ev.size() < n_chunks) {
+        cudaEvent_t e = nullptr;
+        ELG_CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        b->chunk_ev.push_back(e);
+    }
+    // the copies overwrite store 0: everything queued on the bunch's stream so far must be done with it
+    ELG_CK(cudaEventRecord(b->entry_ev, b->stream));
+    ELG_CK(cudaStreamWaitEvent(b->copy_stream, b->entry_ev, 0));
+    if (h_ids) ELG_CK(cudaMemcpyAsync(b->ids(0), h_ids, b->n0 * 8, cudaMemcpyHostToDevice, b->stream));
+    else {
+        iota_kernel<<<b->sms * 4, kBlock, 0, b->stream>>>(b->ids(0), b->n0);
+        g_launches++;
+        ELG_CK(cudaGetLastError());
+    }
+    { int32_t rc = elg_bunch_rewind(b); if (rc != ELG_OK) return rc; }
+    { int32_t rc = upload_tables(b, bl); if (rc != ELG_OK) return rc; }
+    Tracker t{b, bl, o};
+    b->rec_count = 0;
+    const long long per = align_up((b->n0 + n_chunks - 1) / n_chunks, 3072);     // multiple of every chain tile size
+    int slot = 0;
+    for (long long lo = 0; lo < b->n0 && t.ok(); lo += per, slot++) {
+        const long long hi = lo + per < b->n0 ? lo + per : b->n0;
+        for (int c = 0; c < 6; c++)
+            ELG_CK(cudaMemcpyAsync(b->coord(0, c) + lo, h_coords[c] + lo, (size_t)(hi - lo) * 8, cudaMemcpyHostToDevice, b->copy_stream));
+        ELG_CK(cudaEventRecord(b->chunk_ev[slot], b->copy_stream));
+        ELG_CK(cudaStreamWaitEvent(b->stream, b->chunk_ev[slot], 0));
+        t.run_prefix_on_range(b->turn, k_split, lo, hi, slot);
+    }
+    if (t.ok()) t.run_turn(b->turn, k_split);
+    b->turn++;
+    for (int64_t it = 1; it < n_turns && t.ok(); it++) {
         t.run_turn(b->turn);
         b->turn++;
     }

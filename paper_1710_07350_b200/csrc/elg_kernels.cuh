@@ -77,6 +77,8 @@ struct ChainCommon {
     const double* Vy;
     int t_nb;
     int t_interp;
+    long long range_lo;        // chain kernels work on particles [range_lo, min(range_hi, n_alive)); range_hi < 0: n_alive
+    long long range_hi;        // (pipelined upload: one range per chunk, elg_upload_and_track)
 };
 
 template <int MAXOPS>
@@ -374,13 +376,14 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
     constexpr int kSub = 2 * kBlock;            // particles per sub-tile
     constexpr int kTileP = kBlock * P;
     const ChainCommon& c = a.c;
-    const long long n = c.st->n_alive[c.cur];
-    const long long n_tiles = (n + kTileP - 1) / kTileP;
+    const long long n_all = c.st->n_alive[c.cur];
+    const long long n = (c.range_hi >= 0 && c.range_hi < n_all) ? c.range_hi : n_all;       // end of my range
+    const long long n_tiles = (n > c.range_lo) ? (n - c.range_lo + kTileP - 1) / kTileP : 0;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double mn = INFINITY, mx = -INFINITY;
 
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const long long t0 = tile * kTileP + (long long)threadIdx.x * 2;
+        const long long t0 = c.range_lo + tile * kTileP + (long long)threadIdx.x * 2;
         double v[P][6];
 #pragma unroll
         for (int h = 0; h < H; h++) {
@@ -481,15 +484,16 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
     double* s_coef = sm_long;                                    // [n_ops][42]
     double* s_tile = sm_long + MAXOPS * 42;                      // [6][H][kSub]: thread t owns doubles 2t, 2t+1 of each row
     const ChainCommon& c = a.c;
-    const long long n = c.st->n_alive[c.cur];
-    const long long n_tiles = (n + kTileL - 1) / kTileL;
+    const long long n_all = c.st->n_alive[c.cur];
+    const long long n = (c.range_hi >= 0 && c.range_hi < n_all) ? c.range_hi : n_all;       // end of my range
+    const long long n_tiles = (n > c.range_lo) ? (n - c.range_lo + kTileL - 1) / kTileL : 0;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double mn = INFINITY, mx = -INFINITY;
 
     for (int i = threadIdx.x; i < c.n_ops * 42; i += kBlock) s_coef[i] = a.coef[i / 42][i % 42];
 
     auto prefetch = [&](long long tile) {
-        const long long t0 = tile * kTileL + (long long)threadIdx.x * 2;
+        const long long t0 = c.range_lo + tile * kTileL + (long long)threadIdx.x * 2;
 #pragma unroll
         for (int h = 0; h < H; h++) {
             const long long i0 = t0 + (long long)h * kSub;
@@ -522,7 +526,7 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
 
         apply_ops_smem<MAXOPS, PL, LEVEL>(a, s_coef, v);
 
-        const long long t0 = tile * kTileL + (long long)threadIdx.x * 2;
+        const long long t0 = c.range_lo + tile * kTileL + (long long)threadIdx.x * 2;
 #pragma unroll
         for (int h = 0; h < H; h++) {
             const long long i0 = t0 + (long long)h * kSub;

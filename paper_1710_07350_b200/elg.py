@@ -31,6 +31,7 @@ EXPORTS = (
     "elg_beamline_load", "elg_beamline_destroy", "elg_beamline_n_elements", "elg_beamline_length",
     "elg_beamline_s_design", "elg_beamline_launches_per_turn", "elg_workspace_bytes",
     "elg_bunch_create", "elg_bunch_destroy", "elg_bunch_upload", "elg_bunch_rewind", "elg_track",
+    "elg_upload_and_track",
     "elg_moments", "elg_lost", "elg_n_alive", "elg_bunch_read", "elg_bunch_device_array",
     "elg_profile_enable", "elg_profile_read",
     "elg_dbg_histogram", "elg_dbg_wake_samples", "elg_dbg_convolve", "elg_dbg_kick",
@@ -109,6 +110,8 @@ def lib():
     L.elg_bunch_upload.argtypes = [vp, v6, _i64p]; L.elg_bunch_upload.restype = C.c_int32
     L.elg_bunch_rewind.argtypes = [vp]; L.elg_bunch_rewind.restype = C.c_int32
     L.elg_track.argtypes = [vp, vp, C.c_int64, C.POINTER(TrackOpts)]; L.elg_track.restype = C.c_int32
+    L.elg_upload_and_track.argtypes = [vp, vp, v6, _i64p, C.c_int64, C.POINTER(TrackOpts), C.c_int32]
+    L.elg_upload_and_track.restype = C.c_int32
     L.elg_moments.argtypes = [vp, _i64p, _dp, _dp]; L.elg_moments.restype = C.c_int32
     L.elg_lost.argtypes = [vp, _i64p, C.c_int64, _i64p, _i32p, _i32p, _dp]; L.elg_lost.restype = C.c_int32
     L.elg_n_alive.argtypes = [vp, _i64p]; L.elg_n_alive.restype = C.c_int32
@@ -301,9 +304,19 @@ class Bunch:
         self._stream.synchronize()
 
     # -- tracking ------------------------------------------------------------------------------
-    def track(self, bl: Beamline, n_turns: int = 1, moments_every: str = "none",
-              want_stage_outputs: bool = False, records: bool = True):
-        """elg_track.  Returns dict(records (k,43)[, hist, V, window])."""
+    def _host_ptrs(self, coords):
+        if hasattr(coords, "data_ptr"):          # torch CPU tensor (possibly pinned)
+            assert coords.dtype.is_floating_point and coords.element_size() == 8 and coords.is_contiguous()
+            base = coords.data_ptr()
+            ptrs = (_dp * 6)(*[C.cast(base + c * self.n0 * 8, _dp) for c in range(6)])
+        else:
+            coords = _f64(coords)
+            assert coords.shape == (6, self.n0)
+            ptrs = (_dp * 6)(*[_p(coords[c]) for c in range(6)])
+        self._keep = coords
+        return ptrs
+
+    def _opts(self, bl, n_turns, moments_every, want_stage_outputs, records):
         o = TrackOpts()
         o.moments_every = MOM[moments_every]
         n_rec = {"none": 0, "turn": n_turns, "element": n_turns * bl.n_elems}[moments_every]
@@ -322,7 +335,10 @@ class Bunch:
             o.hist_out, o.hist_capacity = _p(hist, _u32p), nh
             o.V_out, o.V_capacity = _p(V), nv
             o.window_out, o.window_capacity = _p(win), nw
-        _ck(lib().elg_track(self._h, bl._h, n_turns, C.byref(o)))
+        return o, rec, hist, V, win
+
+    @staticmethod
+    def _outputs(o, rec, hist, V, win, want_stage_outputs):
         out = {"n_records": o.n_records}
         if rec is not None:
             out["records"] = rec[: o.n_records]
@@ -331,6 +347,30 @@ class Bunch:
             out["V"] = V[: o.V_written]
             out["window"] = win[: o.window_written]
         return out
+
+    def track(self, bl: Beamline, n_turns: int = 1, moments_every: str = "none",
+              want_stage_outputs: bool = False, records: bool = True):
+        """elg_track.  Returns dict(records (k,43)[, hist, V, window])."""
+        o, rec, hist, V, win = self._opts(bl, n_turns, moments_every, want_stage_outputs, records)
+        _ck(lib().elg_track(self._h, bl._h, n_turns, C.byref(o)))
+        return self._outputs(o, rec, hist, V, win, want_stage_outputs)
+
+    def upload_and_track(self, coords, bl: Beamline, n_turns: int = 1, moments_every: str = "none",
+                         want_stage_outputs: bool = False, records: bool = True, n_chunks: int = 8, ids=None):
+        """elg_upload_and_track: upload from host memory pipelined against the first turn's leading maps."""
+        ptrs = self._host_ptrs(coords)
+        idp = None
+        if ids is not None:
+            ids = np.ascontiguousarray(ids, dtype=np.int64)
+            idp = _p(ids, _i64p)
+            self._keep_ids = ids
+        o, rec, hist, V, win = self._opts(bl, n_turns, moments_every, want_stage_outputs, records)
+        _ck(lib().elg_upload_and_track(self._h, bl._h, ptrs, idp, n_turns, C.byref(o), n_chunks))
+        if not (rec is not None or want_stage_outputs):
+            pinned = hasattr(coords, "is_pinned") and coords.is_pinned()
+            if not pinned:
+                self.synchronize()
+        return self._outputs(o, rec, hist, V, win, want_stage_outputs)
 
     # -- read-backs (synchronise) ----------------------------------------------------------------
     @property

@@ -526,6 +526,32 @@ def test_rfcw_composite(elg, elgo, n):
     assert np.array_equal(gid, oid) and rel_err(gv, ov) <= 1e-12
 
 
+@pytest.mark.parametrize("name,n,chunks", [("cfg3", 100_003, 5), ("cfg0", 50_001, 3), ("p6-rfcw", 40_000, 4), ("cfg2", 30_000, 7)])
+def test_upload_and_track_equals_upload_then_track(elg, name, n, chunks):
+    """elg_upload_and_track (upload pipelined against the leading maps, chunk by chunk) gives the same bits as
+    elg_bunch_upload + elg_track: coordinates, IDs, lost log, records, stage outputs."""
+    kw = {"n_turns": 3} if name == "cfg3" else {}
+    w = make_workload(name, n=n, **kw)
+    v0 = w.particles()
+    nt = min(w.n_turns, 3)
+    bl = elg.Beamline(w.elements, ring=w.ring)
+    a = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=bl)
+    oa = a.track(bl, nt, moments_every=w.moments_every, want_stage_outputs=True)
+    b = elg.Bunch(None, w.p0c_eV, w.charge_C, beamline=bl, n0=n)
+    ob = b.upload_and_track(v0, bl, nt, moments_every=w.moments_every, want_stage_outputs=True, n_chunks=chunks)
+    av, aid = a.read(); bv, bid = b.read()
+    assert np.array_equal(aid, bid) and np.array_equal(av, bv)
+    for k in ("hist", "V", "window"):
+        assert np.array_equal(oa[k], ob[k]), k
+    if "records" in oa:
+        assert np.array_equal(oa["records"], ob["records"])
+    for x, y in zip(a.lost(), b.lost()):
+        assert np.array_equal(x, y)
+    # and once more on the same bunch (copy stream and events are reused)
+    ob2 = b.upload_and_track(v0, bl, nt, moments_every=w.moments_every, want_stage_outputs=True, n_chunks=chunks)
+    assert np.array_equal(b.read()[0], av) and np.array_equal(ob2["V"], oa["V"])
+
+
 def test_track_in_two_calls_equals_one(elg, elgo):
     """Turn counter, RF reference and lost log carry across elg_track calls."""
     w = make_workload("cfg3", n=5000, n_matrices=10, n_turns=6)
