@@ -273,6 +273,26 @@ def test_compaction_cases(elg, elgo, case):
         assert nl == 0
 
 
+def test_compaction_randomized_sizes(elg, elgo):
+    """Many sizes around the tile (512) and row (blocks x 512) boundaries and random apertures: survivor IDs / order
+    and the lost log against the oracle's stable partition (the scan has no chained look-back: a block adds the
+    aggregates of one round-robin row to its own prefix, so row boundaries are the edge cases)."""
+    import torch
+    rows = 2 * torch.cuda.get_device_properties(0).multi_processor_count * 512
+    rng = np.random.default_rng(99)
+    sizes = [rows - 1, rows, rows + 1, 2 * rows + 513, 3 * rows - 511] + [int(x) for x in rng.integers(1, 2_000_000, 7)]
+    for n in sizes:
+        a = float(rng.choice([60e-6, 150e-6, 400e-6]))
+        v0 = np.zeros((6, n)); v0[0] = rng.normal(size=n) * 1e-4; v0[2] = rng.normal(size=n) * 1e-4
+        v0[5] = np.arange(n) * 1e-9
+        e = [{"type": "ECOL", "a": a, "b": 1.3 * a}]
+        ob = elgo.Bunch(v0, 1e9, 1e-9); ob.track(elgo.Beamline(e), 1)
+        gbl = elg.Beamline(e); gb = elg.Bunch(v0, 1e9, 1e-9, beamline=gbl); gb.track(gbl, 1)
+        ov, oid = ob.read(); gv, gid = gb.read()
+        assert np.array_equal(gid, oid) and np.array_equal(gv, ov), n
+        check_lost(ob, gb)
+
+
 def test_lost_capacity_truncates(elg, elgo):
     w = make_workload("cfg4", n=50_000)
     v0 = w.particles()
