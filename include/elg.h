@@ -43,7 +43,8 @@ enum { ELG_DRIFT = 1, ELG_MATRIX = 2, ELG_RFKICK = 3, ELG_RCOL = 4, ELG_ECOL = 5
 /* histogram window modes (G10) */
 enum { ELG_WIN_EXPLICIT = 0, ELG_WIN_AUTO_MINMAX = 1, ELG_WIN_AUTO_TABLE = 2 };
 /* wake kinds (G12) */
-enum { ELG_WAKE_RESONATOR = 0, ELG_WAKE_TABLE = 1, ELG_WAKE_RESONATOR_T = 2 /* transverse resonator, TRWAKE only */ };
+enum { ELG_WAKE_RESONATOR = 0, ELG_WAKE_TABLE = 1, ELG_WAKE_RESONATOR_T = 2 /* transverse resonator, TRWAKE only */,
+       ELG_WAKE_RESONATOR_REC = 3 /* the resonator of kind 0 evaluated by the O(nb) recurrence (G37), WAKE only */ };
 /* when elg_track records moments (G26) */
 enum { ELG_MOM_NONE = 0, ELG_MOM_TURN = 1, ELG_MOM_ELEMENT = 2 };
 

@@ -20,6 +20,7 @@
  *   elgo_window/histogram  pinned - hand-placed bins, edge rule, sum of counts
  *   elgo_wake_samples pinned  - beam-loading theorem, independent evaluation
  *   elgo_convolve     pinned  - brute-force double loop, numpy.convolve, continuous closed form
+ *   elgo_convolve_resonator  pinned - equals elgo_convolve of elgo_wake_samples (<= 1e-12 of the maximum)
  *   elgo_kick         pinned  - bin-centre / midpoint / clamped cases
  *   elgo_dipole_histogram, elgo_convolve_d, elgo_tkick (TRWAKE)  pinned - plain weighted sums, brute-force
  *                               convolution, two-particle closed form, zero offset => zero kick, linearity
@@ -47,7 +48,8 @@ enum { ELGO_DRIFT = 1, ELGO_MATRIX = 2, ELGO_RFKICK = 3, ELGO_RCOL = 4, ELGO_ECO
 /* histogram window modes (G10) */
 enum { ELGO_WIN_EXPLICIT = 0, ELGO_WIN_AUTO_MINMAX = 1, ELGO_WIN_AUTO_TABLE = 2 };
 /* wake kinds (G12) */
-enum { ELGO_WAKE_RESONATOR = 0, ELGO_WAKE_TABLE = 1, ELGO_WAKE_RESONATOR_T = 2 /* transverse, G34 */ };
+enum { ELGO_WAKE_RESONATOR = 0, ELGO_WAKE_TABLE = 1, ELGO_WAKE_RESONATOR_T = 2 /* transverse, G34 */,
+       ELGO_WAKE_RESONATOR_REC = 3 /* longitudinal resonator by the O(nb) two-term recurrence, G37 */ };
 /* when elgo_track records moments (G26) */
 enum { ELGO_MOM_NONE = 0, ELGO_MOM_TURN = 1, ELGO_MOM_ELEMENT = 2 };
 
@@ -115,6 +117,9 @@ int64_t elgo_histogram(const double* s, int64_t n, double inv_bc, double t_lo, d
 int32_t elgo_wake_samples(int32_t kind, int32_t nb, double dt, double f, double Q, double Rs,
                           const double* table, int64_t n_table, double dt_table, double* W);
 void   elgo_convolve(const uint32_t* counts, const double* W, int32_t nb, double q, double* Vout);
+/* the same V for the resonator wake of G12 by the O(nb) complex recurrence (G37), no W array */
+int32_t elgo_convolve_resonator(const uint32_t* counts, int32_t nb, double q, double dt, double f, double Q, double Rs,
+                                double* Vout);
 /* TRWAKE (G32-G34): counts[nb] and the per-bin dipole sums Dx[nb], Dy[nb] = sum of x, y of the particles in the
    bin, accumulated exactly in two 64-bit fixed-point words (G33), hence independent of the summation order */
 int64_t elgo_dipole_histogram(const double* s, const double* x, const double* y, int64_t n, double inv_bc, double t_lo,

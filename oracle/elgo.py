@@ -27,7 +27,7 @@ _LIB = os.path.join(_HERE, "libelgo.so")
 OK, EINVAL, ENOMEM, ESTATE, ECAPACITY = 0, -1, -2, -4, -5
 DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2, TRWAKE, MATRIX3 = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 WIN = {"EXPLICIT": 0, "AUTO_MINMAX": 1, "AUTO_TABLE": 2}
-WAKEKIND = {"RESONATOR": 0, "TABLE": 1, "RESONATOR_T": 2}
+WAKEKIND = {"RESONATOR": 0, "TABLE": 1, "RESONATOR_T": 2, "RESONATOR_REC": 3}
 MOM = {"none": 0, "turn": 1, "element": 2}
 ELECTRON_MC2_EV = 0.51099895e6
 
@@ -108,6 +108,8 @@ def lib():
         L.elgo_kick.argtypes = [_dp, _dp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32,
                                 _dp, C.c_double, C.c_int32]
         L.elgo_kick.restype = None
+        L.elgo_convolve_resonator.argtypes = [_u32p, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, _dp]
+        L.elgo_convolve_resonator.restype = C.c_int32
         L.elgo_dipole_histogram.argtypes = [_dp, _dp, _dp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32,
                                             _u32p, _dp, _dp]
         L.elgo_dipole_histogram.restype = C.c_int64
@@ -251,6 +253,15 @@ def convolve(counts: np.ndarray, W: np.ndarray, q: float) -> np.ndarray:
     return V
 
 
+def convolve_resonator(counts, q: float, dt: float, f: float, Q: float, Rs: float) -> np.ndarray:
+    counts = np.ascontiguousarray(counts, dtype=np.uint32)
+    V = np.empty(counts.shape[0], dtype=np.float64)
+    rc = lib().elgo_convolve_resonator(_p(counts, _u32p), counts.shape[0], q, dt, f, Q, Rs, _p(V))
+    if rc != OK:
+        raise ValueError(f"elgo_convolve_resonator rc={rc}")
+    return V
+
+
 def kick(s: np.ndarray, delta: np.ndarray, inv_bc, t_lo, inv_dt, nb, V, inv_E, interp=True) -> None:
     V = _f64(V)
     lib().elgo_kick(_p(s), _p(delta), s.shape[0], inv_bc, t_lo, inv_dt, nb, _p(V), inv_E, 1 if interp else 0)
@@ -336,7 +347,7 @@ def _elements_to_c(elements):
             if t != "HISTO":
                 e.wake = WAKEKIND[d["wake"]]
                 e.interp = 1 if d.get("interp", True) else 0
-                if d["wake"] in ("RESONATOR", "RESONATOR_T"):
+                if d["wake"] in ("RESONATOR", "RESONATOR_T", "RESONATOR_REC"):
                     e.f, e.Q, e.Rs = float(d["f"]), float(d["Q"]), float(d["Rs"])
                 else:
                     tb = _f64(d["table"]); keep.append(tb)

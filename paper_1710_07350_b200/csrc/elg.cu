@@ -298,7 +298,8 @@ extern "C" int32_t elg_beamline_load(elg_beamline** out, const elg_element* elem
                     rc.ratio = 0.0;
                     bl->res[k] = rc;
                 } else if (e.type == ELG_WAKE || e.type == ELG_TRWAKE) {
-                    if (e.wake == ELG_WAKE_RESONATOR) {
+                    if (e.type == ELG_TRWAKE && e.wake == ELG_WAKE_RESONATOR_REC) { why = "TRWAKE: wake kind must be RESONATOR_T or TABLE"; break; }
+                    if (e.wake == ELG_WAKE_RESONATOR || e.wake == ELG_WAKE_RESONATOR_REC) {
                         if (!(e.Q > 0.5) || !(e.f > 0.0) || !std::isfinite(e.Rs)) { why = "resonator: Q > 1/2, f > 0, finite Rs required"; break; }
                         // G12, same expressions as the definition, evaluated once here
                         const double wr = kTwoPi * e.f;
@@ -782,8 +783,21 @@ struct Tracker {
 
     void wake_part(long long k) {                                     // samples, convolution, queue the kick
         const elg_element& e = bl->e[k];
-        count(); count();
-        if (b) {
+        count();
+        if (e.wake != ELG_WAKE_RESONATOR_REC) count();
+        if (b && e.wake == ELG_WAKE_RESONATOR_REC) {                 // O(nb) recurrence: no samples, no convolution (G37)
+            const ResConst& r = bl->res[k];
+            ConvRecArgs cr;
+            cr.counts = b->counts; cr.st = b->st; cr.nb = e.nb; cr.q = b->q_macro;
+            cr.kloss = r.kloss; cr.alpha = r.alpha; cr.wbar = r.wbar; cr.ratio = r.ratio; cr.V = b->V;
+            {
+                ProfScope ps(b, ELG_K_CONV);
+                conv_rec_kernel<<<1, kBlock, 0, b->stream>>>(cr);
+            }
+            check(cudaGetLastError(), "conv_rec_kernel launch");
+            if (o && o->V_out && o->V_written + e.nb <= o->V_capacity)
+                check(cudaMemcpyAsync(o->V_out + o->V_written, b->V, (size_t)e.nb * 8, cudaMemcpyDeviceToHost, b->stream), "V D2H");
+        } else if (b) {
             launch_samples(k);
             ConvArgs<unsigned int> cv;
             cv.counts = b->counts; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro; cv.V = b->V;

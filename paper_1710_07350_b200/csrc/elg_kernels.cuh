@@ -1155,6 +1155,67 @@ __global__ void __launch_bounds__(kBlock) conv_kernel(const ConvArgs<T> a) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// conv_rec_kernel (G37): the resonator wake voltage in O(nb) instead of the O(nb^2) convolution.
+// W_k = Re[B z^k] with z = exp((-alpha + i wbar) dt), so S_{i+1} = z (S_i + c_i), V_i = q (c_i k_loss + Re[B S_i]).
+// One block: every thread runs the recurrence over its own contiguous segment from S = 0, thread 0 chains the
+// 256 segment ends with z^L, then every thread repeats its segment from its carry-in and writes V.  Fixed
+// decomposition, hence deterministic; it differs from the sequential recurrence only by rounding (<< 1e-10).
+// ---------------------------------------------------------------------------------------------------
+struct ConvRecArgs {
+    const unsigned int* counts;
+    const DevState* st;    // dt = win[1]
+    int nb;
+    double q;
+    double kloss, alpha, wbar, ratio;
+    double* V;
+};
+
+__global__ void __launch_bounds__(kBlock) conv_rec_kernel(const ConvRecArgs a) {
+    __shared__ double s_er[kBlock], s_ei[kBlock];
+    const double dt = a.st->win[1];
+    const int L = (a.nb + kBlock - 1) / kBlock;
+    const int lo = threadIdx.x * L, hi = (lo + L < a.nb) ? lo + L : a.nb;
+    const double damp = exp(-a.alpha * dt);
+    const double zr = damp * cos(a.wbar * dt), zi = damp * sin(a.wbar * dt);
+    double Sr = 0.0, Si = 0.0;
+    for (int i = lo; i < hi; i++) {
+        const double tr = Sr + (double)a.counts[i], ti = Si;
+        Sr = fma(zr, tr, -(zi * ti));
+        Si = fma(zr, ti, zi * tr);
+    }
+    // a segment shorter than L (the tail) still has to advance its end state by the missing steps for the chaining
+    for (int i = (hi > lo ? hi : lo); i < lo + L; i++) {
+        const double tr = Sr, ti = Si;
+        Sr = fma(zr, tr, -(zi * ti));
+        Si = fma(zr, ti, zi * tr);
+    }
+    s_er[threadIdx.x] = Sr; s_ei[threadIdx.x] = Si;
+    __syncthreads();
+    if (threadIdx.x == 0) {                                      // carry-in of segment t: C_{t+1} = z^L C_t + E_t
+        const double dL = exp(-a.alpha * dt * (double)L);
+        const double pr = dL * cos(a.wbar * dt * (double)L), pi = dL * sin(a.wbar * dt * (double)L);
+        double Cr = 0.0, Ci = 0.0;
+        for (int t = 0; t < kBlock; t++) {
+            const double er = s_er[t], ei = s_ei[t];
+            s_er[t] = Cr; s_ei[t] = Ci;
+            const double nr = fma(pr, Cr, -(pi * Ci)) + er;
+            const double ni = fma(pr, Ci, pi * Cr) + ei;
+            Cr = nr; Ci = ni;
+        }
+    }
+    __syncthreads();
+    Sr = s_er[threadIdx.x]; Si = s_ei[threadIdx.x];
+    const double Br = 2.0 * a.kloss, Bi = 2.0 * a.kloss * a.ratio;
+    for (int i = lo; i < hi; i++) {
+        const double c = (double)a.counts[i];
+        a.V[i] = a.q * fma(c, a.kloss, fma(Br, Sr, -(Bi * Si)));
+        const double tr = Sr + c, ti = Si;
+        Sr = fma(zr, tr, -(zi * ti));
+        Si = fma(zr, ti, zi * tr);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // kick_kernel: test hook for a12 on caller-supplied arrays (the tracking path applies the kick as the
 // first op of the next fused run, OP_KICK above; same arithmetic).
 // ---------------------------------------------------------------------------------------------------

@@ -17,7 +17,7 @@ from .build import LIB, build
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ECAPACITY = 0, -1, -2, -3, -4, -5
 DRIFT, MATRIX, RFKICK, RCOL, ECOL, WAKE, HISTO, MATRIX2, TRWAKE, MATRIX3 = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 WIN = {"EXPLICIT": 0, "AUTO_MINMAX": 1, "AUTO_TABLE": 2}
-WAKEKIND = {"RESONATOR": 0, "TABLE": 1, "RESONATOR_T": 2}
+WAKEKIND = {"RESONATOR": 0, "TABLE": 1, "RESONATOR_T": 2, "RESONATOR_REC": 3}
 MOM = {"none": 0, "turn": 1, "element": 2}
 ELECTRON_MC2_EV = 0.51099895e6
 
@@ -193,7 +193,7 @@ def _elements_to_c(elements):
             if t != "HISTO":
                 e.wake = WAKEKIND[d["wake"]]
                 e.interp = 1 if d.get("interp", True) else 0
-                if d["wake"] in ("RESONATOR", "RESONATOR_T"):
+                if d["wake"] in ("RESONATOR", "RESONATOR_T", "RESONATOR_REC"):
                     e.f, e.Q, e.Rs = float(d["f"]), float(d["Q"]), float(d["Rs"])
                 else:
                     tb = _f64(d["table"]); keep.append(tb)

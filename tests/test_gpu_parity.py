@@ -367,6 +367,28 @@ def test_wake_samples_and_convolution_stage(elg, elgo):
 
 
 # ------------------------------------------------------------------------------------ (v) kick
+@pytest.mark.parametrize("nb,Q", [(512, 1.0), (1000, 1e4), (8192, 30.0), (70_001, 200.0)])
+def test_recursive_resonator_wake(elg, elgo, nb, Q):
+    """WAKE with wake = RESONATOR_REC (G37): V from the blocked O(nb) recurrence against the oracle's sequential one
+    and against the direct convolution; histogram and window bit-identical, delta to 1e-12."""
+    w = make_workload("cfg0", n=120_001)
+    e = dict(w.elements[3]); e.update(nb=nb, Q=Q, wake="RESONATOR_REC")
+    elems = w.elements[:3] + [e, {"type": "DRIFT", "L": 0.5}]
+    v0 = w.particles()
+    ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
+    oo = ob.track(elgo.Beamline(elems), 1, want_stage_outputs=True)
+    gbl = elg.Beamline(elems); gb = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=gbl)
+    go = gb.track(gbl, 1, want_stage_outputs=True)
+    assert np.array_equal(go["window"], oo["window"]) and np.array_equal(go["hist"], oo["hist"])
+    m = np.max(np.abs(oo["V"]))
+    assert np.max(np.abs(go["V"] - oo["V"])) <= 1e-10 * m
+    W = elgo.wake_samples(0, nb, oo["window"][0, 1], f=e["f"], Q=Q, Rs=e["Rs"])
+    Vd = elgo.convolve(oo["hist"], W, w.charge_C / w.n0)
+    assert np.max(np.abs(go["V"] - Vd)) <= 1e-10 * m
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid) and np.array_equal(gv[:5], ov[:5]) and rel_err(gv, ov) <= 1e-12
+
+
 def test_kick_stage(elg, elgo):
     w = make_workload("cfg0", n=150_001)
     v = w.particles()

@@ -806,3 +806,18 @@ def test_fiducial_is_the_exact_mean_and_makes_kicks_delay_invariant(elgo):
     # with the fiducial the mean phase is phi exactly: the mean kick is A sin(phi) <cos> ~ A sin(phi)
     A = 1e6 * elgo.inv_E(elgo.beta0(1e9), 1e9)
     assert abs(a.mean() / (A * math.sin(0.3)) - 1.0) < 2e-3
+
+
+# ------------------------------------------------------------------------------------ recursive resonator (G37)
+def test_convolve_resonator_equals_direct_convolution(elgo):
+    """The O(nb) recurrence gives the V of elgo_convolve(elgo_wake_samples(resonator)) for damped (Q = 1), ringing
+    (Q = 1e4) and long (8192-bin) cases; a single bin reproduces the wake samples themselves."""
+    rng = np.random.default_rng(41)
+    for nb, dt, f, Q, Rs in [(512, 2e-14, 1e9, 1.0, 1e3), (1024, 1.2e-14, 1.3e9, 1e4, 1e3), (8192, 5e-14, 3e9, 50.0, 2e3)]:
+        c = rng.integers(0, 200_000, nb).astype(np.uint32)
+        W = elgo.wake_samples(0, nb, dt, f=f, Q=Q, Rs=Rs)
+        V = elgo.convolve(c, W, 1e-17)
+        Vr = elgo.convolve_resonator(c, 1e-17, dt, f, Q, Rs)
+        assert np.max(np.abs(V - Vr)) <= 1e-12 * np.max(np.abs(V))
+        one = np.zeros(nb, dtype=np.uint32); one[0] = 1
+        assert np.allclose(elgo.convolve_resonator(one, 1.0, dt, f, Q, Rs), W, rtol=1e-12, atol=1e-12 * np.max(np.abs(W)))
