@@ -135,3 +135,50 @@ def test_compaction_at_1e8(elg, elgo):
     lpos = np.searchsorted(lid, olid)
     assert np.array_equal(lid[lpos], olid), "oracle lost are CUDA lost"
     assert np.array_equal(lco[lpos], olco)
+
+
+def test_rfcw_cavity_at_1e8(elg, elgo):
+    """One RFCW-style cavity (MATRIX + RFKICK + WAKE + TRWAKE sharing one dipole-histogram pass) on 1e8 particles:
+    window, counts and the exact dipole sums bit-identical to the oracle's sequential stage functions fed the CUDA
+    coordinates; voltages to 1e-10; the three kicks on sampled particles."""
+    import torch
+    w = make_workload("p6-rfcw", n=N_FULL, n_cavities=1)
+    h = _pinned_particles(w, N_FULL)
+    v0 = h.numpy()
+    gbl = elg.Beamline(w.elements)
+    gb = elg.Bunch(None, w.p0c_eV, w.charge_C, beamline=gbl, n0=N_FULL, lost_capacity=0)
+    go = gb.upload_and_track(h, gbl, 1, want_stage_outputs=True, n_chunks=8)
+    off, mat, rf, wake, trw = w.elements
+    nb = wake["nb"]
+    b0 = elgo.beta0(w.p0c_eV); inv_bc = elgo.inv_bc(b0); inv_E = elgo.inv_E(b0, w.p0c_eV)
+    q = w.charge_C / N_FULL
+
+    # sampled particles through the per-particle maps (offset MATRIX, MATRIX, RFKICK)
+    idx = _sample(N_FULL, 9)
+    ob = elgo.Bunch(np.ascontiguousarray(v0[:, idx]), w.p0c_eV, w.charge_C)
+    ob.track(elgo.Beamline([off, mat, rf]), 1)
+    ov, _ = ob.read()
+    t_idx = torch.as_tensor(idx, device="cuda")
+    gv = np.stack([gb.device_array(c)[t_idx].cpu().numpy() for c in range(6)])
+    assert np.array_equal(gv[[0, 2, 4]], ov[[0, 2, 4]])            # x, y, s are not touched by the kicks
+
+    s_full = gb.device_array(4)[:N_FULL].cpu().numpy()
+    x_full = gb.device_array(0)[:N_FULL].cpu().numpy()
+    y_full = gb.device_array(2)[:N_FULL].cpu().numpy()
+    t_lo, dt, inv_dt = elgo.window(s_full, inv_bc, 1, nb)
+    assert np.array_equal(go["window"][0], [t_lo, dt, inv_dt]) and np.array_equal(go["window"][1], go["window"][0])
+    counts, Dx, Dy, binned = elgo.dipole_histogram(s_full, x_full, y_full, inv_bc, t_lo, inv_dt, nb)
+    assert binned == N_FULL and np.array_equal(go["hist"][:nb], counts) and np.array_equal(go["hist"][nb:], counts)
+    V = elgo.convolve(counts, elgo.wake_samples(0, nb, dt, f=wake["f"], Q=wake["Q"], Rs=wake["Rs"]), q)
+    Wt = elgo.wake_samples(2, nb, dt, f=trw["f"], Q=trw["Q"], Rs=trw["Rs"])
+    Vx = elgo.convolve_d(Dx, Wt, q); Vy = elgo.convolve_d(Dy, Wt, q)
+    Vg = go["V"]
+    assert np.array_equal(Vg[nb:2 * nb], Dx) and np.array_equal(Vg[2 * nb:3 * nb], Dy), "exact dipole sums"
+    for got, ref in ((Vg[:nb], V), (Vg[3 * nb:4 * nb], Vx), (Vg[4 * nb:5 * nb], Vy)):
+        assert np.max(np.abs(got - ref)) <= 1e-10 * np.max(np.abs(ref))
+
+    d_exp = ov[5].copy(); xp_exp = ov[1].copy(); yp_exp = ov[3].copy()
+    elgo.kick(ov[4], d_exp, inv_bc, t_lo, inv_dt, nb, V, inv_E, True)
+    elgo.tkick(ov[4], xp_exp, yp_exp, inv_bc, t_lo, inv_dt, nb, Vx, Vy, inv_E, True)
+    for c, ref in ((5, d_exp), (1, xp_exp), (3, yp_exp)):
+        assert np.max(np.abs(gv[c] - ref) / np.maximum(np.abs(ref), np.std(ref))) <= 1e-12
