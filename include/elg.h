@@ -5,9 +5,10 @@
  * Citations: "PAPER.md:NN" = line of the paper text; "Gk" = reading k in DESIGN.md ("Readings").
  *
  * Problem statement: a bunch of particles traverses a succession of elements.  Per-particle
- * element maps, particle loss, a longitudinal wake built from a
- * histogram and an array convolution and beam-moment reductions (PAPER.md:123-131,
- * 145) are all computed by CUDA kernels of this library; nothing is computed on the host and there is no
+ * element maps (first- to third-order transport maps), particle loss
+ * (PAPER.md:139-141), longitudinal and transverse wakes built from a histogram and an array convolution
+ * and beam-moment reductions are all computed by CUDA kernels
+ * of this library; nothing is computed on the host and there is no
  * CPU fallback: every compute call fails with ELG_ECUDA when no device is usable.
  *
  * Conventions
@@ -107,9 +108,9 @@ typedef struct elg_beamline elg_beamline;
  *             (population central moments over live particles, G20); taken after every turn
  *             (ELG_MOM_TURN) or after every element (ELG_MOM_ELEMENT, G26).  n_records returns the number
  *             of records taken (may exceed the capacity; the excess is dropped).
- *   hist_out / V_out / window_out : per-stage outputs of the successive WAKE/HISTO executions (counts
- *             uint32[nb]; V double[nb] for WAKE only; window = t_lo, dt, 1/dt), used by the stage-by-stage
- *             parity protocol; *_written return the totals (in entries / triples).
+ *   hist_out / V_out / window_out : per-stage outputs of the successive WAKE / HISTO / TRWAKE executions (counts
+ *             uint32[nb]; V double[nb] for a WAKE, Dx, Dy, Vx, Vy (4 nb doubles) for a TRWAKE; window = t_lo, dt,
+ *             1/dt), used by the stage-by-stage parity protocol; *_written return the totals (in entries / triples).
  */
 typedef struct {
     int32_t moments_every;
