@@ -594,6 +594,38 @@ def test_upload_and_track_equals_upload_then_track(elg, name, n, chunks):
     assert np.array_equal(b.read()[0], av) and np.array_equal(ob2["V"], oa["V"])
 
 
+def test_more_records_than_the_device_ring(elg, elgo):
+    """3 000 per-element records in one call: the 2 048-record device ring is drained to the host mid-run."""
+    ring = _long_line(23, {})[:6]
+    v0 = make_workload("cfg0", n=3001).particles()
+    ob = elgo.Bunch(v0, 1e9, 1e-9)
+    oo = ob.track(elgo.Beamline(ring, ring=True), 500, moments_every="element")
+    gbl = elg.Beamline(ring, ring=True); gb = elg.Bunch(v0, 1e9, 1e-9, beamline=gbl)
+    go = gb.track(gbl, 500, moments_every="element")
+    assert go["records"].shape == oo["records"].shape == (3000, 43)
+    check_records(go, oo)
+    assert np.array_equal(gb.read()[0], ob.read()[0])
+
+
+def test_empty_bunch_and_everything_lost(elg, elgo):
+    """G28: n = 0 from the start, and a bunch that loses every particle half way: later elements are no-ops,
+    histograms are zero, moment records are zero, elg_moments reports ELG_ESTATE."""
+    w = make_workload("cfg0", n=2000)
+    elems = [w.elements[0], {"type": "RCOL", "ax": 1e-9, "ay": 1e-9}] + w.elements[1:]
+    for v0 in (w.particles(), np.zeros((6, 0))):
+        ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
+        oo = ob.track(elgo.Beamline(elems), 1, moments_every="turn", want_stage_outputs=True)
+        gbl = elg.Beamline(elems); gb = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=gbl)
+        go = gb.track(gbl, 1, moments_every="turn", want_stage_outputs=True)
+        assert gb.n_alive == ob.n_alive == 0
+        assert np.array_equal(go["hist"], oo["hist"]) and not go["hist"].any()
+        assert np.array_equal(go["records"], oo["records"]) and not go["records"].any()
+        check_lost(ob, gb)
+        with pytest.raises(elg.ElgError) as ei:
+            gb.moments()
+        assert ei.value.code == elg.ESTATE
+
+
 def test_track_in_two_calls_equals_one(elg, elgo):
     """Turn counter, RF reference and lost log carry across elg_track calls."""
     w = make_workload("cfg3", n=5000, n_matrices=10, n_turns=6)
