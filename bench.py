@@ -411,8 +411,9 @@ def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
         # NEXT row f1: two dipole histograms (s, x, y: 24 B) + one plain (8 B) = 56 B over 3 launches
         ("p5-trwake", "none", {"hist": 56.0 / 3.0}),
     ]
+    cases.insert(2, ("p2-chain-rcol@10%", "none", {"chain_compact": 112.0}))     # 0.6 % and ~10 % loss
     for name, mom, bytes_pp in cases:
-        w = make_workload(name, n=n0)
+        w = make_workload("p2-chain-rcol", n=n0, half_width=197e-6) if name.endswith("@10%") else make_workload(name, n=n0)
         bl = elg.Beamline(w.elements, ring=False)
         for _ in range(3):
             restore(); gb.track(bl, 1, moments_every=mom, records=False)
