@@ -101,7 +101,7 @@ struct elg_bunch {
     std::map<int, int> hist_grids;                      // hist_kernel grid per shared-memory size
     std::map<const void*, int> grids;                   // persistent grid size per chain kernel instantiation
     int force_p = 0;                                    // ELG_CHAIN_P = 2 | 4 overrides the planner's choice
-    int grid_hist = 0, grid_mom = 0, grid_dipole = 0;
+    int grid_mom = 0, grid_dipole = 0;
     int hist_aggregate = 0;
     // pipelined upload (elg_upload_and_track): the library's own copy stream and one event per chunk
     cudaStream_t copy_stream = nullptr;
@@ -404,7 +404,6 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     int32_t rc = ELG_OK;
     if (rc == ELG_OK) rc = long_setup_once();
     if (rc == ELG_OK) rc = hist_setup_once();
-    if (rc == ELG_OK) rc = grid_for(hist_kernel, sms, kHistSmemBins * 4, kBlock, &b->grid_hist);
     if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, kBlock, &b->grid_mom);
     if (rc == ELG_OK) rc = grid_for(dipole_hist_kernel, sms, kDipoleSmemBins * 36, kBlock, &b->grid_dipole);
     if (rc != ELG_OK) { delete b; return rc; }
