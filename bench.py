@@ -500,6 +500,28 @@ def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
                     "paper_ms": {"V100": paper[0], "K20c": paper[1], "i7-3770K 1 core": paper[2]}})
     del small
 
+    # Flagged option, reported separately: zero-pattern specialisation of the cfg3 matrices (drift x thin
+    # quadrupole: 20 of 36 FMAs).  NOT the measured configuration: the headline applies every matrix densely.
+    if w_main.ring and any(e["type"] == "MATRIX" for e in w_main.elements):
+        bl = elg.Beamline(w_main.elements, ring=True)
+        restore()
+        gb.sparse_matrices = True
+        for _ in range(2):
+            gb.track(bl, 1, moments_every=w_main.moments_every, records=False)
+        gb.synchronize()
+        ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(3):
+            gb.track(bl, 1, moments_every=w_main.moments_every, records=False)
+        ev1.record(stream)
+        torch.cuda.synchronize(dev)
+        gb.sparse_matrices = False
+        ms = ev0.elapsed_time(ev1) / 3
+        out.append({"workload": w_main.name + " + ELG_TRACK_SPARSE_MATRICES", "kernel": "whole turn", "ms_per_turn": ms,
+                    "value": float(n0) * w_main.n_pass_elements / (ms * 1e-3) / 1e6, "unit": UNIT,
+                    "note": "flagged option (zero-pattern specialisation), reported separately from the dense headline"})
+        restore()
+
     # fp64-bound probe of the NEXT row: second-order maps in the long-run kernel
     w = make_workload("p4-second-order", n=n0, n_cells=20)
     bl = elg.Beamline(w.elements, ring=True)

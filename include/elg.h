@@ -112,9 +112,16 @@ typedef struct elg_beamline elg_beamline;
  *             uint32[nb]; V double[nb] for a WAKE, Dx, Dy, Vx, Vy (4 nb doubles) for a TRWAKE; window = t_lo, dt,
  *             1/dt), used by the stage-by-stage parity protocol; *_written return the totals (in entries / triples).
  */
+/* elg_track_opts.flags.  ELG_TRACK_SPARSE_MATRICES: a MATRIX whose entries outside the zero pattern of an uncoupled
+ * element (rows x, x': columns x, x', delta; rows y, y': columns y, y', delta; row s: all; row delta: columns s, delta) are
+ * exactly zero is applied with the 20 FMAs of that pattern instead of 36.  For finite coordinates the result equals
+ * the dense one (up to the sign of a zero); NaN / inf coordinates do not propagate through the skipped terms.  Off by
+ * default: the measured configuration applies every matrix densely. */
+enum { ELG_TRACK_SPARSE_MATRICES = 1 };
+
 typedef struct {
     int32_t moments_every;
-    int32_t reserved;
+    int32_t flags;               /* ELG_TRACK_* bits, 0 = none */
     double* records;
     int64_t capacity_records;
     int64_t n_records;

@@ -46,6 +46,7 @@ inline long long align_up(long long x, long long a) { return (x + a - 1) / a * a
 struct HostOp {
     uint8_t type;
     double coef[42];
+    double dense[42];      // OP_MATRIX_UNC only: the dense coefficients, in case the run cannot use the pattern kernel
 };
 
 struct ResConst { double kloss, alpha, wbar, ratio; };
@@ -221,6 +222,8 @@ int32_t long_setup_once() {
                                     chain_long_smem_bytes<kMaxOpsLarge, 1>()));
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     chain_long_smem_bytes<kMaxOpsLarge, 2>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    chain_long_smem_bytes<kMaxOpsLarge, 3>()));
         done = true;
     }
     return ELG_OK;
@@ -583,7 +586,7 @@ struct Tracker {
         for (const HostOp& op : pending) {
             switch (op.type) {
                 case OP_DRIFT: rmask |= 0x1F; wmask |= 0x15; break;           // reads x x' y y' s, writes x y s
-                case OP_MATRIX: case OP_MATRIX2: case OP_MATRIX3: rmask |= 0x3F; wmask |= 0x3F; break;
+                case OP_MATRIX: case OP_MATRIX2: case OP_MATRIX3: case OP_MATRIX_UNC: rmask |= 0x3F; wmask |= 0x3F; break;
                 case OP_RFKICK: case OP_KICK: rmask |= 0x30; wmask |= 0x20; break;   // reads s delta, writes delta
                 case OP_TKICK: rmask |= 0x1A; wmask |= 0x0A; break;                  // reads x' y' s, writes x' y'
             }
@@ -592,24 +595,33 @@ struct Tracker {
         // the long-run kernel (coefficients in shared memory, 6 particles per thread) also takes the short runs that
         // are already fp64-bound: from 5 matrices on it beats the parameter-bank kernel (bench.py p3 sweep)
         int n_mat_run = 0;
-        for (const HostOp& op : pending) n_mat_run += (op.type == OP_MATRIX) + 4 * (op.type == OP_MATRIX2);
+        for (const HostOp& op : pending) n_mat_run += (op.type == OP_MATRIX || op.type == OP_MATRIX_UNC) + 4 * (op.type == OP_MATRIX2);
         const bool large = pending.size() > (size_t)kMaxOpsSmall || (ap_type == AP_NONE && n_mat_run >= kMatricesForLong);
         const bool compact = ap_type != AP_NONE;
         // particles per thread: 2 while the run is HBM-bound; 4 once it holds enough MATRIX maps for the
         // coefficient fetches (one per 2 particles) to matter
         int n_mat = 0;
-        for (const HostOp& op : pending) n_mat += (op.type == OP_MATRIX) + 4 * (op.type == OP_MATRIX2) + 12 * (op.type == OP_MATRIX3);
+        for (const HostOp& op : pending) n_mat += (op.type == OP_MATRIX || op.type == OP_MATRIX_UNC) + 4 * (op.type == OP_MATRIX2) + 12 * (op.type == OP_MATRIX3);
         bool p4 = n_mat >= kMatricesForP4;
         if (b && b->force_p == 2) p4 = false;
         if (b && b->force_p == 4) p4 = true;
         int ext = 0;                                                  // rarely used maps: higher EXT instantiations
+        bool has_unc = false;
         for (const HostOp& op : pending) {
             if (op.type == OP_MATRIX2 || op.type == OP_TKICK) ext = ext < 1 ? 1 : ext;
             if (op.type == OP_MATRIX3) ext = 2;
+            has_unc = has_unc || op.type == OP_MATRIX_UNC;
+        }
+        if (has_unc) {
+            if (large && ext == 0) ext = 3;                           // the pattern level of the long-run kernel
+            else                                                      // short or mixed run: apply them densely
+                for (HostOp& op : pending)
+                    if (op.type == OP_MATRIX_UNC) { op.type = OP_MATRIX; std::memcpy(op.coef, op.dense, sizeof op.coef); }
         }
 #define ELG_LAUNCH(M, C, PP, E) launch_chain<M, C, PP, E>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
         if (large) {
-            if (ext == 2) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 2);
+            if (ext == 3) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 3);
+            else if (ext == 2) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 2);
             else if (ext == 1) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 1);
             else ELG_LAUNCH(kMaxOpsLarge, false, kPL, 0);
         }
@@ -625,6 +637,33 @@ struct Tracker {
     void push(const HostOp& op, int slots = 1) {           // slots: parameter-block slots the op and its continuation take
         if (pending.size() + slots > (size_t)kMaxOpsLarge) flush(AP_NONE, 0, 0, 0, false);
         pending.push_back(op);
+    }
+
+    // MATRIX: dense, or (ELG_TRACK_SPARSE_MATRICES) packed for the uncoupled zero pattern when every entry outside it is
+    // exactly zero (layout only: the 20 kept coefficients and C in the order matrix_unc_map_s128 reads them)
+    void push_matrix(const elg_element& e) {
+        HostOp op{};
+        op.type = OP_MATRIX;
+        std::memcpy(op.coef, e.R, 36 * sizeof(double));
+        if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
+        if (o && (o->flags & ELG_TRACK_SPARSE_MATRICES)) {
+            static const unsigned char keep[6][6] = {{1, 1, 0, 0, 0, 1}, {1, 1, 0, 0, 0, 1}, {0, 0, 1, 1, 0, 1},
+                                                     {0, 0, 1, 1, 0, 1}, {1, 1, 1, 1, 1, 1}, {0, 0, 0, 0, 1, 1}};
+            bool fits = true;
+            for (int r = 0; r < 6; r++)
+                for (int c = 0; c < 6; c++) fits = fits && (keep[r][c] || e.R[6 * r + c] == 0.0);
+            if (fits) {
+                std::memcpy(op.dense, op.coef, sizeof op.dense);
+                const double* R = op.dense; const double* C = op.dense + 36;
+                const double packed[28] = {R[0], R[1], R[5], C[0], R[6], R[7], R[11], C[1], R[14], R[15], R[17], C[2],
+                                           R[20], R[21], R[23], C[3], R[24], R[25], R[26], R[27], R[28], R[29], C[4], R[34],
+                                           R[35], C[5], 0.0, 0.0};
+                std::memset(op.coef, 0, sizeof op.coef);
+                std::memcpy(op.coef, packed, sizeof packed);
+                op.type = OP_MATRIX_UNC;
+            }
+        }
+        push(op);
     }
 
     void push_higher_order(const elg_element& e) {                    // 4 slots: R, C | Tt[21][6]; MATRIX3: + 8 slots Ut[56][6]
@@ -724,7 +763,7 @@ struct Tracker {
     void prepare_hist(long long k, double s_here, bool dipole) {
         const elg_element& e = bl->e[k];
         bool writes_s = false;
-        for (const HostOp& op : pending) writes_s = writes_s || op.type == OP_DRIFT || op.type == OP_MATRIX || op.type == OP_MATRIX2 || op.type == OP_MATRIX3;
+        for (const HostOp& op : pending) writes_s = writes_s || op.type == OP_DRIFT || op.type == OP_MATRIX || op.type == OP_MATRIX2 || op.type == OP_MATRIX3 || op.type == OP_MATRIX_UNC;
         const bool need_mm = !mm_valid || writes_s;
         if (!pending.empty() || need_mm) flush(AP_NONE, 0, 0, 0, need_mm);
         if (!ok()) return;
@@ -867,12 +906,7 @@ struct Tracker {
             HostOp op{};
             switch (e.type) {
                 case ELG_DRIFT: op.type = OP_DRIFT; op.coef[0] = e.L; push(op); break;
-                case ELG_MATRIX:
-                    op.type = OP_MATRIX;
-                    std::memcpy(op.coef, e.R, 36 * sizeof(double));
-                    if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
-                    push(op);
-                    break;
+                case ELG_MATRIX: push_matrix(e); break;
                 case ELG_MATRIX2: case ELG_MATRIX3: push_higher_order(e); break;
                 case ELG_RFKICK:
                     if (e.fiducial) {                                        // G36: needs the particles in memory
@@ -933,12 +967,7 @@ struct Tracker {
             HostOp op{};
             switch (e.type) {
                 case ELG_DRIFT: op.type = OP_DRIFT; op.coef[0] = e.L; push(op); break;
-                case ELG_MATRIX:
-                    op.type = OP_MATRIX;
-                    std::memcpy(op.coef, e.R, 36 * sizeof(double));
-                    if (e.C) std::memcpy(op.coef + 36, e.C, 6 * sizeof(double));
-                    push(op);
-                    break;
+                case ELG_MATRIX: push_matrix(e); break;
                 case ELG_MATRIX2: case ELG_MATRIX3: push_higher_order(e); break;
                 case ELG_RFKICK:
                     op.type = OP_RFKICK;

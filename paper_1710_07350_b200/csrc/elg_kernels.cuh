@@ -30,7 +30,8 @@ enum : uint8_t { OP_DRIFT = 1, OP_MATRIX = 2, OP_RFKICK = 3, OP_KICK = 4,
                  OP_MATRIX2 = 5,      // second-order map: this slot holds R, C; the next three hold T (OP_CONT)
                  OP_CONT = 6,
                  OP_TKICK = 7,        // transverse wake kick of the preceding TRWAKE (G32)
-                 OP_MATRIX3 = 8 };    // third-order map: R, C | 3 slots Tt[21][6] | 8 slots Ut[56][6] (12 slots, G35)
+                 OP_MATRIX3 = 8,      // third-order map: R, C | 3 slots Tt[21][6] | 8 slots Ut[56][6] (12 slots, G35)
+                 OP_MATRIX_UNC = 9 }; // MATRIX whose zero pattern is that of an uncoupled element (flagged option)
 enum { AP_NONE = 0, AP_RCOL = 1, AP_ECOL = 2 };
 
 // Device-resident tracking state (first bytes of the workspace).  Nothing here is read by the host
@@ -214,6 +215,45 @@ __device__ __forceinline__ void matrix3_terms(const double* __restrict__ ut, con
     }
 }
 
+// Zero-pattern specialisation ("may be offered as flagged options and reported separately"): a MATRIX
+// whose entries outside the pattern of an uncoupled element are exactly zero,
+//     rows x, x': columns x, x', delta;  rows y, y': columns y, y', delta;  row s: all;  row delta: columns s, delta,
+// needs 20 of the 36 FMAs.  The kept terms run in the same order as in matrix_map, and a skipped term adds +-0, so
+// for finite coordinates the result equals the dense map's (up to the sign of a zero).  c = 28 packed doubles:
+// (R00 R01)(R05 C0)(R10 R11)(R15 C1)(R22 R23)(R25 C2)(R32 R33)(R35 C3)(R40 R41)(R42 R43)(R44 R45)(C4 R54)(R55 C5)(- -).
+template <int P>
+__device__ __forceinline__ void matrix_unc_map_s128(const double* c, const double (&v)[P][6], double (&w)[P][6]) {
+    const double2* c2 = reinterpret_cast<const double2*>(c);
+#pragma unroll
+    for (int h = 0; h < 2; h++) {                                // transverse planes: rows 2h, 2h + 1
+#pragma unroll
+        for (int rr = 0; rr < 2; rr++) {
+            const double2 k = c2[4 * h + 2 * rr], kc = c2[4 * h + 2 * rr + 1];
+#pragma unroll
+            for (int p = 0; p < P; p++) {
+                double acc = kc.y;
+                acc = fma(k.x, v[p][2 * h], acc);
+                acc = fma(k.y, v[p][2 * h + 1], acc);
+                acc = fma(kc.x, v[p][5], acc);
+                w[p][2 * h + rr] = acc;
+            }
+        }
+    }
+    const double2 s01 = c2[8], s23 = c2[9], s45 = c2[10], m = c2[11], d = c2[12];
+#pragma unroll
+    for (int p = 0; p < P; p++) {
+        double acc = m.x;
+        acc = fma(s01.x, v[p][0], acc); acc = fma(s01.y, v[p][1], acc);
+        acc = fma(s23.x, v[p][2], acc); acc = fma(s23.y, v[p][3], acc);
+        acc = fma(s45.x, v[p][4], acc); acc = fma(s45.y, v[p][5], acc);
+        w[p][4] = acc;
+        double a5 = d.y;
+        a5 = fma(m.y, v[p][4], a5);
+        a5 = fma(d.x, v[p][5], a5);
+        w[p][5] = a5;
+    }
+}
+
 // DRIFT, RFKICK and the wake KICK, in place
 template <int P, bool EXT = true>
 __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, const ChainCommon& cm, double (&v)[P][6]) {
@@ -317,7 +357,7 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
 
 // the run's maps with the coefficients in shared memory (copied there once per block): 128-bit fetches, and
 // consecutive MATRIX maps applied in pairs (v -> w -> v) so that no register copy-back is needed
-// LEVEL 0: MATRIX, DRIFT, RFKICK, KICK; 1: + MATRIX2, TKICK; 2: + MATRIX3.  The planner picks the lowest level a run
+// LEVEL 0: MATRIX, DRIFT, RFKICK, KICK; 1: + MATRIX2, TKICK; 2: + MATRIX3; 3: level 0 + MATRIX_UNC (flagged option).  The planner picks the lowest level a run
 // needs: the higher-order code costs the 200-matrix cfg3 kernel registers and 30 % of its speed when compiled in.
 template <int MAXOPS, int P, int LEVEL>
 __device__ __forceinline__ void apply_ops_smem(const ChainArgs<MAXOPS>& a, const double* s_coef, double (&v)[P][6]) {
@@ -330,18 +370,32 @@ __device__ __forceinline__ void apply_ops_smem(const ChainArgs<MAXOPS>& a, const
             matrix_map_s128<P>(s_coef + 42 * op, v, w);
             matrix_map_s128<P>(s_coef + 42 * (op + 1), w, v);
             op += 2;
-        } else if (ty == OP_MATRIX || (LEVEL >= 1 && ty == OP_MATRIX2) || (LEVEL >= 2 && ty == OP_MATRIX3)) {
+        } else if (LEVEL == 3 && ty == OP_MATRIX_UNC) {
+            double w[P][6];
+            if (op + 1 < c.n_ops && a.type[op + 1] == OP_MATRIX_UNC) {
+                matrix_unc_map_s128<P>(s_coef + 42 * op, v, w);
+                matrix_unc_map_s128<P>(s_coef + 42 * (op + 1), w, v);
+                op += 2;
+            } else {
+                matrix_unc_map_s128<P>(s_coef + 42 * op, v, w);
+#pragma unroll
+                for (int p = 0; p < P; p++)
+#pragma unroll
+                    for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+                op++;
+            }
+        } else if (ty == OP_MATRIX || (LEVEL >= 1 && LEVEL <= 2 && ty == OP_MATRIX2) || (LEVEL == 2 && ty == OP_MATRIX3)) {
             double w[P][6];
             matrix_map_s128<P>(s_coef + 42 * op, v, w);
-            if (LEVEL >= 1 && ty != OP_MATRIX) matrix2_terms<P>(s_coef + 42 * (op + 1), v, w);
-            if (LEVEL >= 2 && ty == OP_MATRIX3) matrix3_terms<P>(s_coef + 42 * (op + 4), v, w);
+            if (LEVEL >= 1 && LEVEL <= 2 && ty != OP_MATRIX) matrix2_terms<P>(s_coef + 42 * (op + 1), v, w);
+            if (LEVEL == 2 && ty == OP_MATRIX3) matrix3_terms<P>(s_coef + 42 * (op + 4), v, w);
 #pragma unroll
             for (int p = 0; p < P; p++)
 #pragma unroll
                 for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
             op += (ty == OP_MATRIX3) ? 12 : ((ty == OP_MATRIX2) ? 4 : 1);
         } else {
-            other_map<P, (LEVEL >= 1)>(ty, s_coef + 42 * op, c, v);
+            other_map<P, (LEVEL >= 1 && LEVEL <= 2)>(ty, s_coef + 42 * op, c, v);
             op++;
         }
     }
@@ -456,7 +510,7 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
 // ---------------------------------------------------------------------------------------------------
 constexpr int kPL = 6;                                  // particles per thread of the long-run kernel (levels 0, 1)
 constexpr int kPL3 = 4;                                 // with third-order maps (level 2): 6 would spill
-__host__ __device__ constexpr int long_pl(int level) { return level >= 2 ? kPL3 : kPL; }
+__host__ __device__ constexpr int long_pl(int level) { return level == 2 ? kPL3 : kPL; }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
     const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);

@@ -58,7 +58,7 @@ class Element(C.Structure):
 
 class TrackOpts(C.Structure):
     _fields_ = [
-        ("moments_every", C.c_int32), ("reserved", C.c_int32),
+        ("moments_every", C.c_int32), ("flags", C.c_int32),
         ("records", _dp), ("capacity_records", C.c_int64), ("n_records", C.c_int64),
         ("hist_out", _u32p), ("hist_capacity", C.c_int64), ("hist_written", C.c_int64),
         ("V_out", _dp), ("V_capacity", C.c_int64), ("V_written", C.c_int64),
@@ -319,6 +319,7 @@ class Bunch:
     def _opts(self, bl, n_turns, moments_every, want_stage_outputs, records):
         o = TrackOpts()
         o.moments_every = MOM[moments_every]
+        o.flags = 1 if getattr(self, "sparse_matrices", False) else 0      # ELG_TRACK_SPARSE_MATRICES
         n_rec = {"none": 0, "turn": n_turns, "element": n_turns * bl.n_elems}[moments_every]
         rec = None
         if records and n_rec:

@@ -626,6 +626,32 @@ def test_empty_bunch_and_everything_lost(elg, elgo):
         assert ei.value.code == elg.ESTATE
 
 
+def test_sparse_matrix_option_equals_dense(elg, elgo):
+    """ELG_TRACK_SPARSE_MATRICES (flagged option, reported separately): matrices with the zero pattern of an uncoupled
+    element take 20 FMAs instead of 36; results equal the dense ones (and hence the oracle's) on finite coordinates.
+    Covers long runs (pattern kernel), a coupled matrix inside the run (stays dense), and short runs (fall back)."""
+    w = make_workload("cfg3", n=60_001, n_turns=3)
+    v0 = w.particles()
+    rng = np.random.default_rng(8)
+    coupled = {"type": "MATRIX", "R": np.eye(6) + 1e-3 * rng.normal(size=(6, 6)), "C": np.zeros(6)}
+    lines = {"ring": (w.elements, True, 3), "mixed": (w.elements[:30] + [coupled] + w.elements[30:60], False, 1),
+             "short": (w.elements[:3] + [{"type": "RCOL", "ax": 1e-3, "ay": 1e-3}] + w.elements[3:6], False, 1)}
+    for name, (elems, ring, nt) in lines.items():
+        outs = []
+        for sparse in (False, True):
+            bl = elg.Beamline(elems, ring=ring)
+            b = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=bl)
+            b.sparse_matrices = sparse
+            o = b.track(bl, nt, moments_every="turn" if ring else "none")
+            outs.append((b.read(), o))
+        (dv, did), _ = outs[0]; (sv, sid), _ = outs[1]
+        assert np.array_equal(did, sid) and np.array_equal(dv, sv), name
+        if name == "ring":
+            ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C); ob.track(elgo.Beamline(elems, ring=True), 3)
+            assert np.array_equal(sv[:5], ob.read()[0][:5])
+            check_records(outs[1][1], outs[0][1])
+
+
 def test_track_in_two_calls_equals_one(elg, elgo):
     """Turn counter, RF reference and lost log carry across elg_track calls."""
     w = make_workload("cfg3", n=5000, n_matrices=10, n_turns=6)
