@@ -151,7 +151,9 @@ int64_t elg_soa_bytes(int64_t n0);
 /* ---- beamline (host only; needs no device) ----------------------------------------------------- */
 /* Validates and copies n_elems elements (L finite, apertures > 0, nb >= 2, Q > 1/2, ...).  On a bad
  * element returns ELG_EINVAL and elg_last_error() names its index.  ring = 1: the line closes on itself,
- * RF phase references and EXPLICIT windows advance by the line length every turn (G8).  The design path
+ * RF phase references and EXPLICIT windows advance by the line length every turn (G8).  ring = 0: a line; a bunch
+ * sent through it again (n_turns > 1 or a second elg_track) enters it afresh: the references of turn 0 are used on
+ * every pass (the turn number still counts up in the lost log).  The design path
  * length is the sequential fp64 sum of L (DRIFT) and C[4] (MATRIX, MATRIX2, MATRIX3) of the preceding elements. */
 int32_t elg_beamline_load(elg_beamline** out, const elg_element* h_elems, int64_t n_elems, int32_t ring);
 void    elg_beamline_destroy(elg_beamline*);

@@ -15,15 +15,19 @@
  *   elgo_matrix2      pinned  - T = 0 equals elgo_matrix bitwise, one-entry index pins, thin sextupole and
  *                               second-order drift closed forms (exact drift to O(x'^4))
  *   elgo_rfkick       pinned  - crest/zero-crossing/periodicity/slope closed forms
- *   elgo_fiducial     pinned  - exact mean (math.fsum), order-free, kicks invariant under a common delay
+ *   elgo_fiducial     pinned  - plain mean against math.fsum, kicks invariant under a common delay
  *   elgo_aperture     pinned  - hand-placed particles, brute-force stable partition, erf fractions
  *   elgo_window/histogram  pinned - hand-placed bins, edge rule, sum of counts
  *   elgo_wake_samples pinned  - beam-loading theorem, independent evaluation
  *   elgo_convolve     pinned  - brute-force double loop, numpy.convolve, continuous closed form
  *   elgo_convolve_resonator  pinned - equals elgo_convolve of elgo_wake_samples (<= 1e-12 of the maximum)
  *   elgo_kick         pinned  - bin-centre / midpoint / clamped cases
- *   elgo_dipole_histogram, elgo_convolve_d, elgo_tkick (TRWAKE)  pinned - plain weighted sums, brute-force
- *                               convolution, two-particle closed form, zero offset => zero kick, linearity
+ *   elgo_dipole_histogram, elgo_convolve_d, elgo_tkick (TRWAKE)  pinned - plain weighted sums (math.fsum), brute-force
+ *                               convolution, two-particle closed form, zero offset => zero kick, linearity, kick at a
+ *                               bin centre / midpoint / beyond the end centres / own bin
+ *   elgo_lost         pinned  - hand-placed losses, canonical order, cap < n_lost truncation
+ *   elgo_track record placement (ELGO_MOM_ELEMENT / ELGO_MOM_TURN, G26)  pinned - three-particle hand case, 77 records
+ *                               for cfg1; ring flag (G8): RF reference advances per turn on a ring only
  *   elgo_moments      pinned  - symmetric hand sets, shift invariance, Gaussian statistics
  *   elgo_track on whole configs: PARITY UNPINNED by the paper (no published end-to-end values);
  *                     it is the composition of the pinned stages in the order of PAPER.md:51.
@@ -97,7 +101,7 @@ void   elgo_matrix2(double* const v[6], int64_t n, const double* R36, const doub
 /* third-order map (G35): ... + sum_{j<=k<=l} U_ijkl v_j v_k v_l */
 void   elgo_matrix3(double* const v[6], int64_t n, const double* R36, const double* C6, const double* T126,
                     const double* U336);
-/* G36: s_design + (exact fixed-point sum of the rounded differences s_i - s_design, G33) / n; n = 0: s_design */
+/* G36: s_design + (plain long-double sum of the rounded differences s_i - s_design) / n; n = 0: s_design */
 double elgo_fiducial(const double* s, int64_t n, double s_design);
 void   elgo_rfkick(const double* s, double* delta, int64_t n, double A, double omega, double phi0,
                    double s_ref, double inv_bc);
@@ -121,7 +125,7 @@ void   elgo_convolve(const uint32_t* counts, const double* W, int32_t nb, double
 int32_t elgo_convolve_resonator(const uint32_t* counts, int32_t nb, double q, double dt, double f, double Q, double Rs,
                                 double* Vout);
 /* TRWAKE (G32-G34): counts[nb] and the per-bin dipole sums Dx[nb], Dy[nb] = sum of x, y of the particles in the
-   bin, accumulated exactly in two 64-bit fixed-point words (G33), hence independent of the summation order */
+   bin, accumulated sequentially in long double (G33: the plain definition; particles out of range are counted only) */
 int64_t elgo_dipole_histogram(const double* s, const double* x, const double* y, int64_t n, double inv_bc, double t_lo,
                               double inv_dt, int32_t nb, uint32_t* counts, double* Dx, double* Dy);
 /* V_i = q sum_{j<=i} D_j W_{i-j} (G13 with real weights) */
@@ -143,6 +147,8 @@ double elgo_inv_E(double beta0, double p0c_eV);            /* 1 / (beta0 * p0c) 
 int32_t elgo_bunch_create(elgo_bunch** out, int64_t n0, const double* const coords[6], const int64_t* ids,
                           double p0c_eV, double mc2_eV, double charge_C);
 void    elgo_bunch_destroy(elgo_bunch*);
+/* ring = 1: RF phase references and EXPLICIT windows advance by the line length every turn (G8); ring = 0: every pass
+ * uses the references of turn 0 (a line is entered afresh) */
 int32_t elgo_beamline_load(elgo_beamline** out, const elgo_element* elems, int64_t n_elems, int32_t ring);
 void    elgo_beamline_destroy(elgo_beamline*);
 /* design path length (G8) in front of element k on turn 0, and the ring/line length */

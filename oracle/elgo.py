@@ -450,13 +450,19 @@ class Bunch:
             raise RuntimeError(f"elgo_moments_now rc={rc}")
         return n.value, cen, sig.reshape(6, 6)
 
-    def lost(self):
+    def lost(self, cap: Optional[int] = None):
+        """elgo_lost.  cap=None: every record.  With a cap the first min(cap, n_lost) records come back together with
+        the status code and the true n_lost (cap < n_lost: ELGO_ECAPACITY)."""
         nl = C.c_int64()
         lib().elgo_lost(self._h, C.byref(nl), 0, None, None, None, None)
-        n = nl.value
+        n = nl.value if cap is None else min(cap, nl.value)
         ids = np.empty(n, dtype=np.int64); turn = np.empty(n, dtype=np.int32)
         elem = np.empty(n, dtype=np.int32); co = np.empty((n, 6), dtype=np.float64)
-        if n:
-            rc = lib().elgo_lost(self._h, C.byref(nl), n, _p(ids, _i64p), _p(turn, _i32p), _p(elem, _i32p), _p(co))
+        rc = OK
+        if n or cap is not None:
+            rc = lib().elgo_lost(self._h, C.byref(nl), n if cap is None else cap, _p(ids, _i64p), _p(turn, _i32p),
+                                 _p(elem, _i32p), _p(co))
+        if cap is None:
             assert rc == OK
-        return ids, turn, elem, co
+            return ids, turn, elem, co
+        return ids, turn, elem, co, rc, nl.value

@@ -902,7 +902,7 @@ struct Tracker {
         for (long long k = k_begin; k < ne && ok(); k++) {
             if (skip_next) { skip_next = false; continue; }           // TRWAKE merged into the preceding WAKE
             const elg_element& e = bl->e[k];
-            const double s_here = std::fma((double)turn, bl->length, bl->s_design[k]);      // G8
+            const double s_here = bl->ring ? std::fma((double)turn, bl->length, bl->s_design[k]) : bl->s_design[k];   // G8
             HostOp op{};
             switch (e.type) {
                 case ELG_DRIFT: op.type = OP_DRIFT; op.coef[0] = e.L; push(op); break;
@@ -963,7 +963,7 @@ struct Tracker {
     void run_turn_range(long long turn, long long k_begin, long long k_end) {       // maps only (no records)
         for (long long k = k_begin; k < k_end && ok(); k++) {
             const elg_element& e = bl->e[k];
-            const double s_here = std::fma((double)turn, bl->length, bl->s_design[k]);
+            const double s_here = bl->ring ? std::fma((double)turn, bl->length, bl->s_design[k]) : bl->s_design[k];
             HostOp op{};
             switch (e.type) {
                 case ELG_DRIFT: op.type = OP_DRIFT; op.coef[0] = e.L; push(op); break;

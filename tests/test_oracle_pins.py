@@ -635,9 +635,10 @@ def test_matrix2_in_track(elgo):
 
 
 # ------------------------------------------------------------------------------------ TRWAKE (G32-G34)
-def test_dipole_histogram_is_the_plain_weighted_sum_and_order_free(elgo):
-    """G33: the fixed-point dipole sums equal the plain per-bin sums of x and y (<= 1e-14 of the largest), do not
-    depend on the particle order (bit for bit), and the counts are elgo_histogram's."""
+def test_dipole_histogram_is_the_plain_weighted_sum(elgo):
+    """G33: the dipole sums are the plain per-bin sums of x and y (against the exactly rounded math.fsum: <= 1e-15 of
+    the sum of magnitudes, i.e. at most the final rounding), a permutation of the particles changes them by no more
+    than that, and the counts are elgo_histogram's."""
     rng = np.random.default_rng(11)
     n, nb = 200_000, 97
     s = rng.normal(size=n) * 1e-3
@@ -649,16 +650,25 @@ def test_dipole_histogram_is_the_plain_weighted_sum_and_order_free(elgo):
     c0, b0, bins = elgo.histogram(s, inv_bc, t_lo, inv_dt, nb, want_bins=True)
     assert np.array_equal(c, c0) and binned == b0 == n
     import math
-    for D, w in ((Dx, x), (Dy, y)):
-        ref = np.array([math.fsum(w[bins == k]) for k in range(nb)])              # exactly rounded sums
-        assert np.max(np.abs(D - ref)) <= 1e-14 * np.max(np.abs(ref))
     p = rng.permutation(n)
     c2, Dx2, Dy2, _ = elgo.dipole_histogram(s[p], x[p], y[p], inv_bc, t_lo, inv_dt, nb)
-    assert np.array_equal(Dx, Dx2) and np.array_equal(Dy, Dy2) and np.array_equal(c, c2)
+    assert np.array_equal(c, c2)
+    for D, D2, w in ((Dx, Dx2, x), (Dy, Dy2, y)):
+        ref = np.array([math.fsum(w[bins == k]) for k in range(nb)])              # exactly rounded sums
+        mag = np.array([math.fsum(np.abs(w[bins == k])) for k in range(nb)])
+        assert np.all(np.abs(D - ref) <= 1e-15 * mag + 1e-300)
+        assert np.all(np.abs(D2 - ref) <= 1e-15 * mag + 1e-300)
+        assert np.max(np.abs(ref)) > 0
+    # a wrong weight (y for x), a dropped particle or a shifted bin would be far outside: sanity of the pin itself
+    assert np.max(np.abs(Dx - Dy)) > 1e-6
     # exactly representable offsets give exact sums; out-of-range / NaN offsets are counted but not summed
     s3 = np.zeros(5); x3 = np.array([0.5, 0.25, -0.125, np.nan, 4.0e6]); y3 = np.ones(5)
     c3, Dx3, Dy3, _ = elgo.dipole_histogram(s3, x3, y3, 1.0, -0.5, 1.0, 2)
     assert c3.tolist() == [5, 0] and Dx3[0] == 0.625 and Dy3[0] == 3.0
+    # two particles in two bins: each sum is that particle's coordinate, bit for bit
+    c4, Dx4, Dy4, _ = elgo.dipole_histogram(np.array([0.0, 1.0]), np.array([1e-4 / 3, -7e-5]), np.array([2e-4, 1e-5 / 7]),
+                                            1.0, -0.5, 1.0, 2)
+    assert c4.tolist() == [1, 1] and Dx4.tolist() == [1e-4 / 3, -7e-5] and Dy4.tolist() == [2e-4, 1e-5 / 7]
 
 
 def test_convolve_d_bruteforce(elgo):
@@ -781,15 +791,18 @@ def test_matrix3_in_track(elgo):
 
 
 # ------------------------------------------------------------------------------------ fiducial RF phase (G36)
-def test_fiducial_is_the_exact_mean_and_makes_kicks_delay_invariant(elgo):
+def test_fiducial_is_the_plain_mean_and_makes_kicks_delay_invariant(elgo):
     import math
     rng = np.random.default_rng(31)
     s0 = 271.25
     s = s0 + rng.normal(size=50_000) * 1e-3 + 3e-4
     f = elgo.fiducial(s, s0)
-    assert abs(f - (s0 + math.fsum(s - s0) / s.size)) <= 1e-15 * s0
-    assert elgo.fiducial(s[rng.permutation(s.size)], s0) == f                 # order-free
+    exact = math.fsum(s - s0) / s.size                                        # mean of the rounded differences
+    assert abs((f - s0) - exact) <= 2.0 ** -52 * s0                           # the final s0 + mean rounds at ulp(s0)
+    assert abs(exact - 3e-4) < 2e-5                                           # the bunch is 0.3 mm late
+    assert abs(elgo.fiducial(s[rng.permutation(s.size)], s0) - f) <= 2.0 ** -52 * s0
     assert elgo.fiducial(s[:0], s0) == s0
+    assert elgo.fiducial(np.array([s0 + 0.5, s0 + 0.25, s0 - 0.125, np.nan, s0 + 4.0e6]), s0) == s0 + 0.625 / 5
     # a common delay of the whole bunch changes the design-orbit kick but not the fiducial one
     w = make_workload("cfg0", n=2000)
     v0 = w.particles()
@@ -821,3 +834,129 @@ def test_convolve_resonator_equals_direct_convolution(elgo):
         assert np.max(np.abs(V - Vr)) <= 1e-12 * np.max(np.abs(V))
         one = np.zeros(nb, dtype=np.uint32); one[0] = 1
         assert np.allclose(elgo.convolve_resonator(one, 1.0, dt, f, Q, Rs), W, rtol=1e-12, atol=1e-12 * np.max(np.abs(W)))
+
+
+# ------------------------------------------------------------------------------------ record placement, lost log, ring
+def test_records_after_every_element_hand_case(elgo):
+    """G26 (statistics after every element): with moments_every = "element" one record follows EVERY
+    element, taken on the live set AFTER that element (after the compaction of an aperture).  Three particles, the
+    middle one is removed by an RCOL: the record behind the RCOL has n = 2 and the survivors' centroid; the record
+    in front of it still has n = 3.  moments_every = "turn": one record, after the last element."""
+    v0 = np.zeros((6, 3))
+    v0[0] = [1e-4, 5e-3, -3e-4]                          # x: the middle particle is outside a 1 mm RCOL
+    v0[1] = [1e-5, 0.0, -2e-5]
+    v0[5] = [1e-3, 2e-3, 4e-3]
+    elems = [{"type": "DRIFT", "L": 2.0}, {"type": "RCOL", "ax": 1e-3, "ay": 1e-3}, {"type": "DRIFT", "L": 1.0}]
+    b = elgo.Bunch(v0, 1e9, 1e-9)
+    out = b.track(elgo.Beamline(elems), 1, moments_every="element")
+    rec = out["records"]
+    assert rec.shape == (3, 43)
+    assert rec[:, 0].tolist() == [3.0, 2.0, 2.0]
+    x_after_drift = v0[0] + 2.0 * v0[1]                  # fma(x', L, x) is exact for these values? compare loosely
+    assert abs(rec[0, 1] - x_after_drift.mean()) <= 1e-18
+    assert abs(rec[1, 1] - x_after_drift[[0, 2]].mean()) <= 1e-18          # survivors only, right behind the RCOL
+    assert abs(rec[1, 6] - 2.5e-3) <= 1e-18 and abs(rec[0, 6] - 7e-3 / 3) <= 1e-18       # <delta>
+    assert abs(rec[1, 5] - 2.0) < 1e-9 and abs(rec[2, 5] - 3.0) < 1e-9      # <s>: 2 m, then 3 m
+    x_end = x_after_drift[[0, 2]] + 1.0 * v0[1, [0, 2]]
+    assert abs(rec[2, 1] - x_end.mean()) <= 1e-18
+    S_xx = np.var(x_end)
+    assert abs(rec[2, 7] - S_xx) <= 1e-12 * S_xx
+    # "turn": one record, after the whole line = the last per-element record
+    b2 = elgo.Bunch(v0, 1e9, 1e-9)
+    out2 = b2.track(elgo.Beamline(elems), 1, moments_every="turn")
+    assert out2["records"].shape == (1, 43) and np.array_equal(out2["records"][0], rec[2])
+    # "none": no record
+    b3 = elgo.Bunch(v0, 1e9, 1e-9)
+    assert b3.track(elgo.Beamline(elems), 1, moments_every="none")["records"].shape[0] == 0
+
+
+def test_records_cfg1_77_and_counts_follow_the_lost_log(elgo):
+    """cfg1: 77 elements -> 77 records; n of record k = n0 - (lost at elements <= k)."""
+    w = make_workload("cfg1", n=20_000)
+    b = elgo.Bunch(w.particles(), w.p0c_eV, w.charge_C)
+    out = b.track(elgo.Beamline(w.elements), 1, moments_every="element")
+    rec = out["records"]
+    assert rec.shape == (77, 43)
+    li, lt, le, lc = b.lost()
+    n_after = w.n0 - np.array([(le <= k).sum() for k in range(77)])
+    assert np.array_equal(rec[:, 0], n_after.astype(np.float64))
+    assert rec[-1, 0] == b.n_alive < w.n0
+
+
+def test_tkick_interpolation(elgo):
+    """elgo_tkick (G14 applied to Vx, Vy): bin centre -> exactly V_k; midway between two centres -> their mean; beyond
+    the first / last centre -> the end value; interp = 0 -> the particle's own bin; unbinned -> untouched."""
+    nb, t_lo, dt = 8, 0.0, 0.25
+    Vx = np.array([1.0, 3.0, 2.0, -4.0, 0.0, 8.0, 8.5, 7.0])
+    Vy = np.array([-2.0, 0.5, 0.25, 6.0, 1.0, -1.0, 3.0, 9.0])
+    iE = 0.5
+    centres = t_lo + (np.arange(nb) + 0.5) * dt
+    xp = np.zeros(nb); yp = np.zeros(nb)
+    elgo.tkick(centres, xp, yp, 1.0, t_lo, 1 / dt, nb, Vx, Vy, iE)
+    assert np.array_equal(xp, Vx * iE) and np.array_equal(yp, Vy * iE)          # sign: x' += Vx / E (G32)
+    mid = centres[:-1] + dt / 2                                                  # exactly representable: k dt
+    xp = np.zeros(nb - 1); yp = np.zeros(nb - 1)
+    elgo.tkick(mid - 1e-12, xp, yp, 1.0, t_lo, 1 / dt, nb, Vx, Vy, iE)
+    assert np.allclose(xp, 0.5 * (Vx[:-1] + Vx[1:]) * iE, rtol=0, atol=1e-9)
+    assert np.allclose(yp, 0.5 * (Vy[:-1] + Vy[1:]) * iE, rtol=0, atol=1e-9)
+    # a quarter of the way from centre 2 to centre 3: V_2 + (V_3 - V_2)/4, exact in binary
+    xp = np.zeros(1); yp = np.zeros(1)
+    elgo.tkick(np.array([centres[2] + dt / 4]), xp, yp, 1.0, t_lo, 1 / dt, nb, Vx, Vy, iE)
+    assert xp[0] == (2.0 + 0.25 * (-4.0 - 2.0)) * iE and yp[0] == (0.25 + 0.25 * (6.0 - 0.25)) * iE
+    xp = np.zeros(2); yp = np.zeros(2)
+    elgo.tkick(np.array([t_lo + 0.01 * dt, t_lo + (nb - 0.01) * dt]), xp, yp, 1.0, t_lo, 1 / dt, nb, Vx, Vy, iE)
+    assert xp.tolist() == [Vx[0] * iE, Vx[-1] * iE] and yp.tolist() == [Vy[0] * iE, Vy[-1] * iE]
+    xp = np.full(3, 0.125); yp = np.full(3, -0.5)
+    elgo.tkick(np.array([t_lo - dt, t_lo + nb * dt, np.nan]), xp, yp, 1.0, t_lo, 1 / dt, nb, Vx, Vy, iE)
+    assert xp.tolist() == [0.125] * 3 and yp.tolist() == [-0.5] * 3
+    xp = np.zeros(1); yp = np.zeros(1)
+    elgo.tkick(np.array([t_lo + 2.9 * dt]), xp, yp, 1.0, t_lo, 1 / dt, nb, Vx, Vy, iE, interp=False)
+    assert xp[0] == Vx[2] * iE and yp[0] == Vy[2] * iE
+
+
+def test_lost_log_truncation(elgo):
+    """elgo_lost with cap < n_lost fills the first cap records (canonical order, G18), returns ELGO_ECAPACITY and the
+    true n_lost; cap >= n_lost returns ELGO_OK."""
+    n = 12
+    v0 = np.zeros((6, n))
+    v0[0] = np.where(np.arange(n) % 3 == 0, 2e-3, 1e-4)        # particles 0, 3, 6, 9 leave a 1 mm RCOL
+    v0[2, 5] = -0.99e-3; v0[0, 5] = 0.5e-3                     # |x|, |y| <= 1 mm but x^2 + y^2 > 1 mm^2: lost at the ECOL only
+    v0[5] = np.arange(n) * 1e-3
+    elems = [{"type": "RCOL", "ax": 1e-3, "ay": 1e-3}, {"type": "ECOL", "a": 1e-3, "b": 1e-3}]
+    b = elgo.Bunch(v0, 1e9, 1e-9)
+    b.track(elgo.Beamline(elems, ring=True), 2)
+    ids, turn, elem, co = b.lost()
+    assert ids.tolist() == [0, 3, 6, 9, 5] and elem.tolist() == [0, 0, 0, 0, 1] and turn.tolist() == [0] * 5
+    assert np.array_equal(co[:, 5], v0[5, [0, 3, 6, 9, 5]]) and np.array_equal(co[:, 0], v0[0, [0, 3, 6, 9, 5]])
+    i3, t3, e3, c3, rc, nl = b.lost(cap=3)
+    assert rc == elgo.ECAPACITY and nl == 5
+    assert i3.tolist() == [0, 3, 6] and np.array_equal(c3, co[:3]) and e3.tolist() == [0, 0, 0]
+    i5, t5, e5, c5, rc, nl = b.lost(cap=5)
+    assert rc == elgo.OK and nl == 5 and i5.tolist() == ids.tolist()
+    i9, t9, e9, c9, rc, nl = b.lost(cap=9)
+    assert rc == elgo.OK and nl == 5 and i9.tolist() == ids.tolist()
+    i0, t0, e0, c0, rc, nl = b.lost(cap=0)
+    assert rc == elgo.ECAPACITY and nl == 5 and i0.size == 0
+
+
+def test_ring_flag_advances_rf_reference_only_on_a_ring(elgo):
+    """G8: on a ring (ring = 1) the RF phase reference advances by the ring length per turn; a line (ring = 0) is
+    entered afresh on every pass (reference of turn 0).  One linear drift MATRIX (C5 = L) + RFKICK at 90 degrees:
+    a particle on the design orbit is on crest every turn on a ring, and off crest by 2 pi f L / (beta0 c) per turn on
+    a line."""
+    from elg_inputs import drift_matrix
+    p0c = 1e9
+    b0 = elgo.beta0(p0c); ibc = elgo.inv_bc(b0); A = 1e6 * elgo.inv_E(b0, p0c)
+    L, f = 0.3, 2.856e9
+    R, Cv = drift_matrix(L)
+    elems = [{"type": "MATRIX", "R": R, "C": Cv}, {"type": "RFKICK", "V": 1e6, "f": f, "phi": math.pi / 2}]
+    v0 = np.zeros((6, 1))
+    out = {}
+    for ring in (True, False):
+        b = elgo.Bunch(v0, p0c, 1e-9)
+        b.track(elgo.Beamline(elems, ring=ring), 3)
+        out[ring] = b.read()[0][5, 0]
+    assert abs(out[True] - 3 * A) <= 1e-15 * A                                   # on crest three times
+    phase = 2 * math.pi * f * L * ibc
+    expect = A * (1.0 + math.cos(phase) + math.cos(2 * phase))                   # sin(pi/2 + k phase)
+    assert abs(out[False] - expect) <= 1e-9 * A and abs(out[False] - out[True]) > 0.1 * A
