@@ -11,6 +11,7 @@ from .configs import (
     ELECTRON_MC2_EV, C_LIGHT, Workload, make_workload, WORKLOAD_NAMES,
     drift_matrix, thin_quad_matrix, compose, pair_index, second_order_drift, thin_quad_sextupole,
     triple_index, thin_quad_sext_octupole, third_order_drift,
+    dense_symplectic_matrix, dense_higher_order, dense_map_element,
 )
 
 __all__ = [
@@ -18,4 +19,5 @@ __all__ = [
     "make_workload", "WORKLOAD_NAMES", "drift_matrix", "thin_quad_matrix", "compose",
     "pair_index", "second_order_drift", "thin_quad_sextupole",
     "triple_index", "thin_quad_sext_octupole", "third_order_drift",
+    "dense_symplectic_matrix", "dense_higher_order", "dense_map_element",
 ]

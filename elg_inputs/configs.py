@@ -145,6 +145,49 @@ def _matrix_elem(R, C):
             "C": np.ascontiguousarray(C, dtype=np.float64)}
 
 
+def dense_symplectic_matrix(seed: int, strength: float = 0.6, c_s: float = 0.7):
+    """A seeded DENSE symplectic 6x6 matrix (all 36 entries non-zero) with all six C entries non-zero, for parity
+    tests whose inputs must exercise every coefficient of a map.  Cayley transform of a random Hamiltonian matrix
+    H = J S (S symmetric): M = (I - H/2)^-1 (I + H/2) satisfies M^T J M = J exactly in exact arithmetic; the pairs
+    are (x, x'), (y, y'), (s, delta).  Layout / coefficient generation only: nothing is applied to a particle."""
+    rng = np.random.default_rng(seed)
+    A = rng.normal(size=(6, 6))
+    S = strength * (A + A.T) / 2.0
+    J = np.zeros((6, 6))
+    for k in range(3):
+        J[2 * k, 2 * k + 1] = 1.0
+        J[2 * k + 1, 2 * k] = -1.0
+    H = J @ S
+    M = np.linalg.solve(np.eye(6) - 0.5 * H, np.eye(6) + 0.5 * H)
+    C = rng.normal(size=6) * np.array([2e-5, 2e-6, 2e-5, 2e-6, c_s, 2e-4])
+    assert np.all(M != 0.0) and np.all(C != 0.0)
+    return np.ascontiguousarray(M), np.ascontiguousarray(C)
+
+
+def dense_higher_order(seed: int, order: int, t_scale: float = 1.0, u_scale: float = 1.0e4):
+    """Seeded DENSE second- (T: all 126 entries non-zero) and third-order (U: all 336 non-zero) coefficients, scaled so
+    that for a 100 um / 10 urad / 1 mm / 1e-3 beam the higher-order terms stay around 1e-3 of the linear ones."""
+    rng = np.random.default_rng(seed + 7919)
+    T = rng.normal(size=(6, 21)) * t_scale
+    T[np.abs(T) < 1e-3 * t_scale] = 1e-3 * t_scale
+    if order < 3:
+        return np.ascontiguousarray(T), None
+    U = rng.normal(size=(6, 56)) * u_scale
+    U[np.abs(U) < 1e-3 * u_scale] = 1e-3 * u_scale
+    return np.ascontiguousarray(T), np.ascontiguousarray(U)
+
+
+def dense_map_element(seed: int, order: int = 1, strength: float = 0.6, t_scale: float = 1.0, u_scale: float = 1.0e4,
+                      c_s: float = 0.7):
+    """One MATRIX / MATRIX2 / MATRIX3 element dictionary with dense seeded coefficients (see above).  Long runs of
+    higher-order maps need small strength / c_s / scales to keep the beam finite (parity is value-independent)."""
+    R, C = dense_symplectic_matrix(seed, strength, c_s)
+    if order == 1:
+        return _matrix_elem(R, C)
+    T, U = dense_higher_order(seed, order, t_scale, u_scale)
+    return _matrix2_elem(R, C, T) if order == 2 else _matrix3_elem(R, C, T, U)
+
+
 def beta0_of(p0c_eV: float, mc2_eV: float) -> float:
     return p0c_eV / np.sqrt(p0c_eV * p0c_eV + mc2_eV * mc2_eV)
 

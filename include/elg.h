@@ -219,15 +219,30 @@ enum { ELG_K_CHAIN = 0, ELG_K_CHAIN_COMPACT = 1, ELG_K_WINDOW = 2, ELG_K_HIST = 
 int32_t elg_profile_enable(elg_bunch*, int32_t on);
 int32_t elg_profile_read(elg_bunch*, int64_t* h_launches, double* h_ms);
 
-/* ---- single-stage test hooks (same kernels as elg_track; device arrays supplied by the caller) ----- */
-int32_t elg_dbg_histogram(const double* d_s, int64_t n, double inv_bc, double t_lo, double inv_dt, int32_t nb,
-                          uint32_t* d_counts, void* stream);
+/* ---- single-stage test hooks (not the user boundary) -------------------------------------------------
+ * For the stage-by-stage parity protocol (the paper compares CPU and GPU element by element on the
+ * same inputs).  The bunch-based hooks run ONE stage of elg_track on the particles currently in
+ * the bunch -- upload the oracle's input of that stage with elg_bunch_upload first -- through the same planner code
+ * and therefore the same kernels, instantiations and launch configurations as tracking itself:
+ *   elg_dbg_histogram         min/max epilogue run, window_kernel (EXPLICIT window t_lo, dt), hist_kernel with the
+ *                             occupied-range privatisation -> counts (uint32[nb], DEVICE)
+ *   elg_dbg_dipole_histogram  the same with dipole_hist_kernel + dipole_finalize_kernel -> counts, Dx[nb] Dy[nb] (G33)
+ *   elg_dbg_kick / _tkick     window as above, then the wake kick as tracking applies it: OP_KICK / OP_TKICK as a
+ *                             fused run of one op reading V (or Vx, Vy) copied from the caller's DEVICE arrays (G14)
+ *   elg_dbg_compact           a run of zero maps ending in the aperture: predicate + stable compaction + lost log
+ *                             (PAPER.md:141 loss contract); read the result with elg_bunch_read / elg_lost
+ * nb must not exceed the bin capacity the workspace was sized for.  The two array-based hooks run the wake-sample and
+ * convolution kernels of tracking on caller-supplied DEVICE arrays (whole bin range). */
+int32_t elg_dbg_histogram(elg_bunch*, double t_lo, double dt, int32_t nb, uint32_t* d_counts);
+int32_t elg_dbg_dipole_histogram(elg_bunch*, double t_lo, double dt, int32_t nb, uint32_t* d_counts, double* d_D);
+int32_t elg_dbg_kick(elg_bunch*, double t_lo, double dt, int32_t nb, const double* d_V, int32_t interp);
+int32_t elg_dbg_tkick(elg_bunch*, double t_lo, double dt, int32_t nb, const double* d_Vx, const double* d_Vy,
+                      int32_t interp);
+int32_t elg_dbg_compact(elg_bunch*, int32_t type /* ELG_RCOL | ELG_ECOL */, double ax, double ay);
 int32_t elg_dbg_wake_samples(int32_t kind, int32_t nb, double dt, double f, double Q, double Rs,
                              const double* d_table, int64_t n_table, double dt_table, double* d_W, void* stream);
 int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W, int32_t nb, double q, double* d_V,
                          void* stream);
-int32_t elg_dbg_kick(const double* d_s, double* d_delta, int64_t n, double inv_bc, double t_lo, double inv_dt,
-                     int32_t nb, const double* d_V, double inv_E, int32_t interp, void* stream);
 
 #ifdef __cplusplus
 }

@@ -1,7 +1,13 @@
 """Build libelg.so (hand-written CUDA for sm_100a) in-tree with nvcc.  No JIT cache, no torch extension:
-the result is a plain C-ABI shared library next to this file (see include/elg.h)."""
+the result is a plain C-ABI shared library next to this file (see include/elg.h).
+
+Staleness is decided by CONTENT, not by modification time: the SHA-256 of the sources and the compiler flags is kept
+in a sidecar file next to the library (file times do not survive a copy to another machine; a hash does).  A library
+whose sidecar does not match the sources is never loaded: it is rebuilt, and if that is impossible the caller gets the
+error."""
 from __future__ import annotations
 
+import hashlib
 import os
 import shutil
 import subprocess
@@ -26,13 +32,35 @@ def nvcc_path() -> str:
     raise RuntimeError("nvcc not found (set NVCC or add /usr/local/cuda/bin to PATH)")
 
 
+def source_hash(extra=()) -> str:
+    h = hashlib.sha256()
+    for p in DEPS:
+        with open(p, "rb") as f:
+            h.update(f.read())
+        h.update(b"\0")
+    h.update(" ".join(NVCC_FLAGS + list(extra)).encode())
+    return h.hexdigest()
+
+
+def is_current(out: str = LIB, extra=()) -> bool:
+    """True when `out` exists and was built from exactly the present sources and flags."""
+    side = out + ".hash"
+    if not (os.path.exists(out) and os.path.exists(side)):
+        return False
+    with open(side) as f:
+        return f.read().strip() == source_hash(extra)
+
+
 def build(force: bool = False, verbose: bool = False, out: str = LIB, extra=()) -> str:
-    """Compile libelg.so.  `extra` / `out` build tuning variants (-DELG_COMPACT_WARPS=..., see elg_kernels.cuh)."""
-    newest = max(os.path.getmtime(p) for p in DEPS)
-    if not force and os.path.exists(out) and os.path.getmtime(out) >= newest:
+    """Compile libelg.so unless it is current.  `extra` / `out` build tuning variants (-D..., see elg_kernels.cuh).
+    Raises if the compiler is missing or the compilation fails: a stale library is never returned."""
+    if not force and is_current(out, extra):
         return out
-    cmd = [nvcc_path()] + NVCC_FLAGS + list(extra) + (["-Xptxas", "-v"] if verbose else []) + [SRC, "-o", out]
+    cmd = [nvcc_path()] + NVCC_FLAGS + list(extra) + (["-Xptxas", "-v"] if verbose else []) + [SRC, "-o", out + ".tmp"]
     subprocess.run(cmd, check=True)
+    os.replace(out + ".tmp", out)
+    with open(out + ".hash", "w") as f:
+        f.write(source_hash(extra) + "\n")
     return out
 
 

@@ -172,7 +172,7 @@ WorkLayout layout(long long n0, long long nb_cap, long long table_cap, long long
     long long o = 0;
     L.off_state = o; o = align_up(o + (long long)sizeof(DevState), 256);
     L.off_soaB = o; o = align_up(o + 7 * stride * 8, 256);
-    L.off_status = o; o = align_up(o + (stride / kTile + 2) * 8, 256);
+    L.off_status = o; o = align_up(o + (stride / kStatusTile + 2) * 8, 256);
     L.off_mm = o; o = align_up(o + 2LL * kMmPartials * 8, 256);
     L.off_mom = o; o = align_up(o + (long long)kNMom * kMaxGrid * 8, 256);
     L.off_rec = o; o = align_up(o + (kRecCap + 1) * 43 * 8, 256);   // + 1: elg_moments' own slot
@@ -224,6 +224,8 @@ int32_t long_setup_once() {
                                     chain_long_smem_bytes<kMaxOpsLarge, 2>()));
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     chain_long_smem_bytes<kMaxOpsLarge, 3>()));
+        ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
+        ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
         done = true;
     }
     return ELG_OK;
@@ -414,7 +416,7 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     b->hist_aggregate = agg ? std::atoi(agg) : -1;                 // -1: automatic
     const char* fp = std::getenv("ELG_CHAIN_P");
     b->force_p = fp ? std::atoi(fp) : 0;
-    cudaError_t ce = cudaMemsetAsync(b->tile_status, 0, (b->stride / kTile + 2) * 8, b->stream);
+    cudaError_t ce = cudaMemsetAsync(b->tile_status, 0, (b->stride / kStatusTile + 2) * 8, b->stream);
     if (ce != cudaSuccess) { delete b; return fail(ELG_ECUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(ce)); }
     rc = elg_bunch_rewind(b);
     if (rc != ELG_OK) { delete b; return rc; }
@@ -509,11 +511,11 @@ struct Tracker {
     }
 
     // blocks of a persistent grid = resident blocks per SM x SMs, looked up once per kernel
-    int cached_grid(const void* kernel, int smem) {
+    int cached_grid(const void* kernel, int smem, int threads = kBlock) {
         auto it = b->grids.find(kernel);
         if (it != b->grids.end()) return it->second;
         int occ = 0;
-        check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kBlock, smem), "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+        check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem), "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
         if (occ < 1 && rc == ELG_OK) rc = fail(ELG_ECUDA, "kernel does not fit on an SM");
         long long g = (long long)occ * b->sms;
         if (g > kMaxGrid) g = kMaxGrid / b->sms * b->sms;
@@ -537,7 +539,7 @@ struct Tracker {
         c.tile_status = b->tile_status;
         if (COMPACT) b->epoch = (b->epoch + 1) & 0x3fffffffu;
         if (COMPACT && b->epoch == 0) {                               // epoch wrapped: stale tags could alias
-            check(cudaMemsetAsync(b->tile_status, 0, (b->stride / kTile + 2) * 8, b->stream), "cudaMemsetAsync");
+            check(cudaMemsetAsync(b->tile_status, 0, (b->stride / kStatusTile + 2) * 8, b->stream), "cudaMemsetAsync");
             b->epoch = 1;
         }
         c.epoch = b->epoch;
@@ -552,10 +554,11 @@ struct Tracker {
         int grid = 0;
         if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS, EXT>, chain_long_smem_bytes<MAXOPS, EXT>());
         else if constexpr (COMPACT) {
-            grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0)>, 0);
+            grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0)>, compact_smem_bytes(), kC2Threads);
             if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
         } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, (EXT != 0)>, 0);
         if (!ok()) return;
+        if ((long long)(mm_slot + 1) * grid > kMmPartials) { rc = fail(ELG_ECAPACITY, "elg_upload_and_track: too many chunks for the min/max partial slots"); return; }
         c.mm_partial = b->mm_partial + 2LL * mm_slot * grid;          // one slot of partials per chunk
         if (want_mm) mm_grid = (mm_slot + 1) * grid;
         {
@@ -565,7 +568,8 @@ struct Tracker {
             else if constexpr (COMPACT)
             {
                 void* kargs[] = {(void*)&a};                     // cooperative: every block resident (static tiles)
-                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS, (EXT != 0)>, dim3(grid), dim3(kBlock), kargs, 0, b->stream),
+                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS, (EXT != 0)>, dim3(grid), dim3(kC2Threads), kargs,
+                                                  compact_smem_bytes(), b->stream),
                       "compact_kernel cooperative launch");
             }
             else
@@ -745,7 +749,7 @@ struct Tracker {
     void wake_or_histo(long long k, double s_here) {
         const elg_element& e = bl->e[k];
         const bool merged = mergeable(k);
-        prepare_hist(k, s_here, e.type == ELG_TRWAKE || merged);
+        prepare_hist(e, b ? s_here * b->inv_bc : 0.0, e.type == ELG_TRWAKE || merged);
         if (!ok() || e.type == ELG_HISTO) return;
         if (e.type == ELG_WAKE) {
             wake_part(k);
@@ -760,8 +764,8 @@ struct Tracker {
         }
     }
 
-    void prepare_hist(long long k, double s_here, bool dipole) {
-        const elg_element& e = bl->e[k];
+    // min/max epilogue of the pending run, window, histogram.  t_design: design arrival time at the element (EXPLICIT)
+    void prepare_hist(const elg_element& e, double t_design, bool dipole) {
         bool writes_s = false;
         for (const HostOp& op : pending) writes_s = writes_s || op.type == OP_DRIFT || op.type == OP_MATRIX || op.type == OP_MATRIX2 || op.type == OP_MATRIX3 || op.type == OP_MATRIX_UNC;
         const bool need_mm = !mm_valid || writes_s;
@@ -770,18 +774,8 @@ struct Tracker {
         count();                                                      // window
         count();                                                      // histogram
         if (b) {
-            if (e.nb > b->nb_cap) { rc = fail(ELG_ECAPACITY, "elg_track: workspace was sized for fewer bins than this beamline needs"); return; }
-            WindowArgs w;
-            w.st = b->st; w.cur = b->cur_slot; w.mm_partial = b->mm_partial; w.n_partial = mm_grid;
-            w.mode = e.window; w.nb = e.nb; w.t_lo_rel = e.t_lo_rel;
-            w.dt_in = (e.window == ELG_WIN_AUTO_TABLE) ? e.dt_table : e.dt;
-            w.t_design = s_here * b->inv_bc; w.inv_bc = b->inv_bc; w.counts = b->counts;
-            w.dacc = dipole ? reinterpret_cast<long long*>(b->dacc) : nullptr;
-            {
-                ProfScope ps(b, ELG_K_WINDOW);
-                window_kernel<<<(e.nb + 4 * kBlock - 1) / (4 * kBlock), kBlock, 0, b->stream>>>(w);
-            }
-            check(cudaGetLastError(), "window_kernel launch");
+            launch_window(e, t_design, dipole);
+            if (!ok()) return;
             if (dipole) {                                             // counts + exact dipole sums (G33)
                 DipoleArgs d;
                 d.s = b->coord(b->cur_buf, 4); d.x = b->coord(b->cur_buf, 0); d.y = b->coord(b->cur_buf, 2);
@@ -803,6 +797,44 @@ struct Tracker {
             check(cudaGetLastError(), "hist_kernel launch");
             stage_out_hist(e.nb);
         } else if (o) { o->window_written++; o->hist_written += e.nb; }
+    }
+
+    // window_kernel: min/max partials of the last epilogue -> device-resident window + occupied bin range, zero counts
+    void launch_window(const elg_element& e, double t_design, bool dipole) {
+        if (e.nb > b->nb_cap) { rc = fail(ELG_ECAPACITY, "elg_track: workspace was sized for fewer bins than this beamline needs"); return; }
+        WindowArgs w;
+        w.st = b->st; w.cur = b->cur_slot; w.mm_partial = b->mm_partial; w.n_partial = mm_grid;
+        w.mode = e.window; w.nb = e.nb; w.t_lo_rel = e.t_lo_rel;
+        w.dt_in = (e.window == ELG_WIN_AUTO_TABLE) ? e.dt_table : e.dt;
+        w.t_design = t_design; w.inv_bc = b->inv_bc; w.counts = b->counts;
+        w.dacc = dipole ? reinterpret_cast<long long*>(b->dacc) : nullptr;
+        {
+            ProfScope ps(b, ELG_K_WINDOW);
+            window_kernel<<<(e.nb + 4 * kBlock - 1) / (4 * kBlock), kBlock, 0, b->stream>>>(w);
+        }
+        check(cudaGetLastError(), "window_kernel launch");
+    }
+
+    void dipole_finalize(int nb) {                                    // fixed-point accumulators -> Dx, Dy (G33)
+        ProfScope ps(b, ELG_K_CONV);
+        dipole_finalize_kernel<<<(nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(b->dacc, nb, b->D);
+        check(cudaGetLastError(), "dipole_finalize_kernel launch");
+    }
+
+    // the wake kicks are not passes of their own: they wait in the pending list as the first ops of the next run
+    void queue_kick(int nb, int interp) {
+        HostOp op{};
+        op.type = OP_KICK;
+        op.coef[0] = b ? b->inv_bc : 0.0; op.coef[1] = b ? b->inv_E : 0.0;
+        pending.push_back(op);
+        kick_nb = nb; kick_interp = interp;
+    }
+    void queue_tkick(int nb, int interp) {
+        HostOp op{};
+        op.type = OP_TKICK;
+        op.coef[0] = b ? b->inv_bc : 0.0; op.coef[1] = b ? b->inv_E : 0.0;
+        pending.push_back(op);
+        tk_nb = nb; tk_interp = interp;
     }
 
     void launch_samples(long long k) {
@@ -848,11 +880,7 @@ struct Tracker {
                 check(cudaMemcpyAsync(o->V_out + o->V_written, b->V, (size_t)e.nb * 8, cudaMemcpyDeviceToHost, b->stream), "V D2H");
         }
         if (o) o->V_written += e.nb;
-        HostOp op{};
-        op.type = OP_KICK;
-        op.coef[0] = b ? b->inv_bc : 0.0; op.coef[1] = b ? b->inv_E : 0.0;
-        pending.push_back(op);
-        kick_nb = e.nb; kick_interp = e.interp;
+        queue_kick(e.nb, e.interp);
     }
 
     void trwake_part(long long k) {                                   // samples, dipole sums -> doubles, two convolutions
@@ -860,11 +888,7 @@ struct Tracker {
         count(); count(); count(); count();
         if (b) {
             launch_samples(k);
-            {
-                ProfScope ps(b, ELG_K_CONV);
-                dipole_finalize_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(b->dacc, e.nb, b->D);
-            }
-            check(cudaGetLastError(), "dipole_finalize_kernel launch");
+            dipole_finalize(e.nb);
             for (int plane = 0; plane < 2; plane++) {
                 ConvArgs<double> cv;
                 cv.counts = b->D + (size_t)plane * e.nb; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro;
@@ -879,11 +903,7 @@ struct Tracker {
             }
         }
         if (o) o->V_written += 4LL * e.nb;
-        HostOp op{};
-        op.type = OP_TKICK;
-        op.coef[0] = b ? b->inv_bc : 0.0; op.coef[1] = b ? b->inv_E : 0.0;
-        pending.push_back(op);
-        tk_nb = e.nb; tk_interp = e.interp;
+        queue_tkick(e.nb, e.interp);
     }
 
     void stage_out_hist(int nb) {
@@ -1176,35 +1196,83 @@ extern "C" int32_t elg_bunch_device_array(elg_bunch* b, int32_t c, void** d_ptr)
 }
 
 // ------------------------------------------------------------------------------------- test hooks
+// The hooks below run ONE stage of elg_track on the particles currently in the bunch (the caller uploads the oracle's
+// input of that stage first), through the same planner code (Tracker) and hence the same kernels and launch
+// configurations as tracking itself.
 namespace {
-int32_t hook_grid(int* grid, int per_sm) {
-    int sms = 0;
-    int32_t rc = device_sms(&sms);
-    if (rc != ELG_OK) return rc;
-    *grid = sms * per_sm;
+elg_element hook_window_element(double dt, int32_t nb) {
+    elg_element e{};
+    e.type = ELG_HISTO; e.nb = nb; e.window = ELG_WIN_EXPLICIT; e.t_lo_rel = 0.0; e.dt = dt;   // t_lo = t_design + 0
+    return e;
+}
+int32_t hook_check(const elg_bunch* b, double dt, int32_t nb, const char* who) {
+    if (!b || nb < 2 || !(dt > 0.0)) return fail(ELG_EINVAL, std::string(who) + ": bad arguments");
+    if (nb > b->nb_cap) return fail(ELG_ECAPACITY, std::string(who) + ": workspace was sized for fewer bins");
     return ELG_OK;
 }
 }  // namespace
 
-extern "C" int32_t elg_dbg_histogram(const double* d_s, int64_t n, double inv_bc, double t_lo, double inv_dt, int32_t nb,
-                                     uint32_t* d_counts, void* stream) {
-    if (n < 0 || nb < 1 || !d_counts || (n > 0 && !d_s)) return fail(ELG_EINVAL, "elg_dbg_histogram: bad arguments");
-    int grid = 0;
-    { int32_t rc = hist_setup_once(); if (rc != ELG_OK) return rc; }
-    { int32_t rc = grid_for(hist_kernel, 1, kHistSmemBins * 4, kBlock, &grid); if (rc != ELG_OK) return rc; }
-    int sms = 0;
-    { int32_t rc = device_sms(&sms); if (rc != ELG_OK) return rc; }
-    ELG_CK(cudaMemsetAsync(d_counts, 0, (size_t)nb * 4, (cudaStream_t)stream));
-    HistArgs h;
-    h.s = d_s; h.st = nullptr; h.cur = 0; h.n_fixed = n; h.inv_bc = inv_bc; h.t_lo = t_lo; h.inv_dt = inv_dt; h.nb = nb;
-    const char* agg = std::getenv("ELG_HIST_AGGREGATE");
-    h.aggregate = agg ? std::atoi(agg) : 0;
-    h.counts = d_counts;
-    h.smem_bins = kHistSmemBins;
-    hist_kernel<<<grid * sms, kBlock, kHistSmemBins * 4, (cudaStream_t)stream>>>(h);
-    g_launches++;
-    ELG_CK(cudaGetLastError());
+extern "C" int32_t elg_dbg_histogram(elg_bunch* b, double t_lo, double dt, int32_t nb, uint32_t* d_counts) {
+    { int32_t rc = hook_check(b, dt, nb, "elg_dbg_histogram"); if (rc != ELG_OK) return rc; }
+    if (!d_counts) return fail(ELG_EINVAL, "elg_dbg_histogram: NULL output");
+    Tracker t{b, nullptr, nullptr};
+    t.prepare_hist(hook_window_element(dt, nb), t_lo, false);
+    if (!t.ok()) return t.rc;
+    ELG_CK(cudaMemcpyAsync(d_counts, b->counts, (size_t)nb * 4, cudaMemcpyDeviceToDevice, b->stream));
     return ELG_OK;
+}
+
+extern "C" int32_t elg_dbg_dipole_histogram(elg_bunch* b, double t_lo, double dt, int32_t nb, uint32_t* d_counts, double* d_D) {
+    { int32_t rc = hook_check(b, dt, nb, "elg_dbg_dipole_histogram"); if (rc != ELG_OK) return rc; }
+    if (!d_counts || !d_D) return fail(ELG_EINVAL, "elg_dbg_dipole_histogram: NULL output");
+    Tracker t{b, nullptr, nullptr};
+    t.prepare_hist(hook_window_element(dt, nb), t_lo, true);
+    if (!t.ok()) return t.rc;
+    t.dipole_finalize(nb);
+    if (!t.ok()) return t.rc;
+    ELG_CK(cudaMemcpyAsync(d_counts, b->counts, (size_t)nb * 4, cudaMemcpyDeviceToDevice, b->stream));
+    ELG_CK(cudaMemcpyAsync(d_D, b->D, (size_t)nb * 16, cudaMemcpyDeviceToDevice, b->stream));
+    return ELG_OK;
+}
+
+// the wake kick exactly as tracking applies it: OP_KICK / OP_TKICK as a fused run of one op, behind the min/max
+// epilogue and the window kernel that set the device-resident window
+extern "C" int32_t elg_dbg_kick(elg_bunch* b, double t_lo, double dt, int32_t nb, const double* d_V, int32_t interp) {
+    { int32_t rc = hook_check(b, dt, nb, "elg_dbg_kick"); if (rc != ELG_OK) return rc; }
+    if (!d_V) return fail(ELG_EINVAL, "elg_dbg_kick: NULL V");
+    Tracker t{b, nullptr, nullptr};
+    t.flush(AP_NONE, 0, 0, 0, true);
+    t.launch_window(hook_window_element(dt, nb), t_lo, false);
+    if (!t.ok()) return t.rc;
+    ELG_CK(cudaMemcpyAsync(b->V, d_V, (size_t)nb * 8, cudaMemcpyDeviceToDevice, b->stream));
+    t.queue_kick(nb, interp);
+    t.flush(AP_NONE, 0, 0, 0, false);
+    return t.rc;
+}
+
+extern "C" int32_t elg_dbg_tkick(elg_bunch* b, double t_lo, double dt, int32_t nb, const double* d_Vx, const double* d_Vy,
+                                 int32_t interp) {
+    { int32_t rc = hook_check(b, dt, nb, "elg_dbg_tkick"); if (rc != ELG_OK) return rc; }
+    if (!d_Vx || !d_Vy) return fail(ELG_EINVAL, "elg_dbg_tkick: NULL V");
+    Tracker t{b, nullptr, nullptr};
+    t.flush(AP_NONE, 0, 0, 0, true);
+    t.launch_window(hook_window_element(dt, nb), t_lo, false);
+    if (!t.ok()) return t.rc;
+    ELG_CK(cudaMemcpyAsync(b->Vt, d_Vx, (size_t)nb * 8, cudaMemcpyDeviceToDevice, b->stream));
+    ELG_CK(cudaMemcpyAsync(b->Vt + nb, d_Vy, (size_t)nb * 8, cudaMemcpyDeviceToDevice, b->stream));
+    t.queue_tkick(nb, interp);
+    t.flush(AP_NONE, 0, 0, 0, false);
+    return t.rc;
+}
+
+// aperture + stable compaction alone: a run of zero maps ending in the aperture (PAPER.md:141 loss contract)
+extern "C" int32_t elg_dbg_compact(elg_bunch* b, int32_t type, double ax, double ay) {
+    if (!b || (type != ELG_RCOL && type != ELG_ECOL) || !(ax > 0.0) || !(ay > 0.0))
+        return fail(ELG_EINVAL, "elg_dbg_compact: bad arguments");
+    Tracker t{b, nullptr, nullptr};
+    const bool rect = type == ELG_RCOL;
+    t.flush(rect ? AP_RCOL : AP_ECOL, rect ? ax : 1.0 / ax, rect ? ay : 1.0 / ay, (b->turn << 32), false);
+    return t.rc;
 }
 
 extern "C" int32_t elg_dbg_wake_samples(int32_t kind, int32_t nb, double dt, double f, double Q, double Rs,
@@ -1235,17 +1303,6 @@ extern "C" int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W,
     ConvArgs<unsigned int> cv;
     cv.counts = d_counts; cv.W = d_W; cv.st = nullptr; cv.nb = nb; cv.q = q; cv.V = d_V;
     conv_kernel<unsigned int><<<(nb + kWarps - 1) / kWarps, kBlock, 0, (cudaStream_t)stream>>>(cv);
-    g_launches++;
-    ELG_CK(cudaGetLastError());
-    return ELG_OK;
-}
-
-extern "C" int32_t elg_dbg_kick(const double* d_s, double* d_delta, int64_t n, double inv_bc, double t_lo, double inv_dt,
-                                int32_t nb, const double* d_V, double inv_E, int32_t interp, void* stream) {
-    if (n < 0 || nb < 1 || !d_V || (n > 0 && (!d_s || !d_delta))) return fail(ELG_EINVAL, "elg_dbg_kick: bad arguments");
-    int grid = 0;
-    { int32_t rc = hook_grid(&grid, 8); if (rc != ELG_OK) return rc; }
-    kick_kernel<<<grid, kBlock, 0, (cudaStream_t)stream>>>(d_s, d_delta, n, inv_bc, t_lo, inv_dt, nb, d_V, inv_E, interp);
     g_launches++;
     ELG_CK(cudaGetLastError());
     return ELG_OK;

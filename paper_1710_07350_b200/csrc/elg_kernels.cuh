@@ -7,8 +7,8 @@
 // from a sequential CPU evaluation.
 //
 // Kernels (one section each):
-//   chain_kernel<MAXOPS, COMPACT>  fused run of element maps; COMPACT ends in an aperture and a stable
-//                                  single-pass (decoupled look-back) stream compaction
+//   chain_kernel, chain_long_kernel    fused run of element maps (short runs / long fp64-bound runs)
+//   compact_kernel                 fused run ending in an aperture + stable single-pass stream compaction
 //   window_kernel                  min/max partials -> histogram window + occupied bin range, zero counts
 //   hist_kernel                    shared-memory privatised time histogram
 //   wake_samples_kernel, conv_kernel   wake function samples and causal convolution
@@ -334,23 +334,47 @@ __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, 
     }
 }
 
-// EXT = false leaves out the rarely used maps (MATRIX2, TKICK): the HBM-bound short kernels stay at 62 registers
+// EXT = false leaves out the rarely used maps (MATRIX2, TKICK): the HBM-bound short kernels stay at ~60 registers
 // (4 blocks per SM); the planner picks the EXT = true instantiation when a run holds one of them.
+// Without the rarely used maps the loop over the MAXOPS parameter slots is fully unrolled, so every coefficient has a
+// compile-time offset in the constant bank and reaches its DFMA as a uniform-register operand (LDCU + DFMA R, R, UR, R):
+// no per-coefficient LDC through the MIO (profiles/r01d: 6 -> 53 DFMA/clk/SM at two particles per thread in a
+// register-only loop).  Only the slots a run uses are ever fetched, so the larger code does not cost instruction cache.
 template <int MAXOPS, int P, bool EXT>
 __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
-    for (int op = 0; op < a.c.n_ops; op++) {
-        const double* c = a.coef[op];
-        const int ty = a.type[op];
-        if (ty == OP_MATRIX || (EXT && ty == OP_MATRIX2)) {
-            double w[P][6];
-            matrix_map<P>(c, v, w);
-            if (EXT && ty == OP_MATRIX2) { matrix2_terms<P>(c + 42, v, w); op += 3; }
+    const int n_ops = a.c.n_ops;
+    if constexpr (!EXT) {
 #pragma unroll
-            for (int p = 0; p < P; p++)
+        for (int op = 0; op < MAXOPS; op++) {
+            if (op >= n_ops) break;
+            const double* c = a.coef[op];
+            const int ty = a.type[op];
+            if (ty == OP_MATRIX) {
+                double w[P][6];
+                matrix_map<P>(c, v, w);
 #pragma unroll
-                for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
-        } else {
-            other_map<P, EXT>(ty, c, a.c, v);
+                for (int p = 0; p < P; p++)
+#pragma unroll
+                    for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+            } else {
+                other_map<P, false>(ty, c, a.c, v);
+            }
+        }
+    } else {                                                     // with the second-order code per slot the unrolled form spills
+        for (int op = 0; op < n_ops; op++) {
+            const double* c = a.coef[op];
+            const int ty = a.type[op];
+            if (ty == OP_MATRIX || ty == OP_MATRIX2) {
+                double w[P][6];
+                matrix_map<P>(c, v, w);
+                if (ty == OP_MATRIX2) { matrix2_terms<P>(c + 42, v, w); op += 3; }
+#pragma unroll
+                for (int p = 0; p < P; p++)
+#pragma unroll
+                    for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+            } else {
+                other_map<P, true>(ty, c, a.c, v);
+            }
         }
     }
 }
@@ -525,6 +549,37 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// mbarrier + 1-D bulk copy (TMA unit, SASS UBLKCP): global -> shared without registers or L1, completion counted in bytes
+__device__ __forceinline__ unsigned int smem_u32(const void* p) { return (unsigned int)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned int bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned int parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "MBAR_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra MBAR_DONE_%=;\n"
+        "bra MBAR_WAIT_%=;\n"
+        "MBAR_DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, unsigned int bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+template <int ID, int N>
+__device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(N) : "memory"); }
+
 template <int MAXOPS, int LEVEL>
 constexpr int chain_long_smem_bytes() { return MAXOPS * 42 * 8 + 6 * kBlock * long_pl(LEVEL) * 8; }
 
@@ -620,183 +675,236 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
 // ---------------------------------------------------------------------------------------------------
 // compact_kernel: a run of maps that ends in an aperture (a6) followed by the stable stream compaction
 // (a7; north_star part 2): survivors are written out of place in their original order, lost particles
-// are appended to the lost log in position order.  Single pass over HBM: survivor ranks come from a
-// decoupled look-back scan over 512-particle tiles.  The grid is persistent and launched cooperatively
-// (every block resident), tiles are dealt round-robin, so a tile's predecessors always make progress.
+// are appended to the lost log in position order.  Single pass over HBM (56 B read + 56 B written per
+// live particle).  The grid is persistent and launched cooperatively (every block resident); tiles of
+// TILE = NT x PP particles are dealt round-robin, iteration i of block b works on tile b + i x gridDim.
 //
-// What made the first version latency-bound (profiles/r01b: 37 % of the HBM peak, 10 us per tile) and
-// what this one does about it (profiles/r01d_long_chain_and_compaction.md).  Under streaming load every global round
-// trip costs 2-3 us, and ticket atomic -> load -> aggregate -> look-back windows -> prefix were 5+ of them
-// in series per tile:
-//   * no ticket: tiles are dealt round-robin, so the next tile is known and is cp.async'd into shared
-//     memory while the current one is scanned and stored;
-//   * no chained look-back: a block keeps its own inclusive prefix from its previous tile and adds the
-//     aggregates of the gridDim.x - 1 tiles in between, all 256 threads polling their share at once: one
-//     round trip, and no block ever waits for another block's look-back, only for its count;
-//   * thread t owns particles t and t + 256 of the tile, so survivors of consecutive lanes have consecutive
-//     ranks: the stores from registers are dense 256-byte warp accesses without a shared-memory partition;
-//   * 64 registers: four blocks (32 warps) per SM.
+// A tile lives in one stage of a shared-memory ring of S stages from its arrival to the moment its survivors
+// leave for global memory; registers hold a particle only while it is mapped.
+//   producer warp (one lane): waits until a stage has been released (mbarrier, NT arrivals) and refills it with
+//       seven 1-D bulk copies (TMA unit, cp.async.bulk, completion counted in bytes on the stage's "full"
+//       mbarrier): the load stream runs F = S - D - 1 tiles ahead of the compute warps, uses no registers, no
+//       L1 and seven instructions per tile, and never waits for the scan;
+//   compute warps, iteration i:
+//   (a) the status words needed for the base of the tile of iteration i - D are requested;
+//   (b) wait for tile i (mbarrier try_wait on its stage);
+//   (c) every thread loads its PP particles (slots t + q NT), applies the run's maps (coefficients as uniform
+//       operands from the parameter bank) and evaluates the aperture;
+//   (d) ranks: one __ballot_sync + __popc per sub-tile (the flags are single bits; the lanes of a warp hold
+//       consecutive particles), warp totals to shared memory; the polled status words are summed per warp here
+//       too, so that ONE named barrier per tile serves both;
+//   (e) the tile's survivor count is published at once as a 64-bit status word (epoch | flag | count);
+//   (f) the mapped particles are scattered back INTO THE SAME STAGE in compacted order: survivors to slots
+//       [0, total), lost ones to [total, valid);
+//   (g) the tile of iteration i - D has its base by now (own inclusive prefix one tile earlier + the
+//       gridDim - 1 aggregates in between, no chained look-back; D = 2 iterations of slack keep the chain
+//       "publish <- poll <- publish" of the blocks from ever stalling: D = 1 costs 25 %); thread t copies
+//       slots t + m NT of that stage to dst[base + slot]: dense 256-byte warp stores; slots past the survivors
+//       go to the lost log at n_lost + (index - survivors before); then the stage is released.
+// Measured variants (tile sizes, ring depths, per-thread cp.async instead of bulk copies, round 1's
+// register-held tile): profiles/r02_compact.md.
 // ---------------------------------------------------------------------------------------------------
-#ifndef ELG_COMPACT_BLOCKS
-#define ELG_COMPACT_BLOCKS 2
+#ifndef ELG_C2_NT
+#define ELG_C2_NT 256
 #endif
-constexpr int kPoll = 3;                                // status words per thread and tile: grids up to 3 * 256 + 1 blocks
-constexpr int kCompactMaxGrid = kPoll * kBlock + 1;
+#ifndef ELG_C2_PP
+#define ELG_C2_PP 2
+#endif
+#ifndef ELG_C2_S
+#define ELG_C2_S 4
+#endif
+#ifndef ELG_C2_D
+#define ELG_C2_D 2
+#endif
+#ifndef ELG_C2_BLOCKS
+#define ELG_C2_BLOCKS 2
+#endif
+constexpr int kC2NT = ELG_C2_NT;                        // compute threads per block
+constexpr int kC2PP = ELG_C2_PP;                        // particles per thread and tile
+constexpr int kC2S = ELG_C2_S;                          // ring stages
+constexpr int kC2D = ELG_C2_D;                          // a tile's base is resolved D iterations after its count
+constexpr int kC2Tile = kC2NT * kC2PP;
+constexpr int kC2Threads = kC2NT + 32;                  // + the producer warp
+constexpr int kPoll = 3;                                // status words per thread and tile
+constexpr int kCompactMaxGrid = kPoll * kC2NT + 1;
+constexpr int kStatusTile = 256;                        // tile_status is sized for tiles of at least this many particles
+constexpr int compact_smem_bytes() { return kC2S * 7 * kC2Tile * 8; }
 
 template <int MAXOPS, bool EXT>
-__global__ void __launch_bounds__(kBlock, ELG_COMPACT_BLOCKS) compact_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+__global__ void __launch_bounds__(kC2Threads, ELG_C2_BLOCKS) compact_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+    constexpr int NT = kC2NT, PP = kC2PP, S = kC2S, D = kC2D, TILE = kC2Tile, NW = NT / 32;
+    static_assert(D >= 1 && S - D - 1 >= 0, "ring: S = D + F + 1");
+    static_assert(kC2Tile >= kStatusTile && kC2Tile % 2 == 0, "tile_status capacity; 16-byte bulk copies");
     const ChainCommon& c = a.c;
     const long long n = c.st->n_alive[c.cur];
-    const long long n_tiles = (n + kTile - 1) / kTile;
+    const long long n_tiles = (n + TILE - 1) / TILE;
     const long long lost_base = c.st->n_lost[c.cur];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned int lt_mask = (1u << lane) - 1u;
     double mn = INFINITY, mx = -INFINITY;
 
-    __shared__ __align__(16) double s_in[7][kTile];              // next tile, cp.async'd: thread t owns [.][t], [.][t + kBlock]
-    __shared__ int s_wtot[kWarps];                               // per warp: survivors of sub-tile 0 | sub-tile 1 << 16
-    __shared__ unsigned int s_part[kWarps];
+    extern __shared__ __align__(16) double c2_ring[];           // [S][7][TILE]; row 6 holds the IDs (bit patterns)
+    __shared__ int s_wtot[2][PP][NW];                            // per iteration parity, sub-tile, warp: survivors
+    __shared__ unsigned int s_part[2][NW];                       // per iteration parity, warp: polled aggregates
+    __shared__ unsigned long long s_full[S], s_empty[S];         // mbarriers: tile landed / stage released by all readers
 
-    auto prefetch = [&](long long tile) {                        // 8-byte copies of exactly the elements this thread reads
+    const long long G = gridDim.x;
+    const long long n_it = (n_tiles > blockIdx.x) ? (n_tiles - blockIdx.x + G - 1) / G : 0;     // my tiles
+
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < S; k++) { mbar_init(&s_full[k], 1); mbar_init(&s_empty[k], NT); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (wid == NW) {                                             // producer warp: one lane feeds the ring
+        if (lane == 0) {
+            for (long long it = 0; it < n_it; it++) {
+                const int stg = (int)(it % S);
+                const long long use = it / S;
+                if (use > 0) mbar_wait(&s_empty[stg], (unsigned int)((use - 1) & 1));
+                const long long tile = blockIdx.x + it * G;
+                const long long left = n - tile * TILE;
+                // whole 16-byte units; an odd tail reads one element past n, inside the array's 256-byte padding
+                const unsigned int bytes = (unsigned int)(((left < TILE ? left : TILE) + 1) / 2) * 16u;
+                double* stage = c2_ring + (size_t)stg * 7 * TILE;
+                mbar_expect_tx(&s_full[stg], 7u * bytes);
 #pragma unroll
-        for (int q = 0; q < 2; q++) {
-            const long long i = tile * kTile + threadIdx.x + q * kBlock;
-            const int bytes = i < n ? 8 : 0;                     // zero-fill past the live prefix
-            const long long is = i < n ? i : 0;
-#pragma unroll
-            for (int cc = 0; cc < 6; cc++) cp_async8(&s_in[cc][threadIdx.x + q * kBlock], c.src[cc] + is, bytes);
-            cp_async8(&s_in[6][threadIdx.x + q * kBlock], c.id_src + is, bytes);
+                for (int cc = 0; cc < 6; cc++) bulk_g2s(stage + cc * TILE, c.src[cc] + tile * TILE, bytes, &s_full[stg]);
+                bulk_g2s(stage + 6 * TILE, c.id_src + tile * TILE, bytes, &s_full[stg]);
+            }
         }
-    };
+        return;
+    }
 
-    // the tile counted in the previous iteration, held in registers until its base is known
-    double pv[2][6];
-    long long pid[2] = {0, 0};
-    bool pok[2] = {false, false}, psurv[2] = {false, false};
-    int prank[2] = {0, 0}, ptotal = 0;
-    long long ptile = -1;                                        // -1: nothing held
-    long long my_incl = 0, pptile = -1;                          // inclusive prefix at this block's tile before ptile
+    int tot_hist[D];                                             // survivor counts of the last D counted tiles
 #pragma unroll
-    for (int q = 0; q < 2; q++)
-#pragma unroll
-        for (int cc = 0; cc < 6; cc++) pv[q][cc] = 0.0;
+    for (int d = 0; d < D; d++) tot_hist[d] = 0;
+    long long my_incl = 0;                                       // inclusive survivor prefix at my last resolved tile
 
-    long long tile = blockIdx.x;                                 // static round-robin tiles: the launch is cooperative,
-    if (tile < n_tiles) prefetch(tile);                          // every block is resident, predecessors always progress
-    for (;; tile += gridDim.x) {
-        const bool cur_valid = tile < n_tiles;
-        // (0) the aggregates between this block's last two tiles were published an iteration ago: request them
-        //     now, they arrive while the current tile is counted
+    for (long long it = 0; it < n_it + D; it++) {
+        const int par = (int)(it & 1);
+        const long long r = it - D;                              // the iteration whose tile is resolved and stored now
+        const bool cur_valid = it < n_it, res_valid = r >= 0 && r < n_it;
+        const long long rtile = blockIdx.x + r * G;              // (only meaningful when res_valid)
+
+        // (a) aggregates between my previous tile and tile r, published at least D - 1 iterations ago
         unsigned long long stt[kPoll];
+        const long long first = (r > 0) ? rtile - G + 1 : 0;     // tiles [first, rtile)
 #pragma unroll
         for (int j = 0; j < kPoll; j++) {
-            const long long w = pptile + 1 + threadIdx.x + j * kBlock;
-            stt[j] = (ptile >= 0 && w < ptile) ? ld_relaxed(c.tile_status + w) : pack_status(c.epoch, kFlagA, 0);
+            const long long w = first + threadIdx.x + j * NT;
+            stt[j] = (res_valid && w < rtile) ? ld_relaxed(c.tile_status + w) : pack_status(c.epoch, kFlagA, 0);
         }
 
-        double v[2][6];
-        long long id[2];
-        bool ok[2] = {false, false}, surv[2] = {false, false};
-        int rank[2] = {0, 0}, total = 0;
+        int total = 0;
+        bool ok[PP], surv[PP];
+        double v[PP][6];
+        long long id[PP];
+        unsigned int bal[PP];
+        double* stage = c2_ring + (size_t)(it % S) * 7 * TILE;
         if (cur_valid) {
-            const long long i0 = tile * kTile + threadIdx.x;     // my particles: i0 and i0 + kBlock
-            cp_async_wait_all();
+            const long long tile = blockIdx.x + it * G;
+            mbar_wait(&s_full[it % S], (unsigned int)((it / S) & 1));    // (b)
 #pragma unroll
-            for (int q = 0; q < 2; q++) {
-                ok[q] = i0 + q * kBlock < n;
+            for (int q = 0; q < PP; q++) {                       // (c)
+                const int slot = threadIdx.x + q * NT;
+                ok[q] = tile * TILE + slot < n;                  // slots past n hold stale bytes: never used
 #pragma unroll
-                for (int cc = 0; cc < 6; cc++) v[q][cc] = s_in[cc][threadIdx.x + q * kBlock];
-                id[q] = __double_as_longlong(s_in[6][threadIdx.x + q * kBlock]);
+                for (int cc = 0; cc < 6; cc++) v[q][cc] = stage[cc * TILE + slot];
+                id[q] = __double_as_longlong(stage[6 * TILE + slot]);
             }
-            if (tile + gridDim.x < n_tiles) prefetch(tile + gridDim.x);   // streams in during this iteration
-
-            apply_ops<MAXOPS, 2, EXT>(a, v);  // short run: coefficients straight from the parameter bank
-
+            apply_ops<MAXOPS, PP, EXT>(a, v);
 #pragma unroll
-            for (int q = 0; q < 2; q++) surv[q] = ok[q] && survives(c.ap_type, c.ap_x, c.ap_y, v[q][0], v[q][2]);
-            const int cnt = (int)surv[0] | ((int)surv[1] << 16);
-            int inc = cnt;                                       // warp inclusive scan of both sub-tiles at once
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const int t = __shfl_up_sync(0xffffffffu, inc, d);
-                if (lane >= d) inc += t;
+            for (int q = 0; q < PP; q++) {                       // (d)
+                surv[q] = ok[q] && survives(c.ap_type, c.ap_x, c.ap_y, v[q][0], v[q][2]);
+                bal[q] = __ballot_sync(0xffffffffu, surv[q]);
+                if (lane == 0) s_wtot[par][q][wid] = __popc(bal[q]);
             }
-            if (lane == 31) s_wtot[wid] = inc;
-            __syncthreads();                                     // (A) warp totals visible
-            int before = 0, all = 0;
-#pragma unroll
-            for (int w = 0; w < kWarps; w++) {
-                const int x = s_wtot[w];
-                if (w < wid) before += x;
-                all += x;
-            }
-            const int total0 = all & 0xffff;
-            total = total0 + (all >> 16);
-            if (threadIdx.x == 0 && tile + 1 < n_tiles)          // published at count time: nobody waits for more than a count
-                st_relaxed(c.tile_status + tile, pack_status(c.epoch, kFlagA, (unsigned long long)total));
-            const int ex = inc - cnt;                            // survivors before me in my warp, both sub-tiles
-            rank[0] = (before & 0xffff) + (ex & 0xffff);
-            rank[1] = total0 + (before >> 16) + (ex >> 16);
-        } else {
-#pragma unroll
-            for (int q = 0; q < 2; q++)
-#pragma unroll
-                for (int cc = 0; cc < 6; cc++) v[q][cc] = 0.0;
-            id[0] = 0; id[1] = 0;
         }
-
-        if (ptile >= 0) {
-            // (1) survivors before the held tile = own inclusive prefix one tile earlier + the aggregates in between
+        if (res_valid) {                                         // the polled aggregates, summed per warp
             unsigned int part = 0;
 #pragma unroll
             for (int j = 0; j < kPoll; j++) {
-                const long long w = pptile + 1 + threadIdx.x + j * kBlock;
-                if (w < ptile) {
+                const long long w = first + threadIdx.x + j * NT;
+                if (w < rtile) {
                     while ((unsigned int)(stt[j] >> 34) != c.epoch || ((stt[j] >> 32) & 3ull) == 0) stt[j] = ld_relaxed(c.tile_status + w);
                     part += (unsigned int)(stt[j] & 0xffffffffull);
                 }
             }
             part = __reduce_add_sync(0xffffffffu, part);
-            if (lane == 0) s_part[wid] = part;
-            __syncthreads();                                     // (B) partial sums visible
+            if (lane == 0) s_part[par][wid] = part;
+        }
+        named_barrier<1, NT>();                                  // the one barrier per tile (compute warps): stage read by all, totals visible
+
+        if (cur_valid) {
+            const long long tile = blockIdx.x + it * G;
+            int before[PP];                                      // survivors before my warp's part of sub-tile q
+#pragma unroll
+            for (int q = 0; q < PP; q++) {
+                int sub = 0, mine = 0;
+#pragma unroll
+                for (int w = 0; w < NW; w++) {
+                    const int x = s_wtot[par][q][w];
+                    if (w < wid) mine += x;
+                    sub += x;
+                }
+                before[q] = total + mine;
+                total += sub;
+            }
+            if (threadIdx.x == 0 && tile + 1 < n_tiles)          // (e)
+                st_relaxed(c.tile_status + tile, pack_status(c.epoch, kFlagA, (unsigned long long)total));
+#pragma unroll
+            for (int q = 0; q < PP; q++) {                       // (f) compacted order inside the stage
+                const int slot = threadIdx.x + q * NT;
+                const int rank = before[q] + __popc(bal[q] & lt_mask);
+                const int pos = surv[q] ? rank : total + (slot - rank);
+                if (ok[q]) {
+#pragma unroll
+                    for (int cc = 0; cc < 6; cc++) stage[cc * TILE + pos] = v[q][cc];
+                    stage[6 * TILE + pos] = __longlong_as_double(id[q]);
+                    if (c.want_minmax && surv[q]) { mn = fmin(mn, v[q][4]); mx = fmax(mx, v[q][4]); }
+                }
+            }
+        }
+
+        if (res_valid) {                                         // (g)
             long long base = my_incl;
 #pragma unroll
-            for (int w = 0; w < kWarps; w++) base += s_part[w];
-            my_incl = base + ptotal;
-            pptile = ptile;
-            if (ptile == n_tiles - 1 && threadIdx.x == 0) {      // the last tile knows the totals
+            for (int w = 0; w < NW; w++) base += s_part[par][w];
+            const int rtotal = tot_hist[D - 1];
+            my_incl = base + rtotal;
+            if (rtile == n_tiles - 1 && threadIdx.x == 0) {      // the last tile knows the totals
                 c.st->n_alive[c.cur ^ 1] = my_incl;
                 c.st->n_lost[c.cur ^ 1] = lost_base + (n - my_incl);
             }
-            const long long lost0 = lost_base + (ptile * kTile - base);      // lost before the tile = index - survivors before
+            const long long left = n - rtile * TILE;
+            const int rvalid = left < TILE ? (int)left : TILE;
+            const long long lost0 = lost_base + (rtile * TILE - base);       // lost before the tile = index - survivors before
+            const double* rs = c2_ring + (size_t)(r % S) * 7 * TILE;
 #pragma unroll
-            for (int q = 0; q < 2; q++) {
-                if (psurv[q]) {
-                    const long long d = base + prank[q];
+            for (int m = 0; m < PP; m++) {
+                const int slot = threadIdx.x + m * NT;
+                if (slot < rtotal) {
+                    const long long d = base + slot;
 #pragma unroll
-                    for (int cc = 0; cc < 6; cc++) c.dst[cc][d] = pv[q][cc];
-                    c.id_dst[d] = pid[q];
-                    if (c.want_minmax) { mn = fmin(mn, pv[q][4]); mx = fmax(mx, pv[q][4]); }
-                } else if (pok[q]) {
-                    const long long lpos = lost0 + ((int)threadIdx.x + q * kBlock - prank[q]);
+                    for (int cc = 0; cc < 6; cc++) c.dst[cc][d] = rs[cc * TILE + slot];
+                    c.id_dst[d] = __double_as_longlong(rs[6 * TILE + slot]);
+                } else if (slot < rvalid) {
+                    const long long lpos = lost0 + (slot - rtotal);
                     if (lpos < c.lost_cap) {
-                        c.lost_id[lpos] = pid[q];
+                        c.lost_id[lpos] = __double_as_longlong(rs[6 * TILE + slot]);
                         c.lost_te[lpos] = c.te_code;
 #pragma unroll
-                        for (int cc = 0; cc < 6; cc++) c.lost_v[cc * c.lost_cap + lpos] = pv[q][cc];
+                        for (int cc = 0; cc < 6; cc++) c.lost_v[cc * c.lost_cap + lpos] = rs[cc * TILE + slot];
                     }
                 }
             }
-            __syncthreads();                                     // s_part free before the next iteration's (B)
+            fence_proxy_async();                                 // my generic-proxy accesses before the next bulk write
+            mbar_arrive(&s_empty[r % S]);                        // stage released (NT arrivals complete the phase)
         }
-        if (!cur_valid) break;
 #pragma unroll
-        for (int q = 0; q < 2; q++) {                            // hold the counted tile
-#pragma unroll
-            for (int cc = 0; cc < 6; cc++) pv[q][cc] = v[q][cc];
-            pid[q] = id[q]; pok[q] = ok[q]; psurv[q] = surv[q]; prank[q] = rank[q];
-        }
-        ptotal = total;
-        ptile = tile;
+        for (int d = D - 1; d > 0; d--) tot_hist[d] = tot_hist[d - 1];
+        tot_hist[0] = total;
     }
 
     if (c.want_minmax) {                                         // exact min/max of s over the survivors (a8)
@@ -805,11 +913,11 @@ __global__ void __launch_bounds__(kBlock, ELG_COMPACT_BLOCKS) compact_kernel(con
             mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, d));
             mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
         }
-        __shared__ double s_mn[kWarps], s_mx[kWarps];
+        __shared__ double s_mn[NW], s_mx[NW];
         if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
-        __syncthreads();
+        named_barrier<1, NT>();
         if (threadIdx.x == 0) {
-            for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
+            for (int w = 1; w < NW; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
             c.mm_partial[2 * blockIdx.x] = mn;
             c.mm_partial[2 * blockIdx.x + 1] = mx;
         }
@@ -1266,35 +1374,6 @@ __global__ void __launch_bounds__(kBlock) conv_rec_kernel(const ConvRecArgs a) {
         const double tr = Sr + c, ti = Si;
         Sr = fma(zr, tr, -(zi * ti));
         Si = fma(zr, ti, zi * tr);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------
-// kick_kernel: test hook for a12 on caller-supplied arrays (the tracking path applies the kick as the
-// first op of the next fused run, OP_KICK above; same arithmetic).
-// ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kBlock) kick_kernel(const double* s, double* delta, long long n, double inv_bc,
-                                                      double t_lo, double inv_dt, int nb, const double* V,
-                                                      double inv_E, int interp) {
-    const long long stride = (long long)gridDim.x * kBlock;
-    for (long long i = (long long)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) {
-        double u0;
-        const int b = bin_of(s[i], inv_bc, t_lo, inv_dt, nb, &u0);
-        if (b < 0) continue;
-        double Vt;
-        if (!interp || nb < 2) Vt = V[b];
-        else {
-            const double u = u0 - 0.5;
-            double k = floor(u);
-            if (k < 0.0) k = 0.0;
-            if (k > (double)(nb - 2)) k = (double)(nb - 2);
-            double fr = u - k;
-            if (fr < 0.0) fr = 0.0;
-            if (fr > 1.0) fr = 1.0;
-            const int ki = (int)k;
-            Vt = fma(fr, V[ki + 1] - V[ki], V[ki]);
-        }
-        delta[i] = fma(-Vt, inv_E, delta[i]);
     }
 }
 

@@ -34,7 +34,8 @@ EXPORTS = (
     "elg_upload_and_track",
     "elg_moments", "elg_lost", "elg_n_alive", "elg_bunch_read", "elg_bunch_device_array",
     "elg_profile_enable", "elg_profile_read",
-    "elg_dbg_histogram", "elg_dbg_wake_samples", "elg_dbg_convolve", "elg_dbg_kick",
+    "elg_dbg_histogram", "elg_dbg_dipole_histogram", "elg_dbg_kick", "elg_dbg_tkick", "elg_dbg_compact",
+    "elg_dbg_wake_samples", "elg_dbg_convolve",
 )
 KERNEL_KINDS = ("chain", "chain_compact", "window", "hist", "wake_samples", "conv", "moments", "chain_long")
 
@@ -70,22 +71,18 @@ _lib = None
 
 
 def lib():
-    """Load libelg.so (building it with nvcc if it is stale).  Fails loudly if that is impossible."""
+    """Load libelg.so (building it with nvcc if it does not match the sources).  Fails loudly if that is impossible."""
     global _lib
     if _lib is not None:
         return _lib
-    path = LIB
-    if os.environ.get("ELG_LIB"):                       # a tuning variant built with build(out=..., extra=...)
+    if os.environ.get("ELG_LIB"):                       # an explicitly named tuning variant (build(out=..., extra=...))
         path = os.environ["ELG_LIB"]
         if not os.path.exists(path):
             raise RuntimeError(f"ELG_LIB={path} does not exist")
-    elif not os.path.exists(path) or os.environ.get("ELG_REBUILD"):
-        path = build()
     else:
-        try:
-            path = build()          # no-op when up to date
-        except Exception:
-            pass                    # no nvcc on this box: use the shipped library
+        # current by content hash: load it; otherwise rebuild.  A compile error or a missing compiler propagates --
+        # a library that does not match the sources is never loaded silently.
+        path = build(force=bool(os.environ.get("ELG_REBUILD")))
     L = C.CDLL(path)
     v6 = _dp * 6
     vp = C.c_void_p
@@ -119,15 +116,16 @@ def lib():
     L.elg_bunch_device_array.argtypes = [vp, C.c_int32, C.POINTER(vp)]; L.elg_bunch_device_array.restype = C.c_int32
     L.elg_profile_enable.argtypes = [vp, C.c_int32]; L.elg_profile_enable.restype = C.c_int32
     L.elg_profile_read.argtypes = [vp, _i64p, _dp]; L.elg_profile_read.restype = C.c_int32
-    L.elg_dbg_histogram.argtypes = [vp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32, vp, vp]
-    L.elg_dbg_histogram.restype = C.c_int32
+    L.elg_dbg_histogram.argtypes = [vp, C.c_double, C.c_double, C.c_int32, vp]; L.elg_dbg_histogram.restype = C.c_int32
+    L.elg_dbg_dipole_histogram.argtypes = [vp, C.c_double, C.c_double, C.c_int32, vp, vp]
+    L.elg_dbg_dipole_histogram.restype = C.c_int32
+    L.elg_dbg_kick.argtypes = [vp, C.c_double, C.c_double, C.c_int32, vp, C.c_int32]; L.elg_dbg_kick.restype = C.c_int32
+    L.elg_dbg_tkick.argtypes = [vp, C.c_double, C.c_double, C.c_int32, vp, vp, C.c_int32]; L.elg_dbg_tkick.restype = C.c_int32
+    L.elg_dbg_compact.argtypes = [vp, C.c_int32, C.c_double, C.c_double]; L.elg_dbg_compact.restype = C.c_int32
     L.elg_dbg_wake_samples.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
                                        vp, C.c_int64, C.c_double, vp, vp]
     L.elg_dbg_wake_samples.restype = C.c_int32
     L.elg_dbg_convolve.argtypes = [vp, vp, C.c_int32, C.c_double, vp, vp]; L.elg_dbg_convolve.restype = C.c_int32
-    L.elg_dbg_kick.argtypes = [vp, vp, C.c_int64, C.c_double, C.c_double, C.c_double, C.c_int32, vp,
-                               C.c_double, C.c_int32, vp]
-    L.elg_dbg_kick.restype = C.c_int32
     _lib = L
     return L
 
@@ -434,13 +432,72 @@ class Bunch:
 
 
 # ------------------------------------------------------------------------------- single-stage hooks
-def dbg_histogram(s, inv_bc: float, t_lo: float, inv_dt: float, nb: int) -> np.ndarray:
+def _stage_bunch(coords, p0c_eV: float, nb: int, charge_C: float = 1e-9) -> "Bunch":
+    """A bunch holding the ORACLE's input of one stage (coords (6, n)), its workspace sized for nb bins."""
+    sizing = Beamline([{"type": "HISTO", "nb": int(nb), "window": "EXPLICIT", "dt": 1.0}])
+    return Bunch(_f64(coords), p0c_eV, charge_C, beamline=sizing, lost_capacity=int(np.shape(coords)[1]))
+
+
+def _coords_from(n: int, **rows) -> np.ndarray:
+    v = np.zeros((6, n), dtype=np.float64)
+    for name, a in rows.items():
+        v[{"x": 0, "xp": 1, "y": 2, "yp": 3, "s": 4, "delta": 5}[name]] = a
+    return v
+
+
+def dbg_histogram(s, p0c_eV: float, t_lo: float, dt: float, nb: int) -> np.ndarray:
+    """elg_dbg_histogram on a bunch whose s coordinates are `s`: tracking's own epilogue + window + hist kernels."""
     torch = _torch()
-    d_s = torch.as_tensor(_f64(s), device="cuda")
-    d_c = torch.empty(nb, dtype=torch.int32, device="cuda")
-    st = torch.cuda.current_stream().cuda_stream
-    _ck(lib().elg_dbg_histogram(d_s.data_ptr(), d_s.numel(), inv_bc, t_lo, inv_dt, nb, d_c.data_ptr(), st))
+    s = _f64(s)
+    b = _stage_bunch(_coords_from(s.size, s=s), p0c_eV, nb)
+    d_c = torch.empty(nb, dtype=torch.int32, device=b.device)
+    _ck(lib().elg_dbg_histogram(b._h, t_lo, dt, nb, d_c.data_ptr()))
+    b.synchronize()
     return d_c.cpu().numpy().view(np.uint32)
+
+
+def dbg_dipole_histogram(s, x, y, p0c_eV: float, t_lo: float, dt: float, nb: int):
+    torch = _torch()
+    s = _f64(s)
+    b = _stage_bunch(_coords_from(s.size, s=s, x=x, y=y), p0c_eV, nb)
+    d_c = torch.empty(nb, dtype=torch.int32, device=b.device)
+    d_D = torch.empty(2 * nb, dtype=torch.float64, device=b.device)
+    _ck(lib().elg_dbg_dipole_histogram(b._h, t_lo, dt, nb, d_c.data_ptr(), d_D.data_ptr()))
+    b.synchronize()
+    D = d_D.cpu().numpy()
+    return d_c.cpu().numpy().view(np.uint32), D[:nb], D[nb:]
+
+
+def dbg_kick(s, delta, p0c_eV: float, t_lo: float, dt: float, nb: int, V, interp=True) -> np.ndarray:
+    """elg_dbg_kick: OP_KICK as a fused run of one op on a bunch holding (s, delta); returns delta."""
+    torch = _torch()
+    s = _f64(s)
+    b = _stage_bunch(_coords_from(s.size, s=s, delta=delta), p0c_eV, nb)
+    d_V = torch.as_tensor(_f64(V), device=b.device)
+    _ck(lib().elg_dbg_kick(b._h, t_lo, dt, nb, d_V.data_ptr(), 1 if interp else 0))
+    b.synchronize()
+    return b.device_array(5)[: s.size].cpu().numpy()
+
+
+def dbg_tkick(s, xp, yp, p0c_eV: float, t_lo: float, dt: float, nb: int, Vx, Vy, interp=True):
+    torch = _torch()
+    s = _f64(s)
+    b = _stage_bunch(_coords_from(s.size, s=s, xp=xp, yp=yp), p0c_eV, nb)
+    d_Vx = torch.as_tensor(_f64(Vx), device=b.device); d_Vy = torch.as_tensor(_f64(Vy), device=b.device)
+    _ck(lib().elg_dbg_tkick(b._h, t_lo, dt, nb, d_Vx.data_ptr(), d_Vy.data_ptr(), 1 if interp else 0))
+    b.synchronize()
+    return b.device_array(1)[: s.size].cpu().numpy(), b.device_array(3)[: s.size].cpu().numpy()
+
+
+def dbg_compact(coords, kind: str, ax: float, ay: float, ids=None):
+    """elg_dbg_compact on a bunch holding `coords` (the oracle's pre-aperture coordinates): returns
+    (survivor coords, survivor ids, lost ids, lost coords (n_lost, 6))."""
+    coords = _f64(coords)
+    b = Bunch(coords, 1e9, 1e-9, ids=ids, lost_capacity=coords.shape[1])
+    _ck(lib().elg_dbg_compact(b._h, {"RCOL": RCOL, "ECOL": ECOL}[kind], ax, ay))
+    v, sid = b.read()
+    lid, _, _, lco = b.lost()
+    return v, sid, lid, lco
 
 
 def dbg_wake_samples(kind: int, nb: int, dt: float, f=0.0, Q=0.0, Rs=0.0, table=None, dt_table=0.0) -> np.ndarray:
@@ -461,14 +518,3 @@ def dbg_convolve(counts, W, q: float) -> np.ndarray:
     st = torch.cuda.current_stream().cuda_stream
     _ck(lib().elg_dbg_convolve(d_c.data_ptr(), d_W.data_ptr(), d_c.numel(), q, d_V.data_ptr(), st))
     return d_V.cpu().numpy()
-
-
-def dbg_kick(s, delta, inv_bc, t_lo, inv_dt, nb, V, inv_E, interp=True) -> np.ndarray:
-    torch = _torch()
-    d_s = torch.as_tensor(_f64(s), device="cuda")
-    d_d = torch.as_tensor(_f64(delta), device="cuda").clone()
-    d_V = torch.as_tensor(_f64(V), device="cuda")
-    st = torch.cuda.current_stream().cuda_stream
-    _ck(lib().elg_dbg_kick(d_s.data_ptr(), d_d.data_ptr(), d_s.numel(), inv_bc, t_lo, inv_dt, nb, d_V.data_ptr(),
-                           inv_E, 1 if interp else 0, st))
-    return d_d.cpu().numpy()

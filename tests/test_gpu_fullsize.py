@@ -173,7 +173,8 @@ def test_rfcw_cavity_at_1e8(elg, elgo):
     Wt = elgo.wake_samples(2, nb, dt, f=trw["f"], Q=trw["Q"], Rs=trw["Rs"])
     Vx = elgo.convolve_d(Dx, Wt, q); Vy = elgo.convolve_d(Dy, Wt, q)
     Vg = go["V"]
-    assert np.array_equal(Vg[nb:2 * nb], Dx) and np.array_equal(Vg[2 * nb:3 * nb], Dy), "exact dipole sums"
+    for got, ref in ((Vg[nb:2 * nb], Dx), (Vg[2 * nb:3 * nb], Dy)):           # dipole sums (G33) vs the plain long-double sums
+        assert np.max(np.abs(got - ref)) <= 1e-10 * np.max(np.abs(ref))
     for got, ref in ((Vg[:nb], V), (Vg[3 * nb:4 * nb], Vx), (Vg[4 * nb:5 * nb], Vy)):
         assert np.max(np.abs(got - ref)) <= 1e-10 * np.max(np.abs(ref))
 
@@ -182,3 +183,83 @@ def test_rfcw_cavity_at_1e8(elg, elgo):
     elgo.tkick(ov[4], xp_exp, yp_exp, inv_bc, t_lo, inv_dt, nb, Vx, Vy, inv_E, True)
     for c, ref in ((5, d_exp), (1, xp_exp), (3, yp_exp)):
         assert np.max(np.abs(gv[c] - ref) / np.maximum(np.abs(ref), np.std(ref))) <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------------------------
+# BASELINE.json configs[1], [2], [4] at their FULL sizes, whole arrays (the oracle needs seconds for each):
+# north_star "matches the oracle at the stated tolerances on all 5 configs"; PAPER.md:233 (per-element comparison).
+# ------------------------------------------------------------------------------------------------------------
+def _both_full(elg, elgo, w):
+    v0 = w.particles()
+    ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
+    oo = ob.track(elgo.Beamline(w.elements, ring=w.ring), w.n_turns, moments_every=w.moments_every, n_threads=16,
+                  want_stage_outputs=True)
+    gbl = elg.Beamline(w.elements, ring=w.ring)
+    gb = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=gbl)
+    go = gb.track(gbl, w.n_turns, moments_every=w.moments_every, want_stage_outputs=True)
+    return ob, oo, gb, go
+
+
+def _rel_err(a, b):
+    sig = b.std(axis=1, keepdims=True)
+    return float(np.max(np.abs(a - b) / np.maximum(np.abs(b), np.maximum(sig, 1e-300))))
+
+
+def _check_lost_full(ob, gb):
+    oi, ot, oe, oc = ob.lost(); gi, gt, ge, gc = gb.lost()
+    assert np.array_equal(gi, oi), "lost IDs / order"
+    assert np.array_equal(gt, ot) and np.array_equal(ge, oe)
+    assert np.array_equal(gc[:, :5], oc[:, :5])
+    if oc.size:
+        assert np.max(np.abs(gc[:, 5] - oc[:, 5])) <= 1e-12 * np.max(np.abs(oc[:, 5]))
+    return oi.size
+
+
+def test_cfg1_full_size(elg, elgo):
+    """configs[1]: 1e6 particles, 77 elements (25 ECOL, 2 RFKICK), moments after every element: survivor IDs and order,
+    lost log, x x' y y' s bit-exact; delta <= 1e-12; 77 records <= 1e-10."""
+    w = make_workload("cfg1")
+    assert w.n0 == 1_000_000
+    ob, oo, gb, go = _both_full(elg, elgo, w)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid) and 0 < gid.size < w.n0
+    assert np.array_equal(gv[:5], ov[:5])
+    assert _rel_err(gv, ov) <= 1e-12
+    assert _check_lost_full(ob, gb) + gid.size == w.n0
+    gr, orr = go["records"], oo["records"]
+    assert gr.shape == orr.shape == (77, 43) and np.array_equal(gr[:, 0], orr[:, 0])
+    for k in range(77):
+        S = orr[k, 7:].reshape(6, 6); sig = np.sqrt(np.diag(S))
+        assert np.all(np.abs(gr[k, 1:7] - orr[k, 1:7]) <= 1e-10 * np.maximum(np.max(np.abs(orr[k, 1:7])), sig)), k
+        assert np.max(np.abs(gr[k, 7:] - orr[k, 7:])) <= 1e-10 * np.max(np.abs(S)), k
+
+
+def test_cfg2_full_size(elg, elgo):
+    """configs[2]: 1e7 particles, 10 passes of DRIFT + tabulated WAKE (8192 bins): 10 windows and 10 x 8192 histograms
+    bit-exact, V <= 1e-10 of its maximum per pass, x x' y y' s bit-exact, delta <= 1e-10 (ten kicks good to 1e-10)."""
+    w = make_workload("cfg2")
+    assert w.n0 == 10_000_000 and w.n_turns == 10
+    ob, oo, gb, go = _both_full(elg, elgo, w)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid) and gid.size == w.n0
+    assert np.array_equal(gv[:5], ov[:5])
+    assert np.array_equal(go["window"], oo["window"]) and go["window"].shape == (10, 3)
+    assert np.array_equal(go["hist"], oo["hist"]) and go["hist"].size == 10 * 8192
+    assert np.all(go["hist"].reshape(10, 8192).sum(axis=1) == w.n0)
+    Vo = oo["V"].reshape(10, 8192); Vg = go["V"].reshape(10, 8192)
+    assert np.max(np.abs(Vg - Vo) / np.max(np.abs(Vo), axis=1, keepdims=True)) <= 1e-10
+    assert _rel_err(gv, ov) <= 1e-10
+
+
+def test_cfg4_full_size(elg, elgo):
+    """configs[4]: 1e7 particles, 20 x [RCOL, 65 536-bin HISTO, DRIFT]: survivor order, lost records, coordinates and
+    the 20 histograms bit-exact."""
+    w = make_workload("cfg4")
+    assert w.n0 == 10_000_000
+    ob, oo, gb, go = _both_full(elg, elgo, w)
+    ov, oid = ob.read(); gv, gid = gb.read()
+    assert np.array_equal(gid, oid) and np.array_equal(gv, ov)
+    assert np.array_equal(go["window"], oo["window"]) and go["window"].shape == (20, 3)
+    assert np.array_equal(go["hist"], oo["hist"]) and go["hist"].size == 20 * 65536
+    nl = _check_lost_full(ob, gb)
+    assert nl + gid.size == w.n0 and nl / w.n0 > 0.9
