@@ -216,8 +216,8 @@ int32_t device_sms(int* sms) {
 int32_t long_setup_once() {
     static bool done = false;
     if (!done) {
-        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    chain_long_smem_bytes<kMaxOpsLarge, 0>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long0_kernel<kMaxOpsLarge>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    chain_long0_smem_bytes<kMaxOpsLarge>()));
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     chain_long_smem_bytes<kMaxOpsLarge, 1>()));
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -551,8 +551,11 @@ struct Tracker {
             a.type[k] = pending[k].type;
             std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
         }
+        for (int k = (int)pending.size() - 1; k >= 0; k--)            // lengths of the runs of consecutive MATRIX slots
+            a.mat_run[k] = pending[k].type != OP_MATRIX ? 0 : (uint8_t)(1 + ((size_t)k + 1 < pending.size() ? a.mat_run[k + 1] : 0));
         int grid = 0;
-        if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS, EXT>, chain_long_smem_bytes<MAXOPS, EXT>());
+        if constexpr (MAXOPS == kMaxOpsLarge && EXT == 0) grid = cached_grid((const void*)chain_long0_kernel<MAXOPS>, chain_long0_smem_bytes<MAXOPS>(), kLong0Threads);
+        else if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS, EXT>, chain_long_smem_bytes<MAXOPS, EXT>());
         else if constexpr (COMPACT) {
             grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0)>, compact_smem_bytes(), kC2Threads);
             if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
@@ -563,7 +566,9 @@ struct Tracker {
         if (want_mm) mm_grid = (mm_slot + 1) * grid;
         {
             ProfScope ps(b, MAXOPS == kMaxOpsLarge ? ELG_K_CHAIN_LONG : (COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN));
-            if constexpr (MAXOPS == kMaxOpsLarge)
+            if constexpr (MAXOPS == kMaxOpsLarge && EXT == 0)
+                chain_long0_kernel<MAXOPS><<<grid, kLong0Threads, chain_long0_smem_bytes<MAXOPS>(), b->stream>>>(a);
+            else if constexpr (MAXOPS == kMaxOpsLarge)
                 chain_long_kernel<MAXOPS, EXT><<<grid, kBlock, chain_long_smem_bytes<MAXOPS, EXT>(), b->stream>>>(a);
             else if constexpr (COMPACT)
             {
@@ -1058,7 +1063,7 @@ extern "C" int32_t elg_upload_and_track(elg_bunch* b, const elg_beamline* bl, co
     for (int c = 0; c < 6; c++) if (!h_coords[c]) return fail(ELG_EINVAL, "elg_upload_and_track: NULL coordinate array");
     Tracker probe{b, bl, o};
     const long long k_split = probe.map_prefix();
-    if (n_turns < 1 || k_split == 0 || n_chunks <= 1 || b->n0 < 4 * 3072) {       // nothing to overlap
+    if (n_turns < 1 || k_split == 0 || n_chunks <= 1 || b->n0 < 4 * 9216) {       // nothing to overlap
         int32_t rc = elg_bunch_upload(b, h_coords, h_ids);
         return rc != ELG_OK ? rc : elg_track(b, bl, n_turns, o);
     }
@@ -1086,7 +1091,7 @@ extern "C" int32_t elg_upload_and_track(elg_bunch* b, const elg_beamline* bl, co
     { int32_t rc = upload_tables(b, bl); if (rc != ELG_OK) return rc; }
     Tracker t{b, bl, o};
     b->rec_count = 0;
-    const long long per = align_up((b->n0 + n_chunks - 1) / n_chunks, 3072);     // multiple of every chain tile size
+    const long long per = align_up((b->n0 + n_chunks - 1) / n_chunks, 9216);     // multiple of every chain tile size (512 ... 2304)
     int slot = 0;
     for (long long lo = 0; lo < b->n0 && t.ok(); lo += per, slot++) {
         const long long hi = lo + per < b->n0 ? lo + per : b->n0;

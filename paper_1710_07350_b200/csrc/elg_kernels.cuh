@@ -49,6 +49,7 @@ struct DevState {
     unsigned int fid_done;
     unsigned long long fid_acc[2];   // exact fixed-point sum of s - s_design (G36)
     double s_ref;              // fiducial path length of the bunch, read by RFKICK ops with the fiducial flag
+    long long zero_bits;       // always 0: a value the compiler cannot see through (matrix_map_uniform)
 };
 
 struct ChainCommon {
@@ -86,6 +87,7 @@ template <int MAXOPS>
 struct ChainArgs {
     ChainCommon c;
     uint8_t type[MAXOPS];
+    uint8_t mat_run[MAXOPS];               // number of consecutive OP_MATRIX slots starting at this one (host-computed)
     alignas(16) double coef[MAXOPS][42];   // MATRIX: R[36], C[6].  DRIFT: L.  RFKICK: A, omega, phi0, s_ref, inv_bc.
                                // KICK: inv_bc, inv_E.  MATRIX2: R[36], C[6], then 3 slots = Tt[21][6] (pair-major)
 };
@@ -666,6 +668,163 @@ __global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_cons
         __syncthreads();
         if (threadIdx.x == 0) {
             for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
+            c.mm_partial[2 * blockIdx.x] = mn;
+            c.mm_partial[2 * blockIdx.x + 1] = mx;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// chain_long0_kernel: long runs of first-order maps (cfg3: 80 MATRIX per launch), the kernel the headline metric
+// spends 97 % of its time in.  Bound by the fp64 pipe, and on sm_100 every coefficient that reaches a DFMA through
+// a vector register (LDS, LDC, LDG) costs that pipe a write-back slot: with the coefficients in shared memory the
+// bound is 36P / (36P + 42) of the DFMA rate for P particles per thread (0.84 at P = 6; round 1 measured 0.80).
+// Here the coefficients never touch a vector register: they stay in the kernel-parameter constant bank and reach
+// the DFMA as UNIFORM-register operands, loaded by UR-indexed LDCU in the runtime loop over the run's maps
+// (LDCU.64 UR, c[0x0][UR+imm]; DFMA R, R, UR, R).  A DFMA takes one uniform operand, so the row constant C[r] is made
+// a vector value once per row (matrix_map_uniform below); with two uniform operands in the first term ptxas falls
+// back to per-thread LDC for everything.  tests/test_abi.py checks the SASS for the uniform form.
+// 6 particles per thread, one block of 384 threads per SM (144 registers): a register-only loop of 80 matrices runs
+// at 61.5 DFMA/clk/SM = 96 % of the pipe (50.0 with shared-memory coefficients; profiles/r02_long.md).
+// Same arithmetic, in the same order, as chain_kernel.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kPL0 = 6;                                 // particles per thread
+constexpr int kLong0Threads = 384;
+constexpr int kLong0Regs = 160;
+template <int MAXOPS>
+constexpr int chain_long0_smem_bytes() { return 6 * kLong0Threads * kPL0 * 8; }
+
+// `zero` is a 0 loaded from the device state (opaque to the compiler, and a per-thread value to it): OR-ing it into the
+// bits of C[r] makes C[r] a vector value once per ROW without changing a bit of it, so that every DFMA of the row has
+// exactly one uniform operand.
+template <int P>
+__device__ __forceinline__ void matrix_map_uniform(const double* __restrict__ c, long long zero, const double (&v)[P][6], double (&w)[P][6]) {
+#pragma unroll
+    for (int r = 0; r < 6; r++) {
+        const double cv = __longlong_as_double(__double_as_longlong(c[36 + r]) | zero);
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            double acc = cv;
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) acc = fma(c[6 * r + cc], v[p][cc], acc);
+            w[p][r] = acc;
+        }
+    }
+}
+
+template <int MAXOPS, int P>
+__device__ __forceinline__ void apply_ops_uniform(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
+    const long long zero = a.c.st->zero_bits;                    // 0, but loaded: opaque to the compiler, and a vector value
+    const int n_ops = a.c.n_ops;
+    int op = 0;
+    while (op < n_ops) {
+        if (a.type[op] == OP_MATRIX) {
+            const int end = op + a.mat_run[op];                  // [op, end): consecutive MATRIX maps
+#pragma unroll 1
+            for (; op + 1 < end; op += 2) {                      // pairs: v -> w -> v, no copy-back; nothing else in this loop
+                double w[P][6];
+                matrix_map_uniform<P>(a.coef[op], zero, v, w);
+                matrix_map_uniform<P>(a.coef[op + 1], zero, w, v);
+            }
+            if (op < end) {
+                double w[P][6];
+                matrix_map_uniform<P>(a.coef[op], zero, v, w);
+#pragma unroll
+                for (int p = 0; p < P; p++)
+#pragma unroll
+                    for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+                op++;
+            }
+        } else {
+            other_map<P, false>(a.type[op], a.coef[op], a.c, v);
+            op++;
+        }
+    }
+}
+
+template <int MAXOPS>
+__global__ void __maxnreg__(kLong0Regs) chain_long0_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+    constexpr int PL = kPL0;
+    constexpr int NT = kLong0Threads, NW = NT / 32;
+    constexpr int kTileL = NT * PL;
+    constexpr int H = PL / 2;
+    constexpr int kSub = 2 * NT;
+    extern __shared__ __align__(16) double s_tile0[];            // [6][H][kSub]: thread t owns doubles 2t, 2t+1 of each row
+    const ChainCommon& c = a.c;
+    const long long n_all = c.st->n_alive[c.cur];
+    const long long n = (c.range_hi >= 0 && c.range_hi < n_all) ? c.range_hi : n_all;       // end of my range
+    const long long n_tiles = (n > c.range_lo) ? (n - c.range_lo + kTileL - 1) / kTileL : 0;
+    __shared__ double s_mn[NT], s_mx[NT];                        // running min / max of s per thread: not in registers,
+    if (c.want_minmax) { s_mn[threadIdx.x] = INFINITY; s_mx[threadIdx.x] = -INFINITY; }     // the map loop needs them all
+
+    auto prefetch = [&](long long tile) {
+        const long long t0 = c.range_lo + tile * kTileL + (long long)threadIdx.x * 2;
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            const long long i0 = t0 + (long long)h * kSub;
+            const long long left = n - i0;
+            const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);          // zero-fill beyond the live prefix
+            const long long is = left >= 1 ? i0 : 0;
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++)
+                if (c.rmask & (1u << cc))
+                    cp_async16(s_tile0 + (cc * H + h) * kSub + threadIdx.x * 2, c.src[cc] + is, bytes);
+        }
+    };
+
+    long long tile = blockIdx.x;
+    if (tile < n_tiles) prefetch(tile);
+    while (tile < n_tiles) {
+        double v[PL][6];
+        cp_async_wait_all();
+#pragma unroll
+        for (int h = 0; h < H; h++)
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) {
+                double2 t = make_double2(0.0, 0.0);
+                if (c.rmask & (1u << cc)) t = *reinterpret_cast<const double2*>(s_tile0 + (cc * H + h) * kSub + threadIdx.x * 2);
+                v[2 * h][cc] = t.x; v[2 * h + 1][cc] = t.y;
+            }
+        const long long next = tile + gridDim.x;
+        if (next < n_tiles) prefetch(next);                      // own slots only: already in registers
+
+        apply_ops_uniform<MAXOPS, PL>(a, v);
+
+        const long long t0 = c.range_lo + tile * kTileL + (long long)threadIdx.x * 2;
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            const long long i0 = t0 + (long long)h * kSub;
+            const bool full = (i0 + 2 <= n);
+#pragma unroll
+            for (int cc = 0; cc < 6; cc++) {
+                if (c.wmask & (1u << cc)) {
+                    if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[2 * h][cc], v[2 * h + 1][cc]);
+                    else if (i0 < n) c.dst[cc][i0] = v[2 * h][cc];
+                }
+            }
+            if (c.want_minmax) {
+                double mn = s_mn[threadIdx.x], mx = s_mx[threadIdx.x];
+                if (i0 < n) { mn = fmin(mn, v[2 * h][4]); mx = fmax(mx, v[2 * h][4]); }
+                if (full) { mn = fmin(mn, v[2 * h + 1][4]); mx = fmax(mx, v[2 * h + 1][4]); }
+                s_mn[threadIdx.x] = mn; s_mx[threadIdx.x] = mx;
+            }
+        }
+        tile = next;
+    }
+
+    if (c.want_minmax) {                                         // exact min/max of s (a8)
+        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+        double mn = s_mn[threadIdx.x], mx = s_mx[threadIdx.x];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, d));
+            mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+        }
+        __syncthreads();
+        if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < NW; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
             c.mm_partial[2 * blockIdx.x] = mn;
             c.mm_partial[2 * blockIdx.x + 1] = mx;
         }
@@ -1494,6 +1653,7 @@ __global__ void init_state_kernel(DevState* st, long long n0) {
     st->bin_lo = 0; st->bin_hi = -1;
     st->tile_counter = 0; st->done_counter = 0; st->mom_done = 0; st->fid_done = 0;
     st->fid_acc[0] = 0ull; st->fid_acc[1] = 0ull; st->s_ref = 0.0;
+    st->zero_bits = 0;
 }
 
 }  // namespace elg
