@@ -216,14 +216,10 @@ int32_t device_sms(int* sms) {
 int32_t long_setup_once() {
     static bool done = false;
     if (!done) {
-        ELG_CK(cudaFuncSetAttribute(chain_long0_kernel<kMaxOpsLarge>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    chain_long0_smem_bytes<kMaxOpsLarge>()));
-        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    chain_long_smem_bytes<kMaxOpsLarge, 1>()));
-        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    chain_long_smem_bytes<kMaxOpsLarge, 2>()));
-        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    chain_long_smem_bytes<kMaxOpsLarge, 3>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<0>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<1>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<2>()));
+        ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<3>()));
         ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
         ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
         done = true;
@@ -552,10 +548,14 @@ struct Tracker {
             std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
         }
         for (int k = (int)pending.size() - 1; k >= 0; k--)            // lengths of the runs of consecutive MATRIX slots
-            a.mat_run[k] = pending[k].type != OP_MATRIX ? 0 : (uint8_t)(1 + ((size_t)k + 1 < pending.size() ? a.mat_run[k + 1] : 0));
+        {
+            const uint8_t ty = pending[k].type;                       // (MATRIX and MATRIX_UNC runs are counted separately)
+            const bool run_type = ty == OP_MATRIX || ty == OP_MATRIX_UNC;
+            const bool same_next = (size_t)k + 1 < pending.size() && pending[k + 1].type == ty;
+            a.mat_run[k] = !run_type ? 0 : (uint8_t)(1 + (same_next ? a.mat_run[k + 1] : 0));
+        }
         int grid = 0;
-        if constexpr (MAXOPS == kMaxOpsLarge && EXT == 0) grid = cached_grid((const void*)chain_long0_kernel<MAXOPS>, chain_long0_smem_bytes<MAXOPS>(), kLong0Threads);
-        else if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS, EXT>, chain_long_smem_bytes<MAXOPS, EXT>());
+        if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS, EXT>, chain_long_smem_bytes<EXT>(), LongCfg<EXT>::NT);
         else if constexpr (COMPACT) {
             grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0)>, compact_smem_bytes(), kC2Threads);
             if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
@@ -566,10 +566,8 @@ struct Tracker {
         if (want_mm) mm_grid = (mm_slot + 1) * grid;
         {
             ProfScope ps(b, MAXOPS == kMaxOpsLarge ? ELG_K_CHAIN_LONG : (COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN));
-            if constexpr (MAXOPS == kMaxOpsLarge && EXT == 0)
-                chain_long0_kernel<MAXOPS><<<grid, kLong0Threads, chain_long0_smem_bytes<MAXOPS>(), b->stream>>>(a);
-            else if constexpr (MAXOPS == kMaxOpsLarge)
-                chain_long_kernel<MAXOPS, EXT><<<grid, kBlock, chain_long_smem_bytes<MAXOPS, EXT>(), b->stream>>>(a);
+            if constexpr (MAXOPS == kMaxOpsLarge)
+                chain_long_kernel<MAXOPS, EXT><<<grid, LongCfg<EXT>::NT, chain_long_smem_bytes<EXT>(), b->stream>>>(a);
             else if constexpr (COMPACT)
             {
                 void* kargs[] = {(void*)&a};                     // cooperative: every block resident (static tiles)
@@ -629,10 +627,10 @@ struct Tracker {
         }
 #define ELG_LAUNCH(M, C, PP, E) launch_chain<M, C, PP, E>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
         if (large) {
-            if (ext == 3) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 3);
-            else if (ext == 2) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 2);
-            else if (ext == 1) ELG_LAUNCH(kMaxOpsLarge, false, kPL, 1);
-            else ELG_LAUNCH(kMaxOpsLarge, false, kPL, 0);
+            if (ext == 3) ELG_LAUNCH(kMaxOpsLarge, false, 0, 3);
+            else if (ext == 2) ELG_LAUNCH(kMaxOpsLarge, false, 0, 2);
+            else if (ext == 1) ELG_LAUNCH(kMaxOpsLarge, false, 0, 1);
+            else ELG_LAUNCH(kMaxOpsLarge, false, 0, 0);
         }
         else if (compact) { if (ext) ELG_LAUNCH(kMaxOpsSmall, true, 2, 1); else ELG_LAUNCH(kMaxOpsSmall, true, 2, 0); }
         else if (p4) { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 4, 1); else ELG_LAUNCH(kMaxOpsSmall, false, 4, 0); }
@@ -649,7 +647,7 @@ struct Tracker {
     }
 
     // MATRIX: dense, or (ELG_TRACK_SPARSE_MATRICES) packed for the uncoupled zero pattern when every entry outside it is
-    // exactly zero (layout only: the 20 kept coefficients and C in the order matrix_unc_map_s128 reads them)
+    // exactly zero (layout only: the 20 kept coefficients and C in the order matrix_unc_map_uniform reads them)
     void push_matrix(const elg_element& e) {
         HostOp op{};
         op.type = OP_MATRIX;

@@ -7,7 +7,7 @@
 // from a sequential CPU evaluation.
 //
 // Kernels (one section each):
-//   chain_kernel, chain_long_kernel    fused run of element maps (short runs / long fp64-bound runs)
+//   chain_kernel, chain_long_kernel    fused run of element maps (short HBM-bound runs / long fp64-bound runs)
 //   compact_kernel                 fused run ending in an aperture + stable single-pass stream compaction
 //   window_kernel                  min/max partials -> histogram window + occupied bin range, zero counts
 //   hist_kernel                    shared-memory privatised time histogram
@@ -25,6 +25,17 @@ constexpr int kP = 2;                  // particles per thread = one 128-bit acc
 constexpr int kTile = kBlock * kP;     // particles per tile
 constexpr int kHistSmemBins = 16384;   // 64 KB of privatised bins per block
 constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
+// long-run kernel geometry of the higher-order levels (threads per block, particles per thread, register cap)
+#ifndef ELG_L1_NT
+#define ELG_L1_NT 256
+#define ELG_L1_PL 6
+#define ELG_L1_REGS 200
+#endif
+#ifndef ELG_L2_NT
+#define ELG_L2_NT 384
+#define ELG_L2_PL 4
+#define ELG_L2_REGS 144
+#endif
 
 enum : uint8_t { OP_DRIFT = 1, OP_MATRIX = 2, OP_RFKICK = 3, OP_KICK = 4,
                  OP_MATRIX2 = 5,      // second-order map: this slot holds R, C; the next three hold T (OP_CONT)
@@ -144,44 +155,21 @@ __device__ __forceinline__ void matrix_map(const double* __restrict__ c, const d
     }
 }
 
-// the same map with the 42 coefficients fetched from shared memory 128 bits at a time (16-byte aligned block)
-template <int P>
-__device__ __forceinline__ void matrix_map_s128(const double* c, const double (&v)[P][6], double (&w)[P][6]) {
-    const double2* c2 = reinterpret_cast<const double2*>(c);
-    const double2 C01 = c2[18], C23 = c2[19], C45 = c2[20];
-    const double Cc[6] = {C01.x, C01.y, C23.x, C23.y, C45.x, C45.y};
-#pragma unroll
-    for (int r = 0; r < 6; r++) {
-        const double2 k01 = c2[3 * r], k23 = c2[3 * r + 1], k45 = c2[3 * r + 2];
-        const double k[6] = {k01.x, k01.y, k23.x, k23.y, k45.x, k45.y};
-#pragma unroll
-        for (int p = 0; p < P; p++) {
-            double acc = Cc[r];
-#pragma unroll
-            for (int cc = 0; cc < 6; cc++) acc = fma(k[cc], v[p][cc], acc);
-            w[p][r] = acc;
-        }
-    }
-}
-
 // second-order terms of MATRIX2 (G31): w[p][r] += sum over the pairs q = (j,k), j <= k, of T[r][q] (v_j v_k),
-// q ascending, continuing row r's FMA chain after the six first-order terms.  tt = Tt[21][6] (pair-major), so
-// one pair costs P products and three 128-bit coefficient fetches for 6 P DFMA.
+// q ascending, continuing row r's FMA chain after the six first-order terms.  tt = Tt[21][6] (pair-major), so one
+// pair costs P products and 6 P DFMA on six coefficients (uniform operands when tt points into the parameter bank).
 template <int P>
 __device__ __forceinline__ void matrix2_terms(const double* __restrict__ tt, const double (&v)[P][6], double (&w)[P][6]) {
-    const double2* t2 = reinterpret_cast<const double2*>(tt);
     int q = 0;
 #pragma unroll
     for (int j = 0; j < 6; j++) {
 #pragma unroll
         for (int k = j; k < 6; k++) {
-            const double2 t01 = t2[3 * q], t23 = t2[3 * q + 1], t45 = t2[3 * q + 2];
-            const double t[6] = {t01.x, t01.y, t23.x, t23.y, t45.x, t45.y};
 #pragma unroll
             for (int p = 0; p < P; p++) {
                 const double pr = v[p][j] * v[p][k];            // rounded product (-fmad=false: never contracted)
 #pragma unroll
-                for (int r = 0; r < 6; r++) w[p][r] = fma(t[r], pr, w[p][r]);
+                for (int r = 0; r < 6; r++) w[p][r] = fma(tt[6 * q + r], pr, w[p][r]);
             }
             q++;
         }
@@ -190,9 +178,11 @@ __device__ __forceinline__ void matrix2_terms(const double* __restrict__ tt, con
 
 // third-order terms of MATRIX3 (G35): w[p][r] += sum over the triples t = (j,k,l), j <= k <= l, lexicographic, of
 // U[r][t] ((v_j v_k) v_l), continuing row r's FMA chain after the second-order terms.  ut = Ut[56][6].
+// `zero` (an opaque 0, see matrix_map_uniform) ties every pair product to the accumulator it will feed:
+// v_j | (zero & w) is v_j, bit for bit, but cannot be formed before w is: without it ptxas hoists all 77 products of a
+// particle to the front of the 1344-DFMA block and spills them.
 template <int P>
-__device__ __forceinline__ void matrix3_terms(const double* __restrict__ ut, const double (&v)[P][6], double (&w)[P][6]) {
-    const double2* u2 = reinterpret_cast<const double2*>(ut);
+__device__ __forceinline__ void matrix3_terms(const double* __restrict__ ut, long long zero, const double (&v)[P][6], double (&w)[P][6]) {
     int t = 0;
 #pragma unroll
     for (int j = 0; j < 6; j++) {
@@ -200,16 +190,17 @@ __device__ __forceinline__ void matrix3_terms(const double* __restrict__ ut, con
         for (int k = j; k < 6; k++) {
             double pjk[P];
 #pragma unroll
-            for (int p = 0; p < P; p++) pjk[p] = v[p][j] * v[p][k];
+            for (int p = 0; p < P; p++) {
+                const double vj = __longlong_as_double(__double_as_longlong(v[p][j]) | (zero & __double_as_longlong(w[p][0])));
+                pjk[p] = vj * v[p][k];
+            }
 #pragma unroll
             for (int l = k; l < 6; l++) {
-                const double2 u01 = u2[3 * t], u23 = u2[3 * t + 1], u45 = u2[3 * t + 2];
-                const double u[6] = {u01.x, u01.y, u23.x, u23.y, u45.x, u45.y};
 #pragma unroll
                 for (int p = 0; p < P; p++) {
                     const double pr = pjk[p] * v[p][l];
 #pragma unroll
-                    for (int r = 0; r < 6; r++) w[p][r] = fma(u[r], pr, w[p][r]);
+                    for (int r = 0; r < 6; r++) w[p][r] = fma(ut[6 * t + r], pr, w[p][r]);
                 }
                 t++;
             }
@@ -223,35 +214,36 @@ __device__ __forceinline__ void matrix3_terms(const double* __restrict__ ut, con
 // needs 20 of the 36 FMAs.  The kept terms run in the same order as in matrix_map, and a skipped term adds +-0, so
 // for finite coordinates the result equals the dense map's (up to the sign of a zero).  c = 28 packed doubles:
 // (R00 R01)(R05 C0)(R10 R11)(R15 C1)(R22 R23)(R25 C2)(R32 R33)(R35 C3)(R40 R41)(R42 R43)(R44 R45)(C4 R54)(R55 C5)(- -).
+// Coefficients are uniform operands; `zero` makes the row constants vector values (see matrix_map_uniform).
 template <int P>
-__device__ __forceinline__ void matrix_unc_map_s128(const double* c, const double (&v)[P][6], double (&w)[P][6]) {
-    const double2* c2 = reinterpret_cast<const double2*>(c);
+__device__ __forceinline__ void matrix_unc_map_uniform(const double* __restrict__ c, long long zero, const double (&v)[P][6], double (&w)[P][6]) {
 #pragma unroll
     for (int h = 0; h < 2; h++) {                                // transverse planes: rows 2h, 2h + 1
 #pragma unroll
         for (int rr = 0; rr < 2; rr++) {
-            const double2 k = c2[4 * h + 2 * rr], kc = c2[4 * h + 2 * rr + 1];
+            const double* k = c + 8 * h + 4 * rr;                // k[0] k[1] | k[2] = R[.][5], k[3] = C
+            const double cv = __longlong_as_double(__double_as_longlong(k[3]) | zero);
 #pragma unroll
             for (int p = 0; p < P; p++) {
-                double acc = kc.y;
-                acc = fma(k.x, v[p][2 * h], acc);
-                acc = fma(k.y, v[p][2 * h + 1], acc);
-                acc = fma(kc.x, v[p][5], acc);
+                double acc = cv;
+                acc = fma(k[0], v[p][2 * h], acc);
+                acc = fma(k[1], v[p][2 * h + 1], acc);
+                acc = fma(k[2], v[p][5], acc);
                 w[p][2 * h + rr] = acc;
             }
         }
     }
-    const double2 s01 = c2[8], s23 = c2[9], s45 = c2[10], m = c2[11], d = c2[12];
+    const double c4 = __longlong_as_double(__double_as_longlong(c[22]) | zero);
+    const double c5 = __longlong_as_double(__double_as_longlong(c[25]) | zero);
 #pragma unroll
     for (int p = 0; p < P; p++) {
-        double acc = m.x;
-        acc = fma(s01.x, v[p][0], acc); acc = fma(s01.y, v[p][1], acc);
-        acc = fma(s23.x, v[p][2], acc); acc = fma(s23.y, v[p][3], acc);
-        acc = fma(s45.x, v[p][4], acc); acc = fma(s45.y, v[p][5], acc);
+        double acc = c4;
+#pragma unroll
+        for (int cc = 0; cc < 6; cc++) acc = fma(c[16 + cc], v[p][cc], acc);
         w[p][4] = acc;
-        double a5 = d.y;
-        a5 = fma(m.y, v[p][4], a5);
-        a5 = fma(d.x, v[p][5], a5);
+        double a5 = c5;
+        a5 = fma(c[23], v[p][4], a5);
+        a5 = fma(c[24], v[p][5], a5);
         w[p][5] = a5;
     }
 }
@@ -381,52 +373,6 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
     }
 }
 
-// the run's maps with the coefficients in shared memory (copied there once per block): 128-bit fetches, and
-// consecutive MATRIX maps applied in pairs (v -> w -> v) so that no register copy-back is needed
-// LEVEL 0: MATRIX, DRIFT, RFKICK, KICK; 1: + MATRIX2, TKICK; 2: + MATRIX3; 3: level 0 + MATRIX_UNC (flagged option).  The planner picks the lowest level a run
-// needs: the higher-order code costs the 200-matrix cfg3 kernel registers and 30 % of its speed when compiled in.
-template <int MAXOPS, int P, int LEVEL>
-__device__ __forceinline__ void apply_ops_smem(const ChainArgs<MAXOPS>& a, const double* s_coef, double (&v)[P][6]) {
-    const ChainCommon& c = a.c;
-    int op = 0;
-    while (op < c.n_ops) {
-        const int ty = a.type[op];
-        if (ty == OP_MATRIX && op + 1 < c.n_ops && a.type[op + 1] == OP_MATRIX) {
-            double w[P][6];
-            matrix_map_s128<P>(s_coef + 42 * op, v, w);
-            matrix_map_s128<P>(s_coef + 42 * (op + 1), w, v);
-            op += 2;
-        } else if (LEVEL == 3 && ty == OP_MATRIX_UNC) {
-            double w[P][6];
-            if (op + 1 < c.n_ops && a.type[op + 1] == OP_MATRIX_UNC) {
-                matrix_unc_map_s128<P>(s_coef + 42 * op, v, w);
-                matrix_unc_map_s128<P>(s_coef + 42 * (op + 1), w, v);
-                op += 2;
-            } else {
-                matrix_unc_map_s128<P>(s_coef + 42 * op, v, w);
-#pragma unroll
-                for (int p = 0; p < P; p++)
-#pragma unroll
-                    for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
-                op++;
-            }
-        } else if (ty == OP_MATRIX || (LEVEL >= 1 && LEVEL <= 2 && ty == OP_MATRIX2) || (LEVEL == 2 && ty == OP_MATRIX3)) {
-            double w[P][6];
-            matrix_map_s128<P>(s_coef + 42 * op, v, w);
-            if (LEVEL >= 1 && LEVEL <= 2 && ty != OP_MATRIX) matrix2_terms<P>(s_coef + 42 * (op + 1), v, w);
-            if (LEVEL == 2 && ty == OP_MATRIX3) matrix3_terms<P>(s_coef + 42 * (op + 4), v, w);
-#pragma unroll
-            for (int p = 0; p < P; p++)
-#pragma unroll
-                for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
-            op += (ty == OP_MATRIX3) ? 12 : ((ty == OP_MATRIX2) ? 4 : 1);
-        } else {
-            other_map<P, (LEVEL >= 1 && LEVEL <= 2)>(ty, s_coef + 42 * op, c, v);
-            op++;
-        }
-    }
-}
-
 __device__ __forceinline__ bool survives(int ap_type, double ax, double ay, double x, double y) {
     if (ap_type == AP_RCOL) return (fabs(x) <= ax) && (fabs(y) <= ay);        // NaN -> false (G17)
     const double xa = x * ax, yb = y * ay;                                    // ECOL: ax, ay hold 1/a, 1/b
@@ -521,23 +467,6 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
 }
 
 // ---------------------------------------------------------------------------------------------------
-// chain_long_kernel: runs of more than kMaxOpsSmall maps (cfg3: 80 MATRIX per launch), bound by the fp64
-// pipe, not by HBM.  On sm_100 every operand fetch that returns through the MIO (LDS, LDC) costs DFMA
-// issue slots (profiles/r01d_long_chain_and_compaction.md: a broadcast LDS.128 costs about two DFMA), so the design minimises
-// coefficient fetches per DFMA:
-//   * kPL = 6 particles per thread: one 128-bit coefficient fetch feeds 12 DFMA;
-//   * the run's coefficients are copied once per block from the parameter bank to shared memory and read
-//     with LDS.128;
-//   * consecutive MATRIX maps are applied in pairs (v -> w -> v), so no register copy-back;
-//   * one block of 256 threads per SM (about 220 registers per thread); the next tile is prefetched into
-//     shared memory with cp.async while the current one is in the fp64 pipe, every thread copying exactly
-//     the 16-byte chunks it will read itself (no block-wide barrier in the tile loop).
-// Same arithmetic, in the same order, as chain_kernel.
-// ---------------------------------------------------------------------------------------------------
-constexpr int kPL = 6;                                  // particles per thread of the long-run kernel (levels 0, 1)
-constexpr int kPL3 = 4;                                 // with third-order maps (level 2): 6 would spill
-__host__ __device__ constexpr int long_pl(int level) { return level == 2 ? kPL3 : kPL; }
-
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
     const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(src_bytes) : "memory");
@@ -582,117 +511,32 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 template <int ID, int N>
 __device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(N) : "memory"); }
 
-template <int MAXOPS, int LEVEL>
-constexpr int chain_long_smem_bytes() { return MAXOPS * 42 * 8 + 6 * kBlock * long_pl(LEVEL) * 8; }
-
-template <int MAXOPS, int LEVEL>
-__global__ void __launch_bounds__(kBlock, 1) chain_long_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
-    constexpr int PL = long_pl(LEVEL);
-    constexpr int kTileL = kBlock * PL;
-    constexpr int H = PL / 2;
-    constexpr int kSub = 2 * kBlock;
-    extern __shared__ __align__(16) double sm_long[];
-    double* s_coef = sm_long;                                    // [n_ops][42]
-    double* s_tile = sm_long + MAXOPS * 42;                      // [6][H][kSub]: thread t owns doubles 2t, 2t+1 of each row
-    const ChainCommon& c = a.c;
-    const long long n_all = c.st->n_alive[c.cur];
-    const long long n = (c.range_hi >= 0 && c.range_hi < n_all) ? c.range_hi : n_all;       // end of my range
-    const long long n_tiles = (n > c.range_lo) ? (n - c.range_lo + kTileL - 1) / kTileL : 0;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    double mn = INFINITY, mx = -INFINITY;
-
-    for (int i = threadIdx.x; i < c.n_ops * 42; i += kBlock) s_coef[i] = a.coef[i / 42][i % 42];
-
-    auto prefetch = [&](long long tile) {
-        const long long t0 = c.range_lo + tile * kTileL + (long long)threadIdx.x * 2;
-#pragma unroll
-        for (int h = 0; h < H; h++) {
-            const long long i0 = t0 + (long long)h * kSub;
-            const long long left = n - i0;
-            const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);          // zero-fill beyond the live prefix
-            const long long is = left >= 1 ? i0 : 0;
-#pragma unroll
-            for (int cc = 0; cc < 6; cc++)
-                if (c.rmask & (1u << cc))
-                    cp_async16(s_tile + (cc * H + h) * kSub + threadIdx.x * 2, c.src[cc] + is, bytes);
-        }
-    };
-
-    long long tile = blockIdx.x;
-    if (tile < n_tiles) prefetch(tile);
-    __syncthreads();                                             // s_coef complete
-    while (tile < n_tiles) {
-        double v[PL][6];
-        cp_async_wait_all();
-#pragma unroll
-        for (int h = 0; h < H; h++)
-#pragma unroll
-            for (int cc = 0; cc < 6; cc++) {
-                double2 t = make_double2(0.0, 0.0);
-                if (c.rmask & (1u << cc)) t = *reinterpret_cast<const double2*>(s_tile + (cc * H + h) * kSub + threadIdx.x * 2);
-                v[2 * h][cc] = t.x; v[2 * h + 1][cc] = t.y;
-            }
-        const long long next = tile + gridDim.x;
-        if (next < n_tiles) prefetch(next);                      // own slots only: already in registers
-
-        apply_ops_smem<MAXOPS, PL, LEVEL>(a, s_coef, v);
-
-        const long long t0 = c.range_lo + tile * kTileL + (long long)threadIdx.x * 2;
-#pragma unroll
-        for (int h = 0; h < H; h++) {
-            const long long i0 = t0 + (long long)h * kSub;
-            const bool full = (i0 + 2 <= n);
-#pragma unroll
-            for (int cc = 0; cc < 6; cc++) {
-                if (c.wmask & (1u << cc)) {
-                    if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[2 * h][cc], v[2 * h + 1][cc]);
-                    else if (i0 < n) c.dst[cc][i0] = v[2 * h][cc];
-                }
-            }
-            if (c.want_minmax) {
-                if (i0 < n) { mn = fmin(mn, v[2 * h][4]); mx = fmax(mx, v[2 * h][4]); }
-                if (full) { mn = fmin(mn, v[2 * h + 1][4]); mx = fmax(mx, v[2 * h + 1][4]); }
-            }
-        }
-        tile = next;
-    }
-
-    if (c.want_minmax) {                                         // exact min/max of s (a8)
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, d));
-            mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
-        }
-        __shared__ double s_mn[kWarps], s_mx[kWarps];
-        if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            for (int w = 1; w < kWarps; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
-            c.mm_partial[2 * blockIdx.x] = mn;
-            c.mm_partial[2 * blockIdx.x + 1] = mx;
-        }
-    }
-}
-
 // ---------------------------------------------------------------------------------------------------
-// chain_long0_kernel: long runs of first-order maps (cfg3: 80 MATRIX per launch), the kernel the headline metric
-// spends 97 % of its time in.  Bound by the fp64 pipe, and on sm_100 every coefficient that reaches a DFMA through
-// a vector register (LDS, LDC, LDG) costs that pipe a write-back slot: with the coefficients in shared memory the
-// bound is 36P / (36P + 42) of the DFMA rate for P particles per thread (0.84 at P = 6; round 1 measured 0.80).
+// chain_long_kernel: long runs of maps (cfg3: 80 MATRIX per launch), the kernel the headline metric spends 97 % of
+// its time in.  Bound by the fp64 pipe, and on sm_100 every coefficient that reaches a DFMA through a vector
+// register (LDS, LDC, LDG) costs that pipe a write-back slot: with the coefficients in shared memory the bound is
+// 36P / (36P + 42) of the DFMA rate for P particles per thread (0.84 at P = 6; round 1 measured 0.80).
 // Here the coefficients never touch a vector register: they stay in the kernel-parameter constant bank and reach
 // the DFMA as UNIFORM-register operands, loaded by UR-indexed LDCU in the runtime loop over the run's maps
 // (LDCU.64 UR, c[0x0][UR+imm]; DFMA R, R, UR, R).  A DFMA takes one uniform operand, so the row constant C[r] is made
-// a vector value once per row (matrix_map_uniform below); with two uniform operands in the first term ptxas falls
-// back to per-thread LDC for everything.  tests/test_abi.py checks the SASS for the uniform form.
-// 6 particles per thread, one block of 384 threads per SM (144 registers): a register-only loop of 80 matrices runs
-// at 61.5 DFMA/clk/SM = 96 % of the pipe (50.0 with shared-memory coefficients; profiles/r02_long.md).
+// a vector value once per row (matrix_map_uniform); with two uniform operands in the first term ptxas falls back to
+// per-thread LDC for everything.  tests/test_abi.py checks the SASS for the uniform form.
+// LEVEL 0: MATRIX, DRIFT, RFKICK, KICK; 1: + MATRIX2, TKICK; 2: + MATRIX3; 3: level 0 + MATRIX_UNC (flagged option).
+// The planner picks the lowest level a run needs; particles per thread, block size and register cap per level below.
+// Level 0: 6 particles per thread, one block of 384 threads per SM (152 registers): a register-only loop of 80
+// matrices runs at 61.5 DFMA/clk/SM = 96 % of the pipe (50.0 with shared-memory coefficients; profiles/r02_long.md).
+// The next tile is prefetched into shared memory with cp.async while the current one is in the pipe, every thread
+// copying exactly the 16-byte chunks it will read itself (no block-wide barrier in the tile loop).
 // Same arithmetic, in the same order, as chain_kernel.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kPL0 = 6;                                 // particles per thread
-constexpr int kLong0Threads = 384;
-constexpr int kLong0Regs = 160;
-template <int MAXOPS>
-constexpr int chain_long0_smem_bytes() { return 6 * kLong0Threads * kPL0 * 8; }
+template <int LEVEL> struct LongCfg;
+template <> struct LongCfg<0> { static constexpr int NT = 384, PL = 6, REGS = 160; };
+template <> struct LongCfg<1> { static constexpr int NT = ELG_L1_NT, PL = ELG_L1_PL, REGS = ELG_L1_REGS; };
+template <> struct LongCfg<2> { static constexpr int NT = ELG_L2_NT, PL = ELG_L2_PL, REGS = ELG_L2_REGS; };
+template <> struct LongCfg<3> { static constexpr int NT = 384, PL = 6, REGS = 160; };
+__host__ __device__ constexpr int long_pl(int level) { return level == 0 ? LongCfg<0>::PL : level == 1 ? LongCfg<1>::PL : level == 2 ? LongCfg<2>::PL : LongCfg<3>::PL; }
+template <int LEVEL>
+constexpr int chain_long_smem_bytes() { return 6 * LongCfg<LEVEL>::NT * LongCfg<LEVEL>::PL * 8; }
 
 // `zero` is a 0 loaded from the device state (opaque to the compiler, and a per-thread value to it): OR-ing it into the
 // bits of C[r] makes C[r] a vector value once per ROW without changing a bit of it, so that every DFMA of the row has
@@ -712,13 +556,14 @@ __device__ __forceinline__ void matrix_map_uniform(const double* __restrict__ c,
     }
 }
 
-template <int MAXOPS, int P>
+template <int MAXOPS, int P, int LEVEL>
 __device__ __forceinline__ void apply_ops_uniform(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
     const long long zero = a.c.st->zero_bits;                    // 0, but loaded: opaque to the compiler, and a vector value
     const int n_ops = a.c.n_ops;
     int op = 0;
     while (op < n_ops) {
-        if (a.type[op] == OP_MATRIX) {
+        const int ty = a.type[op];
+        if (ty == OP_MATRIX) {
             const int end = op + a.mat_run[op];                  // [op, end): consecutive MATRIX maps
 #pragma unroll 1
             for (; op + 1 < end; op += 2) {                      // pairs: v -> w -> v, no copy-back; nothing else in this loop
@@ -735,20 +580,48 @@ __device__ __forceinline__ void apply_ops_uniform(const ChainArgs<MAXOPS>& a, do
                     for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
                 op++;
             }
+        } else if (LEVEL == 3 && ty == OP_MATRIX_UNC) {
+            const int end = op + a.mat_run[op];                  // consecutive MATRIX_UNC maps (host-computed like MATRIX)
+#pragma unroll 1
+            for (; op + 1 < end; op += 2) {
+                double w[P][6];
+                matrix_unc_map_uniform<P>(a.coef[op], zero, v, w);
+                matrix_unc_map_uniform<P>(a.coef[op + 1], zero, w, v);
+            }
+            if (op < end) {
+                double w[P][6];
+                matrix_unc_map_uniform<P>(a.coef[op], zero, v, w);
+#pragma unroll
+                for (int p = 0; p < P; p++)
+#pragma unroll
+                    for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+                op++;
+            }
+        } else if ((LEVEL == 1 || LEVEL == 2) && (ty == OP_MATRIX2 || (LEVEL == 2 && ty == OP_MATRIX3))) {
+            double w[P][6];
+            matrix_map_uniform<P>(a.coef[op], zero, v, w);
+            matrix2_terms<P>(a.coef[op + 1], v, w);              // slots op + 1 .. op + 3: Tt[21][6]
+            if (LEVEL == 2 && ty == OP_MATRIX3) matrix3_terms<P>(a.coef[op + 4], zero, v, w);     // op + 4 .. op + 11: Ut[56][6]
+#pragma unroll
+            for (int p = 0; p < P; p++)
+#pragma unroll
+                for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
+            op += (ty == OP_MATRIX3) ? 12 : 4;
         } else {
-            other_map<P, false>(a.type[op], a.coef[op], a.c, v);
+            other_map<P, (LEVEL == 1 || LEVEL == 2)>(ty, a.coef[op], a.c, v);
             op++;
         }
     }
 }
 
-template <int MAXOPS>
-__global__ void __maxnreg__(kLong0Regs) chain_long0_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
-    constexpr int PL = kPL0;
-    constexpr int NT = kLong0Threads, NW = NT / 32;
+template <int MAXOPS, int LEVEL>
+__global__ void __maxnreg__(LongCfg<LEVEL>::REGS) chain_long_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+    constexpr int PL = LongCfg<LEVEL>::PL;
+    constexpr int NT = LongCfg<LEVEL>::NT, NW = NT / 32;
     constexpr int kTileL = NT * PL;
     constexpr int H = PL / 2;
     constexpr int kSub = 2 * NT;
+    static_assert(PL % 2 == 0, "128-bit accesses: particles per thread come in pairs");
     extern __shared__ __align__(16) double s_tile0[];            // [6][H][kSub]: thread t owns doubles 2t, 2t+1 of each row
     const ChainCommon& c = a.c;
     const long long n_all = c.st->n_alive[c.cur];
@@ -788,7 +661,7 @@ __global__ void __maxnreg__(kLong0Regs) chain_long0_kernel(const __grid_constant
         const long long next = tile + gridDim.x;
         if (next < n_tiles) prefetch(next);                      // own slots only: already in registers
 
-        apply_ops_uniform<MAXOPS, PL>(a, v);
+        apply_ops_uniform<MAXOPS, PL, LEVEL>(a, v);
 
         const long long t0 = c.range_lo + tile * kTileL + (long long)threadIdx.x * 2;
 #pragma unroll

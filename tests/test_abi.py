@@ -125,3 +125,37 @@ def test_rfcw_composite_shares_one_histogram_pass():
         if e["type"] == "TRWAKE":
             e["nb"] = 256
     assert elg.Beamline(e2).launches_per_turn("none") == 3 * (1 + 2 + 2 + 1 + 2 + 4) + 1
+
+
+def test_long_run_kernels_use_uniform_coefficient_operands():
+    """The fp64-bound long-run kernels must read their coefficients as uniform-register operands (DFMA R, R, UR, R fed
+    by UR-indexed LDCU): ptxas chooses that form by heuristics (elg_kernels.cuh, chain_long_kernel), so the SASS of the
+    built library is checked.  A per-thread LDC fallback or register spills would cost the headline 10-20 %."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    elg.lib()
+    from paper_1710_07350_b200.build import LIB
+    sass = subprocess.run([cuobjdump, "-sass", LIB], capture_output=True, text=True, check=True).stdout
+    kernels = {}
+    name = None
+    for line in sass.splitlines():
+        if "Function :" in line:
+            name = line.split("Function :")[1].strip()
+            kernels[name] = []
+        elif name is not None:
+            kernels[name].append(line)
+    seen = 0
+    for level in range(4):
+        body = [l for k, v in kernels.items() if f"chain_long_kernelILi80ELi{level}E" in k for l in v]
+        assert body, f"chain_long_kernel level {level} not found in the library"
+        seen += 1
+        dfma = [l for l in body if " DFMA " in l]
+        uniform = [l for l in dfma if "UR" in l]
+        spills = [l for l in body if " LDL" in l or " STL" in l]
+        assert len(uniform) >= 0.85 * len(dfma), f"level {level}: {len(uniform)} of {len(dfma)} DFMA take a uniform operand"
+        assert sum("LDCU" in l and "UR" in l.split("c[0x0]")[-1] for l in body) >= 40, f"level {level}: UR-indexed LDCU missing"
+        assert len(spills) <= 8, f"level {level}: {len(spills)} local-memory instructions (register spills)"
+    assert seen == 4
