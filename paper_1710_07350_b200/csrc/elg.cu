@@ -220,8 +220,9 @@ int32_t long_setup_once() {
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<1>()));
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<2>()));
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<3>()));
-        ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
-        ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
+        ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
+        ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
+        ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
         done = true;
     }
     return ELG_OK;
@@ -519,7 +520,8 @@ struct Tracker {
         return (int)g;
     }
 
-    template <int MAXOPS, bool COMPACT, int P, int EXT>                // EXT: 0 basic maps, 1 + MATRIX2 / TKICK, 2 + MATRIX3
+    // EXT: 0 basic maps, 1 + MATRIX2 / TKICK, 2 + MATRIX3, 3 pattern matrices.  MOM: moment epilogue (record slot rec_count)
+    template <int MAXOPS, bool COMPACT, int P, int EXT, bool MOM = false>
     void launch_chain(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm, unsigned rmask, unsigned wmask) {
         count();
         if (!b) return;
@@ -543,6 +545,7 @@ struct Tracker {
         c.range_lo = range_lo; c.range_hi = range_hi;
         c.V = b->V; c.nb = kick_nb; c.interp = kick_interp;
         c.Vx = b->Vt; c.Vy = b->Vt + tk_nb; c.t_nb = tk_nb; c.t_interp = tk_interp;
+        c.mom_partial = b->mom_partial; c.mom_record = b->records + 43 * b->rec_count;
         for (size_t k = 0; k < pending.size(); k++) {
             a.type[k] = pending[k].type;
             std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
@@ -557,9 +560,9 @@ struct Tracker {
         int grid = 0;
         if constexpr (MAXOPS == kMaxOpsLarge) grid = cached_grid((const void*)chain_long_kernel<MAXOPS, EXT>, chain_long_smem_bytes<EXT>(), LongCfg<EXT>::NT);
         else if constexpr (COMPACT) {
-            grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0)>, compact_smem_bytes(), kC2Threads);
+            grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0), MOM>, compact_smem_bytes(), kC2Threads);
             if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
-        } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, (EXT != 0)>, 0);
+        } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, (EXT != 0), MOM>, 0);
         if (!ok()) return;
         if ((long long)(mm_slot + 1) * grid > kMmPartials) { rc = fail(ELG_ECAPACITY, "elg_upload_and_track: too many chunks for the min/max partial slots"); return; }
         c.mm_partial = b->mm_partial + 2LL * mm_slot * grid;          // one slot of partials per chunk
@@ -571,24 +574,31 @@ struct Tracker {
             else if constexpr (COMPACT)
             {
                 void* kargs[] = {(void*)&a};                     // cooperative: every block resident (static tiles)
-                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS, (EXT != 0)>, dim3(grid), dim3(kC2Threads), kargs,
+                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS, (EXT != 0), MOM>, dim3(grid), dim3(kC2Threads), kargs,
                                                   compact_smem_bytes(), b->stream),
                       "compact_kernel cooperative launch");
             }
             else
-                chain_kernel<MAXOPS, P, (EXT != 0)><<<grid, kBlock, 0, b->stream>>>(a);
+                chain_kernel<MAXOPS, P, (EXT != 0), MOM><<<grid, kBlock, 0, b->stream>>>(a);
         }
         check(cudaGetLastError(), "chain_kernel launch");
         if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
     }
 
-    // launch the pending maps (+ aperture terminator, + min/max epilogue)
+    // launch the pending maps (+ aperture terminator, + min/max epilogue, + moment epilogue when a record follows)
+    bool want_mom = false;         // set by moments_record(): the run being flushed is followed by a record
+    bool mom_fused = false;        // ... and this flush has taken it in its epilogue
     void flush(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm) {
         if (!ok()) return;
         if (ap_type == AP_NONE && pending.empty() && !want_mm) return;
         // a long run that ends in an aperture: the maps go through the fp64-bound long-run kernel, the
         // aperture and the compaction follow as a run of their own (112 B per particle more, rare)
-        if (ap_type != AP_NONE && pending.size() > (size_t)kMaxOpsSmall) flush(AP_NONE, 0, 0, 0, false);
+        if (ap_type != AP_NONE && pending.size() > (size_t)kMaxOpsSmall) {
+            const bool keep = want_mom;
+            want_mom = false;
+            flush(AP_NONE, 0, 0, 0, false);
+            want_mom = keep;
+        }
         unsigned rmask = 0, wmask = 0;
         for (const HostOp& op : pending) {
             switch (op.type) {
@@ -625,8 +635,16 @@ struct Tracker {
                 for (HostOp& op : pending)
                     if (op.type == OP_MATRIX_UNC) { op.type = OP_MATRIX; std::memcpy(op.coef, op.dense, sizeof op.coef); }
         }
+        // moment epilogue: short runs of the basic maps over the whole live set (the record needs all six coordinates)
+        const bool mom = want_mom && !large && ext == 0 && range_hi < 0;
+        if (mom) { rmask = 0x3F; mom_fused = true; }
 #define ELG_LAUNCH(M, C, PP, E) launch_chain<M, C, PP, E>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
-        if (large) {
+#define ELG_LAUNCH_MOM(M, C, PP) launch_chain<M, C, PP, 0, true>(ap_type, ap_x, ap_y, te_code, want_mm, rmask, wmask)
+        if (mom) {
+            if (compact) ELG_LAUNCH_MOM(kMaxOpsSmall, true, 2);
+            else ELG_LAUNCH_MOM(kMaxOpsSmall, false, 2);              // (27 sums + 4 particles per thread would spill)
+        }
+        else if (large) {
             if (ext == 3) ELG_LAUNCH(kMaxOpsLarge, false, 0, 3);
             else if (ext == 2) ELG_LAUNCH(kMaxOpsLarge, false, 0, 2);
             else if (ext == 1) ELG_LAUNCH(kMaxOpsLarge, false, 0, 1);
@@ -636,6 +654,7 @@ struct Tracker {
         else if (p4) { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 4, 1); else ELG_LAUNCH(kMaxOpsSmall, false, 4, 0); }
         else         { if (ext) ELG_LAUNCH(kMaxOpsSmall, false, 2, 1); else ELG_LAUNCH(kMaxOpsSmall, false, 2, 0); }
 #undef ELG_LAUNCH
+#undef ELG_LAUNCH_MOM
         if (compact || (wmask & 0x10)) mm_valid = want_mm;
         else mm_valid = mm_valid || want_mm;
         pending.clear();
@@ -700,13 +719,19 @@ struct Tracker {
         }
     }
 
-    void moments_record() {
-        flush(AP_NONE, 0, 0, 0, false);
+    // one record (G26) of the live set as it is after the pending maps (and the aperture ap_type, if any): taken in the
+    // epilogue of the run that is flushed when that is possible, else by a pass of moments_kernel
+    void moments_record(int ap_type = AP_NONE, double ap_x = 0, double ap_y = 0, long long te_code = 0, bool want_mm = false) {
         if (!ok()) return;
-        count();
+        if (b && b->rec_count == kRecCap) flush_records();
+        want_mom = true; mom_fused = false;
+        flush(ap_type, ap_x, ap_y, te_code, want_mm);
+        want_mom = false;
+        if (!ok()) return;
         rec_total++;
+        if (mom_fused) { if (b) b->rec_count++; return; }
+        count();
         if (!b) return;
-        if (b->rec_count == kRecCap) flush_records();
         MomArgs m;
         for (int k = 0; k < 6; k++) m.src[k] = b->coord(b->cur_buf, k);
         m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial;
@@ -926,6 +951,7 @@ struct Tracker {
             if (skip_next) { skip_next = false; continue; }           // TRWAKE merged into the preceding WAKE
             const elg_element& e = bl->e[k];
             const double s_here = bl->ring ? std::fma((double)turn, bl->length, bl->s_design[k]) : bl->s_design[k];   // G8
+            bool recorded = false;
             HostOp op{};
             switch (e.type) {
                 case ELG_DRIFT: op.type = OP_DRIFT; op.coef[0] = e.L; push(op); break;
@@ -949,13 +975,15 @@ struct Tracker {
                     break;
                 case ELG_RCOL: case ELG_ECOL: {
                     const bool rect = e.type == ELG_RCOL;                    // ECOL carries 1/a, 1/b (G17)
-                    flush(rect ? AP_RCOL : AP_ECOL, rect ? e.ax : 1.0 / e.ax, rect ? e.ay : 1.0 / e.ay,
-                          (turn << 32) | k, next_is_hist(k, ne));
+                    const int ap = rect ? AP_RCOL : AP_ECOL;
+                    const double px = rect ? e.ax : 1.0 / e.ax, py = rect ? e.ay : 1.0 / e.ay;
+                    if (mom == ELG_MOM_ELEMENT) { moments_record(ap, px, py, (turn << 32) | k, next_is_hist(k, ne)); recorded = true; }
+                    else flush(ap, px, py, (turn << 32) | k, next_is_hist(k, ne));
                     break;
                 }
                 case ELG_WAKE: case ELG_HISTO: case ELG_TRWAKE: wake_or_histo(k, s_here); break;
             }
-            if (mom == ELG_MOM_ELEMENT) moments_record();                                    // G26
+            if (mom == ELG_MOM_ELEMENT && !recorded) moments_record();                       // G26
         }
         if (mom == ELG_MOM_TURN) moments_record();
     }

@@ -92,6 +92,8 @@ struct ChainCommon {
     int t_interp;
     long long range_lo;        // chain kernels work on particles [range_lo, min(range_hi, n_alive)); range_hi < 0: n_alive
     long long range_hi;        // (pipelined upload: one range per chunk, elg_upload_and_track)
+    double* mom_partial;       // moment epilogue (MOM instantiations): per-block partials [kNMom][gridDim.x]
+    double* mom_record;        //   and the 43-double record to fill (n, centroid, Sigma), a13 / G26
 };
 
 template <int MAXOPS>
@@ -123,6 +125,51 @@ __device__ __forceinline__ double ld_stream1(const double* p) {
     asm volatile("ld.global.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
     return r;
 }
+
+// asynchronous copies, mbarriers, named barriers (PTX)
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
+    const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc, int src_bytes) {
+    const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gsrc), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// mbarrier + 1-D bulk copy (TMA unit, SASS UBLKCP): global -> shared without registers or L1, completion counted in bytes
+__device__ __forceinline__ unsigned int smem_u32(const void* p) { return (unsigned int)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned int bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned int parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "MBAR_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra MBAR_DONE_%=;\n"
+        "bra MBAR_WAIT_%=;\n"
+        "MBAR_DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, unsigned int bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+template <int ID, int N>
+__device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(N) : "memory"); }
 
 // bin of a time coordinate (G10): floor((s*inv_bc - t_lo)*inv_dt) in [0, nb) else -1
 __device__ __forceinline__ int bin_of(double s, double inv_bc, double t_lo, double inv_dt, int nb, double* u_out) {
@@ -387,6 +434,105 @@ __device__ __forceinline__ unsigned long long pack_status(unsigned int epoch, un
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Moments (a13; G20) as pieces shared by moments_kernel and by the moment EPILOGUE of the fused
+// kernels (statistics after an element without a second pass over the particles): shifted one-pass
+// sums of d = v - K, a fixed shuffle tree per block, per-block partials combined in block order by the last block
+// to finish (the paper's "last block" scheme) -- deterministic for a fixed grid.
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void moments_add(double (&acc)[kNMom], const double (&x)[6], const double (&K)[6]) {
+    double d[6];
+#pragma unroll
+    for (int c = 0; c < 6; c++) d[c] = x[c] - K[c];
+    int q = 6;
+#pragma unroll
+    for (int r = 0; r < 6; r++) {
+        acc[r] += d[r];
+#pragma unroll
+        for (int c = r; c < 6; c++) { acc[q] = fma(d[r], d[c], acc[q]); q++; }
+    }
+}
+
+// every thread of the block calls this once with its sums; n_ptr: where the live count the record reports is found
+// (read after every block has finished).  NWARPS warps take part; barrier_id 0 = __syncthreads.
+template <int NWARPS, int BAR_ID>
+__device__ __forceinline__ void moments_finish(const double (&acc)[kNMom], const double (&K)[6], DevState* st, const long long* n_ptr,
+                                               double* partial, double* rec) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __shared__ double s_part[NWARPS][kNMom];
+    __shared__ double s_tot[kNMom];
+    __shared__ bool s_last;
+    auto block_sync = [&]() {
+        if constexpr (BAR_ID == 0) __syncthreads();
+        else named_barrier<BAR_ID, NWARPS * 32>();
+    };
+#pragma unroll
+    for (int q = 0; q < kNMom; q++) {
+        double x = acc[q];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
+        if (lane == 0) s_part[wid][q] = x;
+    }
+    block_sync();
+    if (threadIdx.x < kNMom) {
+        double x = 0.0;
+        for (int w = 0; w < NWARPS; w++) x += s_part[w][threadIdx.x];
+        partial[(long long)threadIdx.x * gridDim.x + blockIdx.x] = x;
+    }
+    __threadfence();
+    block_sync();
+    if (threadIdx.x == 0) s_last = (atomicAdd(&st->mom_done, 1u) == gridDim.x - 1);
+    block_sync();
+    if (!s_last) return;
+    __threadfence();
+    // the last block combines the per-block partials: thread t takes blocks t, t + NT, ... (all 27 loads of a step are
+    // independent and in flight together), then the same fixed tree as above
+    double tot[kNMom];
+#pragma unroll
+    for (int q = 0; q < kNMom; q++) tot[q] = 0.0;
+    for (int bk = threadIdx.x; bk < (int)gridDim.x; bk += NWARPS * 32) {
+        double t[kNMom];
+#pragma unroll
+        for (int q = 0; q < kNMom; q++) t[q] = __ldcg(partial + (long long)q * gridDim.x + bk);
+#pragma unroll
+        for (int q = 0; q < kNMom; q++) tot[q] += t[q];
+    }
+#pragma unroll
+    for (int q = 0; q < kNMom; q++) {
+        double x = tot[q];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
+        if (lane == 0) s_part[wid][q] = x;
+    }
+    block_sync();
+    if (threadIdx.x < kNMom) {
+        double x = 0.0;
+        for (int w = 0; w < NWARPS; w++) x += s_part[w][threadIdx.x];
+        s_tot[threadIdx.x] = x;
+    }
+    block_sync();
+    if (threadIdx.x == 0) {
+        const long long n = *reinterpret_cast<const volatile long long*>(n_ptr);
+        rec[0] = (double)n;
+        if (n <= 0) {
+            for (int k = 1; k < 43; k++) rec[k] = 0.0;                       // G28
+        } else {
+            const double inv_n = 1.0 / (double)n;
+            double m[6];
+            for (int c = 0; c < 6; c++) { m[c] = s_tot[c] * inv_n; rec[1 + c] = K[c] + m[c]; }
+            int q = 6;
+            for (int r = 0; r < 6; r++)
+                for (int c = r; c < 6; c++) {
+                    const double val = s_tot[q] * inv_n - m[r] * m[c];
+                    rec[7 + 6 * r + c] = val;
+                    rec[7 + 6 * c + r] = val;
+                    q++;
+                }
+        }
+        st->mom_done = 0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // chain_kernel: one launch applies a RUN of consecutive elements to every live particle: each
 // coordinate is loaded once (128-bit), carried in registers through all maps and stored once
 // (north_star part 1; the paper launches one kernel per element).
@@ -396,8 +542,23 @@ __device__ __forceinline__ unsigned long long pack_status(unsigned int epoch, un
 // sub-tile, warp accesses are 512 contiguous bytes).  Only the coordinates the run reads / writes are
 // loaded / stored (accessor masks).
 // ---------------------------------------------------------------------------------------------------
-template <int MAXOPS, int P, bool EXT>
-__global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+// The shift K of the moment epilogue: the run's maps applied to particle 0 of the store (every thread computes the
+// same K; non-finite components become 0).  It only has to lie inside the distribution (conditioning of the
+// one-pass formula: s is an absolute path length), it need not be a survivor.
+template <int MAXOPS, bool EXT>
+__device__ __forceinline__ void moment_shift(const ChainArgs<MAXOPS>& a, long long n, double (&K)[6]) {
+    double k2[2][6];
+#pragma unroll
+    for (int cc = 0; cc < 6; cc++) { k2[0][cc] = (n > 0) ? __ldg(a.c.src[cc]) : 0.0; k2[1][cc] = k2[0][cc]; }
+    apply_ops<MAXOPS, 2, EXT>(a, k2);
+#pragma unroll
+    for (int cc = 0; cc < 6; cc++) K[cc] = (fabs(k2[0][cc]) < INFINITY) ? k2[0][cc] : 0.0;
+}
+
+// MOM: the run is followed by a moments record (G26): the 27 shifted sums are accumulated on the mapped particles
+// while they are in registers and the record is finished by the last block -- no second pass over the particles.
+template <int MAXOPS, int P, bool EXT, bool MOM>
+__global__ void __launch_bounds__(kBlock, ((P >= 4 || MOM) ? 2 : 3)) chain_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
     constexpr int H = P / 2;                    // sub-tiles per tile
     constexpr int kSub = 2 * kBlock;            // particles per sub-tile
     constexpr int kTileP = kBlock * P;
@@ -407,6 +568,12 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
     const long long n_tiles = (n > c.range_lo) ? (n - c.range_lo + kTileP - 1) / kTileP : 0;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double mn = INFINITY, mx = -INFINITY;
+    double K[MOM ? 6 : 1], acc[MOM ? kNMom : 1];
+    if constexpr (MOM) {
+        moment_shift<MAXOPS, EXT>(a, n, K);
+#pragma unroll
+        for (int q = 0; q < kNMom; q++) acc[q] = 0.0;
+    }
 
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const long long t0 = c.range_lo + tile * kTileP + (long long)threadIdx.x * 2;
@@ -446,8 +613,13 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
                 if (i0 < n) { mn = fmin(mn, v[2 * h][4]); mx = fmax(mx, v[2 * h][4]); }
                 if (full) { mn = fmin(mn, v[2 * h + 1][4]); mx = fmax(mx, v[2 * h + 1][4]); }
             }
+            if constexpr (MOM) {
+                if (i0 < n) moments_add(acc, v[2 * h], K);
+                if (full) moments_add(acc, v[2 * h + 1], K);
+            }
         }
     }
+    if constexpr (MOM) moments_finish<kWarps, 0>(acc, K, c.st, &c.st->n_alive[c.cur], c.mom_partial, c.mom_record);
 
     if (c.want_minmax) {                                       // exact min/max of s (a8): order-independent
 #pragma unroll
@@ -465,51 +637,6 @@ __global__ void __launch_bounds__(kBlock, (P >= 4 ? 2 : 3)) chain_kernel(const _
         }
     }
 }
-
-// ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
-    const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gsrc), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc, int src_bytes) {
-    const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gsrc), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// mbarrier + 1-D bulk copy (TMA unit, SASS UBLKCP): global -> shared without registers or L1, completion counted in bytes
-__device__ __forceinline__ unsigned int smem_u32(const void* p) { return (unsigned int)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned int bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned int parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "MBAR_WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra MBAR_DONE_%=;\n"
-        "bra MBAR_WAIT_%=;\n"
-        "MBAR_DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, unsigned int bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
-                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-template <int ID, int N>
-__device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(N) : "memory"); }
 
 // ---------------------------------------------------------------------------------------------------
 // chain_long_kernel: long runs of maps (cfg3: 80 MATRIX per launch), the kernel the headline metric spends 97 % of
@@ -762,8 +889,8 @@ constexpr int kCompactMaxGrid = kPoll * kC2NT + 1;
 constexpr int kStatusTile = 256;                        // tile_status is sized for tiles of at least this many particles
 constexpr int compact_smem_bytes() { return kC2S * 7 * kC2Tile * 8; }
 
-template <int MAXOPS, bool EXT>
-__global__ void __launch_bounds__(kC2Threads, ELG_C2_BLOCKS) compact_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+template <int MAXOPS, bool EXT, bool MOM>
+__global__ void __launch_bounds__(kC2Threads, (MOM ? 1 : ELG_C2_BLOCKS)) compact_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
     constexpr int NT = kC2NT, PP = kC2PP, S = kC2S, D = kC2D, TILE = kC2Tile, NW = NT / 32;
     static_assert(D >= 1 && S - D - 1 >= 0, "ring: S = D + F + 1");
     static_assert(kC2Tile >= kStatusTile && kC2Tile % 2 == 0, "tile_status capacity; 16-byte bulk copies");
@@ -812,6 +939,12 @@ __global__ void __launch_bounds__(kC2Threads, ELG_C2_BLOCKS) compact_kernel(cons
 #pragma unroll
     for (int d = 0; d < D; d++) tot_hist[d] = 0;
     long long my_incl = 0;                                       // inclusive survivor prefix at my last resolved tile
+    double K[MOM ? 6 : 1], acc[MOM ? kNMom : 1];                 // moment epilogue over the survivors (G26)
+    if constexpr (MOM) {
+        moment_shift<MAXOPS, EXT>(a, n, K);
+#pragma unroll
+        for (int q = 0; q < kNMom; q++) acc[q] = 0.0;
+    }
 
     for (long long it = 0; it < n_it + D; it++) {
         const int par = (int)(it & 1);
@@ -895,6 +1028,7 @@ __global__ void __launch_bounds__(kC2Threads, ELG_C2_BLOCKS) compact_kernel(cons
                     for (int cc = 0; cc < 6; cc++) stage[cc * TILE + pos] = v[q][cc];
                     stage[6 * TILE + pos] = __longlong_as_double(id[q]);
                     if (c.want_minmax && surv[q]) { mn = fmin(mn, v[q][4]); mx = fmax(mx, v[q][4]); }
+                    if constexpr (MOM) { if (surv[q]) moments_add(acc, v[q], K); }
                 }
             }
         }
@@ -958,6 +1092,8 @@ __global__ void __launch_bounds__(kC2Threads, ELG_C2_BLOCKS) compact_kernel(cons
         c.st->n_alive[c.cur ^ 1] = 0;
         c.st->n_lost[c.cur ^ 1] = lost_base;
     }
+    // the survivor count of the record was written above by the block that resolved the last tile, before its arrival
+    if constexpr (MOM) moments_finish<NW, 1>(acc, K, c.st, &c.st->n_alive[c.cur ^ 1], c.mom_partial, c.mom_record);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -1427,7 +1563,6 @@ struct MomArgs {
 
 __global__ void __launch_bounds__(kBlock) moments_kernel(const MomArgs a) {
     const long long n = a.st->n_alive[a.cur];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double K[6];
 #pragma unroll
     for (int c = 0; c < 6; c++) K[c] = (n > 0) ? __ldg(a.src[c]) : 0.0;
@@ -1437,79 +1572,21 @@ __global__ void __launch_bounds__(kBlock) moments_kernel(const MomArgs a) {
 
     const long long stride = (long long)gridDim.x * kTile;
     for (long long i0 = (long long)blockIdx.x * kTile + (long long)threadIdx.x * kP; i0 < n; i0 += stride) {
-        double d[kP][6];
+        double x[kP][6];
         const bool full = (i0 + kP <= n);
 #pragma unroll
         for (int c = 0; c < 6; c++) {
             if (full) {
                 const double2 t = ld_stream2(a.src[c] + i0);
-                d[0][c] = t.x - K[c]; d[1][c] = t.y - K[c];
+                x[0][c] = t.x; x[1][c] = t.y;
             } else {
-                d[0][c] = ld_stream1(a.src[c] + i0) - K[c]; d[1][c] = 0.0;
+                x[0][c] = ld_stream1(a.src[c] + i0); x[1][c] = 0.0;
             }
         }
-#pragma unroll
-        for (int p = 0; p < kP; p++) {
-            if (p == 1 && !full) break;
-            int q = 6;
-#pragma unroll
-            for (int r = 0; r < 6; r++) {
-                acc[r] += d[p][r];
-#pragma unroll
-                for (int c = r; c < 6; c++) { acc[q] = fma(d[p][r], d[p][c], acc[q]); q++; }
-            }
-        }
+        moments_add(acc, x[0], K);
+        if (full) moments_add(acc, x[1], K);
     }
-    __shared__ double s_part[kWarps][kNMom];
-#pragma unroll
-    for (int q = 0; q < kNMom; q++) {
-        double x = acc[q];
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
-        if (lane == 0) s_part[wid][q] = x;
-    }
-    __syncthreads();
-    if (threadIdx.x < kNMom) {
-        double x = 0.0;
-        for (int w = 0; w < kWarps; w++) x += s_part[w][threadIdx.x];
-        a.partial[(long long)threadIdx.x * gridDim.x + blockIdx.x] = x;
-    }
-    __shared__ bool s_last;
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(&a.st->mom_done, 1u) == gridDim.x - 1);
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    __shared__ double s_tot[kNMom];
-    for (int q = wid; q < kNMom; q += kWarps) {                 // one warp per quantity, blocks in order
-        double x = 0.0;
-        for (int b = lane; b < (int)gridDim.x; b += 32) x += __ldcg(a.partial + (long long)q * gridDim.x + b);
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
-        if (lane == 0) s_tot[q] = x;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double* rec = a.record;
-        rec[0] = (double)n;
-        if (n <= 0) {
-            for (int k = 1; k < 43; k++) rec[k] = 0.0;                       // G28
-        } else {
-            const double inv_n = 1.0 / (double)n;
-            double m[6];
-            for (int c = 0; c < 6; c++) { m[c] = s_tot[c] * inv_n; rec[1 + c] = K[c] + m[c]; }
-            int q = 6;
-            for (int r = 0; r < 6; r++)
-                for (int c = r; c < 6; c++) {
-                    const double val = s_tot[q] * inv_n - m[r] * m[c];
-                    rec[7 + 6 * r + c] = val;
-                    rec[7 + 6 * c + r] = val;
-                    q++;
-                }
-        }
-        a.st->mom_done = 0;
-    }
+    moments_finish<kWarps, 0>(acc, K, a.st, &a.st->n_alive[a.cur], a.partial, a.record);
 }
 
 // ---------------------------------------------------------------------------------------------------

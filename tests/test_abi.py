@@ -64,10 +64,10 @@ def test_beamline_design_orbit_and_validation():
 def test_run_planning_fuses_elements():
     """north_star part 1: runs of consecutive elements are one launch."""
     # cfg0: [DRIFT, MATRIX, RCOL] -> 1 fused compacting launch; WAKE -> window, histogram, samples,
-    # convolution; the kick is flushed as one launch; + 1 moments kernel per turn
+    # convolution; the kick is flushed as one launch, which also takes the turn's moments record
     bl = elg.Beamline(make_workload("cfg0").elements)
     assert bl.launches_per_turn("none") == 1 + 4 + 1
-    assert bl.launches_per_turn("turn") == 1 + 4 + 1 + 1
+    assert bl.launches_per_turn("turn") == 1 + 4 + 1          # the record rides in the kick run's epilogue
     # cfg3: 201 maps -> ceil(201/80) = 3 chain launches (last one carries the min/max epilogue)
     bl = elg.Beamline(make_workload("cfg3", n=8).elements, ring=True)
     assert bl.launches_per_turn("none") == 3 + 4 + 1
@@ -76,9 +76,9 @@ def test_run_planning_fuses_elements():
     # cfg4: 20 x [RCOL, HISTO, DRIFT]: every RCOL launch carries the preceding DRIFT and the min/max
     # epilogue for the HISTO: 20 x (1 + 2) + the trailing DRIFT
     assert elg.Beamline(make_workload("cfg4", n=8).elements).launches_per_turn("none") == 20 * 3 + 1
-    # cfg1 with moments after every element: one chain launch + one moments launch per element
+    # cfg1 with moments after every element: ONE launch per element, the record taken in its epilogue
     bl = elg.Beamline(make_workload("cfg1", n=8).elements)
-    assert bl.launches_per_turn("element") == 77 * 2
+    assert bl.launches_per_turn("element") == 77
     assert bl.launches_per_turn("none") == 25 + 1
 
 
