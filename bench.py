@@ -31,6 +31,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+KERNEL_NAMES = {"chain": "chain_kernel", "chain_compact": "compact_kernel", "chain_long": "chain_long_kernel", "hist": "hist_kernel",
+                "moments": "moments_kernel", "window": "window_kernel", "conv": "conv_kernel", "wake_samples": "wake_samples_kernel"}
 METRIC = "Mparticle-element passes/s"
 UNIT = "Mpasses/s"
 # algorithmic fp64 flops per particle per element (MATRIX = 36 FMA, the constant C
@@ -151,14 +153,19 @@ def run_reference(args):
     mom = w.moments_every
     per_turn = w.n_pass_elements
     for _ in range(args.warmup):
+        if not w.ring:
+            ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
         ob.track(obl, 1, moments_every=mom, n_threads=threads)
     passes = 0
-    t0 = time.perf_counter()
+    dt = 0.0
     for _ in range(args.steps):
+        if not w.ring:                                 # a line is traversed once: fresh bunch per step (not timed)
+            ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
         n_in = ob.n_alive
+        t0 = time.perf_counter()
         ob.track(obl, 1, moments_every=mom, n_threads=threads)
+        dt += time.perf_counter() - t0
         passes += n_in * per_turn          # ring workloads have no aperture; line workloads: upper bound
-    dt = time.perf_counter() - t0
     value = passes / dt / 1e6
     sample = f"{args.cpu_sample} particles of {w.name}, {args.steps} turn(s), {threads} threads"
     line = {
@@ -175,29 +182,55 @@ def run_reference(args):
     return 0
 
 
-def cpu_baseline(workload_name: str, sample: int):
+def _time_oracle(workload_name: str, sample: int, threads: int, budget_s: float, max_turns: int):
     from elg_inputs import make_workload
     from oracle import elgo
-    elgo.build()
-    cores = os.cpu_count() or 1
-    threads = max(1, min(cores, 64))
     w = make_workload(workload_name, n=sample)
     v0 = w.particles()
     ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
     obl = elgo.Beamline(w.elements, ring=w.ring)
     ob.track(obl, 1, moments_every=w.moments_every, n_threads=threads)          # warm-up turn
+    if not w.ring:
+        ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
     turns = 0
+    passes = 0.0
     t0 = time.perf_counter()
     while True:
+        if not w.ring:                                                           # a line is traversed once per fresh bunch
+            ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
+        n_in = ob.n_alive
         ob.track(obl, 1, moments_every=w.moments_every, n_threads=threads)
         turns += 1
-        if time.perf_counter() - t0 > 10.0 or turns >= 50:
+        if w.ring:
+            passes += float(n_in) * w.n_pass_elements
+        else:
+            _, _, elem, _ = ob.lost()
+            lost_at = np.bincount(elem, minlength=len(w.elements)) if elem.size else np.zeros(len(w.elements), dtype=np.int64)
+            n = sample
+            for k, e in enumerate(w.elements):
+                if e["type"] != "HISTO":
+                    passes += n
+                n -= int(lost_at[k])
+        if time.perf_counter() - t0 > budget_s or turns >= max_turns:
             break
     dt = time.perf_counter() - t0
-    value = sample * w.n_pass_elements * turns / dt / 1e6
-    return {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": f"{sample} particles of {w.name} x {turns} turn(s) in {dt:.1f} s, {threads} threads "
-                      f"of {cores} host cores"}
+    return passes / dt / 1e6, turns, dt, w.name
+
+
+def cpu_baseline(workload_name: str, sample: int):
+    """The oracle as it stands on the host cores: all cores (chunked independent per-particle loops) and ONE
+    core (the definition of the oracle; the paper's own speed-ups are quoted against one core)."""
+    from oracle import elgo
+    elgo.build()
+    cores = os.cpu_count() or 1
+    threads = max(1, min(cores, 64))
+    v_all, turns, dt, name = _time_oracle(workload_name, sample, threads, 8.0, 50)
+    s1 = max(1000, sample // 8)
+    v_one, turns1, dt1, _ = _time_oracle(workload_name, s1, 1, 6.0, 20)
+    return {"value": v_all, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{sample} particles of {name} x {turns} turn(s) in {dt:.1f} s, {threads} threads of {cores} host cores",
+            "one_core": {"value": v_one, "unit": UNIT, "cores": 1,
+                         "sample": f"{s1} particles of {name} x {turns1} turn(s) in {dt1:.1f} s, 1 thread"}}
 
 
 # ------------------------------------------------------------------------------------------- our arm
@@ -285,7 +318,7 @@ def run_ours(args):
             passes += line_passes(gb, w)
     t_wall1 = time.perf_counter()
     launches = elg.launch_count() - launches0
-    prof = gb.profile_read()
+    prof = gb.profile_read(work=True)
     pdist.barrier()
     torch.cuda.synchronize(dev)
     time.sleep(0.15)
@@ -295,38 +328,37 @@ def run_ours(args):
     t_max, passes_all = pdist.aggregate(elapsed_ms, passes, dev if world > 1 else None)
     value = passes_all / (t_max * 1e-3) / 1e6
 
-    # ---- roofline of the dominant kernel of the step
+    # ---- roofline of the dominant kernel of the step.  Algorithmic bytes / flops come from the library (elg_profile_read:
+    # coordinates read + written x live particles of every launch, per-particle flop counts of DESIGN.md section 5), the
+    # time from CUDA events around every launch of that kernel kind inside the timed region.
     roofline = None
     kinds = {k: v for k, v in prof.items() if v[0] > 0}
     total_kernel_ms = sum(v[1] for v in kinds.values())
     dominant = max(kinds, key=lambda k: kinds[k][1]) if kinds else None
     shares = {k: round(v[1] / total_kernel_ms, 4) for k, v in kinds.items()} if kinds else {}
-    if dominant == "chain_long" and w.ring:
-        # chain_long_kernel: runs of more than 8 maps (cfg3: 80 + 80 + 41 per turn); the wake kick is a short run
-        n_short = sum(1 for e in w.elements if e["type"] == "WAKE")
-        fl = (flops_per_particle_turn(w.elements) - FLOPS["WAKE"] * n_short) * float(n0) * args.steps
-        n_l, ms = kinds["chain_long"]
-        ach = fl / (ms * 1e-3) / 1e12
-        by = 96.0 * n0 * n_l                                                      # 48 B in + 48 B out per launch
-        roofline = {"kernel": "chain_long_kernel", "bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS,
-                    "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
-                    "peak_source": "derived: 148 SMs x 64 DFMA/clk/SM x 2 x 1.965 GHz (DESIGN.md)",
-                    "traffic": ncu_traffic("chain_long_kernel", w.name),
-                    "launches": n_l, "avg_launch_ms": ms / n_l,
-                    "flops_per_launch": fl / n_l, "algorithmic_bytes_per_launch": by / n_l,
-                    "hbm_gbs": by / (ms * 1e-3) / 1e9, "hbm_frac_of_measured": by / (ms * 1e-3) / 1e9 / hbm_peak,
-                    "share_of_step": shares.get("chain_long")}
-    elif dominant is not None:
-        bpp = {"chain": 96.0, "chain_compact": 112.0, "hist": 8.0, "moments": 48.0}.get(dominant)
-        n_l, ms = kinds[dominant]
-        if bpp is not None:
-            ach = bpp * n0 * n_l / (ms * 1e-3) / 1e9
-            roofline = {"kernel": dominant + "_kernel", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
-                        "unit": "GB/s", "frac": ach / hbm_peak, "peak_source": peak_src,
-                        "traffic": ncu_traffic(dominant + "_kernel", w.name), "launches": n_l,
-                        "avg_launch_ms": ms / n_l, "algorithmic_bytes_per_launch": bpp * n0,
-                        "note": "bytes use n0 live particles per launch (upper bound when particles are lost)",
-                        "share_of_step": shares.get(dominant)}
+    fp64_peak, fp64_peak_ms = elg.dbg_fp64_peak(20000) if rank == 0 or world == 1 else (FP64_PEAK_TFLOPS, None)
+    if dominant is not None:
+        n_l, ms, by, fl = kinds[dominant]
+        intensity = fl / max(by, 1.0)                                            # flop per byte of the kernel's launches
+        alu_bound = intensity > fp64_peak * 1e12 / (hbm_peak * 1e9)
+        common = {"kernel": KERNEL_NAMES.get(dominant, dominant), "launches": n_l, "avg_launch_ms": ms / n_l,
+                  "algorithmic_bytes_per_launch": by / n_l, "flops_per_launch": fl / n_l, "flop_per_byte": intensity,
+                  "share_of_step": shares.get(dominant), "traffic": ncu_traffic(KERNEL_NAMES.get(dominant, dominant), w.name),
+                  "hbm_gbs": by / (ms * 1e-3) / 1e9, "hbm_frac_of_measured": by / (ms * 1e-3) / 1e9 / hbm_peak}
+        if alu_bound:
+            ach = fl / (ms * 1e-3) / 1e12
+            roofline = dict(common, bound="alu", achieved=ach, peak=fp64_peak, unit="TFLOP/s", frac=ach / fp64_peak,
+                            peak_source="measured in this run: elg_dbg_fp64_peak (DFMA-only kernel, %.2f ms); nominal 148 SMs x 64 "
+                                        "DFMA/clk x 2 x 1.965 GHz = %.2f" % (fp64_peak_ms or 0.0, FP64_PEAK_TFLOPS),
+                            frac_of_nominal=ach / FP64_PEAK_TFLOPS)
+        else:
+            ach = by / (ms * 1e-3) / 1e9
+            roofline = dict(common, bound="hbm", achieved=ach, peak=hbm_peak, unit="GB/s", frac=ach / hbm_peak,
+                            peak_source=peak_src, frac_of_8TBs=ach / NOMINAL_HBM_GBS)
+            if 7 * n0 * 8 < 126e6:
+                roofline["note"] = ("the %.0f MB particle store fits the 126 MB L2 and a launch lasts %.1f us: this workload is "
+                                    "launch-latency bound, the HBM fraction is not a measure of the kernel (SURVEY 8(d))"
+                                    % (7 * n0 * 8 / 1e6, ms / n_l * 1e3))
 
     # ---- end to end through the C ABI with HOST buffers: upload (pinned H2D) + one turn + record D2H
     e2e = None
@@ -360,6 +392,19 @@ def run_ours(args):
     if want_probes:
         probes = run_probes(elg, gb, restore, n0, w, hbm_peak, stream, dev, args)
 
+    if roofline is not None and probes:
+        # north_star's target sentence: ">= 70 % of B200 HBM bandwidth on the fused element-chain and compaction kernels at
+        # 1e8 particles" -- kept inside `roofline` so that it survives with the headline (fractions of the measured copy
+        # peak and of the nominal 8 TB/s)
+        def pick(wl, kern):
+            for pr in probes:
+                if pr.get("workload") == wl and pr.get("kernel") == kern:
+                    return {"gbs": pr["achieved"], "frac": pr["frac"], "frac_of_8TBs": pr["frac_of_8TBs"], "ms": pr["avg_launch_ms"]}
+            return None
+        roofline["targets"] = {"particles": n0,
+                               "chain": pick("p1-chain", "chain_kernel"),
+                               "compact_0.6pct_loss": pick("p2-chain-rcol", "compact_kernel"),
+                               "compact_10pct_loss": pick("p2-chain-rcol@10%", "compact_kernel")}
     if rank != 0:
         return 0
     cpu = None
@@ -404,15 +449,16 @@ def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
     import torch
     from elg_inputs import make_workload
     out = []
+    # (workload, moments mode, kernel kinds reported): bytes per launch come from the library (elg_profile_read)
     cases = [
-        ("p1-chain", "none", {"chain": 96.0}),
-        ("p2-chain-rcol", "none", {"chain_compact": 112.0}),
-        ("cfg0", "turn", {"chain_compact": 112.0, "hist": 8.0, "moments": 48.0, "chain": 24.0}),
-        # NEXT row f1: two dipole histograms (s, x, y: 24 B) + one plain (8 B) = 56 B over 3 launches
-        ("p5-trwake", "none", {"hist": 56.0 / 3.0}),
+        ("p1-chain", "none", ("chain",)),
+        ("p2-chain-rcol", "none", ("chain_compact",)),
+        ("p2-chain-rcol@10%", "none", ("chain_compact",)),                        # 0.6 % and ~10 % loss
+        ("cfg0", "turn", ("chain_compact", "hist", "chain")),
+        ("p5-trwake", "none", ("hist", "chain")),                                 # NEXT row f1: dipole histograms (24 B) + kicks
+        ("p6-rfcw", "none", ("hist", "chain")),                                   # NEXT row f2: one dipole pass per cavity
     ]
-    cases.insert(2, ("p2-chain-rcol@10%", "none", {"chain_compact": 112.0}))     # 0.6 % and ~10 % loss
-    for name, mom, bytes_pp in cases:
+    for name, mom, kinds_wanted in cases:
         w = make_workload("p2-chain-rcol", n=n0, half_width=197e-6) if name.endswith("@10%") else make_workload(name, n=n0)
         bl = elg.Beamline(w.elements, ring=False)
         for _ in range(3):
@@ -421,7 +467,6 @@ def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
         gb.profile(True); gb.profile_read()
         ms_total = 0.0
         k = args.probe_steps
-        passes = 0.0
         for _ in range(k):
             restore()
             ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
@@ -430,18 +475,17 @@ def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):
             ev1.record(stream)
             torch.cuda.synchronize(dev)
             ms_total += ev0.elapsed_time(ev1)
-        prof = gb.profile_read()
+        prof = gb.profile_read(work=True)
         gb.profile(False)
         passes = line_passes(gb, w)
         n_alive = gb.n_alive
-        for kind, bpp in bytes_pp.items():
-            n_l, ms = prof[kind]
+        for kind in kinds_wanted:
+            n_l, ms, by, fl = prof[kind]
             if n_l == 0:
                 continue
-            n_eff = n0 if kind in ("chain_compact",) or name == "p1-chain" else n_alive
-            ach = bpp * n_eff * n_l / (ms * 1e-3) / 1e9
-            out.append({"workload": name, "kernel": kind + "_kernel", "bound": "hbm", "particles": int(n_eff),
-                        "bytes_per_particle": bpp, "avg_launch_ms": ms / n_l, "achieved": ach, "unit": "GB/s",
+            ach = by / (ms * 1e-3) / 1e9
+            out.append({"workload": name, "kernel": KERNEL_NAMES[kind], "bound": "hbm", "launches_per_pass": n_l // k,
+                        "bytes_per_launch": by / n_l, "avg_launch_ms": ms / n_l, "achieved": ach, "unit": "GB/s",
                         "peak": hbm_peak, "frac": ach / hbm_peak, "frac_of_8TBs": ach / NOMINAL_HBM_GBS})
         out.append({"workload": name, "kernel": "whole pass", "ms_per_pass": ms_total / k,
                     "value": passes / (ms_total / k * 1e-3) / 1e6, "unit": UNIT, "n_alive_after": int(n_alive)})

@@ -213,11 +213,14 @@ int32_t elg_bunch_device_array(elg_bunch*, int32_t c, void** d_ptr);
  * With profiling on, every kernel the bunch launches is bracketed by a pair of CUDA events on the bunch's
  * stream.  elg_profile_read synchronises the stream, returns per kernel kind the number of launches and
  * their summed device time since the last read (h_launches, h_ms: ELG_K_COUNT entries each) and resets
- * the counters.  Off by default (no events are recorded). */
+ * the counters.  h_bytes / h_flops (nullable): the ALGORITHMIC work of those launches per kind -- bytes = 8 x (coordinates
+ * the run reads + coordinates it writes) x live particles of the launch (+ 16 for the IDs of a compacting run, which
+ * moves all seven arrays), flops = the per-particle flop counts of DESIGN.md section 5 x live particles -- accumulated
+ * on the device from the live count each launch sees (the host never knows it).  Off by default. */
 enum { ELG_K_CHAIN = 0, ELG_K_CHAIN_COMPACT = 1, ELG_K_WINDOW = 2, ELG_K_HIST = 3, ELG_K_WAKE_SAMPLES = 4,
        ELG_K_CONV = 5, ELG_K_MOMENTS = 6, ELG_K_CHAIN_LONG = 7, ELG_K_COUNT = 8 };
 int32_t elg_profile_enable(elg_bunch*, int32_t on);
-int32_t elg_profile_read(elg_bunch*, int64_t* h_launches, double* h_ms);
+int32_t elg_profile_read(elg_bunch*, int64_t* h_launches, double* h_ms, double* h_bytes, double* h_flops);
 
 /* ---- single-stage test hooks (not the user boundary) -------------------------------------------------
  * For the stage-by-stage parity protocol (the paper compares CPU and GPU element by element on the
@@ -239,6 +242,10 @@ int32_t elg_dbg_kick(elg_bunch*, double t_lo, double dt, int32_t nb, const doubl
 int32_t elg_dbg_tkick(elg_bunch*, double t_lo, double dt, int32_t nb, const double* d_Vx, const double* d_Vy,
                       int32_t interp);
 int32_t elg_dbg_compact(elg_bunch*, int32_t type /* ELG_RCOL | ELG_ECOL */, double ax, double ay);
+/* the fp64 roofline denominator, measured: a DFMA-only kernel (8 independent chains per thread, register operands, two
+ * blocks of 256 threads per SM) timed with CUDA events; d_scratch: >= 2048 bytes of DEVICE memory; iters: loop trips of
+ * 128 DFMA per thread.  Returns 2 x DFMA/s in TFLOP/s and the kernel time. */
+int32_t elg_dbg_fp64_peak(double* d_scratch, int64_t iters, double* h_tflops, double* h_ms, void* stream);
 int32_t elg_dbg_wake_samples(int32_t kind, int32_t nb, double dt, double f, double Q, double Rs,
                              const double* d_table, int64_t n_table, double dt_table, double* d_W, void* stream);
 int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W, int32_t nb, double q, double* d_V,

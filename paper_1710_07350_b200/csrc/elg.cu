@@ -413,7 +413,8 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     b->hist_aggregate = agg ? std::atoi(agg) : -1;                 // -1: automatic
     const char* fp = std::getenv("ELG_CHAIN_P");
     b->force_p = fp ? std::atoi(fp) : 0;
-    cudaError_t ce = cudaMemsetAsync(b->tile_status, 0, (b->stride / kStatusTile + 2) * 8, b->stream);
+    cudaError_t ce = cudaMemsetAsync(b->st, 0, sizeof(DevState), b->stream);       // incl. the work counters of elg_profile_read
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(b->tile_status, 0, (b->stride / kStatusTile + 2) * 8, b->stream);
     if (ce != cudaSuccess) { delete b; return fail(ELG_ECUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(ce)); }
     rc = elg_bunch_rewind(b);
     if (rc != ELG_OK) { delete b; return rc; }
@@ -438,14 +439,49 @@ extern "C" int32_t elg_profile_enable(elg_bunch* b, int32_t on) {
     return ELG_OK;
 }
 
-extern "C" int32_t elg_profile_read(elg_bunch* b, int64_t* h_launches, double* h_ms) {
+extern "C" int32_t elg_profile_read(elg_bunch* b, int64_t* h_launches, double* h_ms, double* h_bytes, double* h_flops) {
     if (!b || !h_launches || !h_ms) return fail(ELG_EINVAL, "elg_profile_read: bad arguments");
+    unsigned long long work[16];
+    ELG_CK(cudaMemcpyAsync(work, b->st->work, sizeof work, cudaMemcpyDeviceToHost, b->stream));
+    ELG_CK(cudaMemsetAsync(b->st->work, 0, sizeof work, b->stream));
     ELG_CK(cudaStreamSynchronize(b->stream));
     b->prof_drain();
     for (int k = 0; k < ELG_K_COUNT; k++) {
         h_launches[k] = b->prof_launches[k]; h_ms[k] = b->prof_ms[k];
+        if (h_bytes) h_bytes[k] = (double)work[2 * k];
+        if (h_flops) h_flops[k] = (double)work[2 * k + 1];
         b->prof_launches[k] = 0; b->prof_ms[k] = 0.0;
     }
+    return ELG_OK;
+}
+
+// The fp64 roofline denominator, measured: a DFMA-only kernel (8 independent chains per thread, register operands) on
+// two blocks of 256 threads per SM, timed with CUDA events on `stream`.  d_scratch: >= 2048 bytes of device memory.
+extern "C" int32_t elg_dbg_fp64_peak(double* d_scratch, int64_t iters, double* h_tflops, double* h_ms, void* stream) {
+    if (!d_scratch || iters < 1 || !h_tflops) return fail(ELG_EINVAL, "elg_dbg_fp64_peak: bad arguments");
+    int sms = 0;
+    { int32_t rc = device_sms(&sms); if (rc != ELG_OK) return rc; }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    ELG_CK(cudaEventCreate(&e0));
+    ELG_CK(cudaEventCreate(&e1));
+    const int grid = 2 * sms;
+    float ms = 0.f;
+    for (int rep = 0; rep < 4; rep++) {                                // rep 0 warms the clocks up; best of the other three
+        ELG_CK(cudaEventRecord(e0, st));
+        fp64_peak_kernel<<<grid, kBlock, 0, st>>>(d_scratch, iters, 0.999, 1e-7);
+        ELG_CK(cudaEventRecord(e1, st));
+        g_launches++;
+        ELG_CK(cudaGetLastError());
+        ELG_CK(cudaEventSynchronize(e1));
+        float t = 0.f;
+        ELG_CK(cudaEventElapsedTime(&t, e0, e1));
+        if (rep >= 1 && (ms == 0.f || t < ms)) ms = t;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    const double fma = (double)grid * kBlock * kPeakIlp * kPeakUnroll * (double)iters;
+    *h_tflops = 2.0 * fma / ((double)ms * 1e-3) / 1e12;
+    if (h_ms) *h_ms = (double)ms;
     return ELG_OK;
 }
 
@@ -546,6 +582,23 @@ struct Tracker {
         c.V = b->V; c.nb = kick_nb; c.interp = kick_interp;
         c.Vx = b->Vt; c.Vy = b->Vt + tk_nb; c.t_nb = tk_nb; c.t_interp = tk_interp;
         c.mom_partial = b->mom_partial; c.mom_record = b->records + 43 * b->rec_count;
+        c.prof_kind = b->prof_on ? (MAXOPS == kMaxOpsLarge ? ELG_K_CHAIN_LONG : (COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN)) : -1;
+        // a compacting run moves all seven arrays (56 B in, 56 B out); the others only the coordinates they read / write
+        c.bytes_pp = COMPACT ? 112u : 8u * (unsigned)(__builtin_popcount(rmask) + __builtin_popcount(wmask));
+        c.flops_pp = MOM ? 60u : 0u;                                  // algorithmic flops per particle
+        for (const HostOp& op : pending) {
+            switch (op.type) {
+                case OP_MATRIX: c.flops_pp += 72u; break;
+                case OP_MATRIX_UNC: c.flops_pp += 40u; break;
+                case OP_MATRIX2: c.flops_pp += 72u + 21u + 252u; break;
+                case OP_MATRIX3: c.flops_pp += 72u + 21u + 252u + 56u + 672u; break;
+                case OP_DRIFT: c.flops_pp += 11u; break;
+                case OP_RFKICK: c.flops_pp += 6u; break;
+                case OP_KICK: c.flops_pp += 10u; break;
+                case OP_TKICK: c.flops_pp += 14u; break;
+                default: break;
+            }
+        }
         for (size_t k = 0; k < pending.size(); k++) {
             a.type[k] = pending[k].type;
             std::memcpy(a.coef[k], pending[k].coef, sizeof(double) * 42);
@@ -734,7 +787,7 @@ struct Tracker {
         if (!b) return;
         MomArgs m;
         for (int k = 0; k < 6; k++) m.src[k] = b->coord(b->cur_buf, k);
-        m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial;
+        m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial; m.prof_kind = b->prof_on ? ELG_K_MOMENTS : -1;
         m.record = b->records + 43 * b->rec_count;
         {
             ProfScope ps(b, ELG_K_MOMENTS);
@@ -808,11 +861,12 @@ struct Tracker {
                 DipoleArgs d;
                 d.s = b->coord(b->cur_buf, 4); d.x = b->coord(b->cur_buf, 0); d.y = b->coord(b->cur_buf, 2);
                 d.st = b->st; d.cur = b->cur_slot; d.inv_bc = b->inv_bc; d.nb = e.nb; d.counts = b->counts; d.dacc = b->dacc;
+                d.prof_kind = b->prof_on ? ELG_K_HIST : -1;
                 ProfScope ps(b, ELG_K_HIST);
                 dipole_hist_kernel<<<b->grid_dipole, kBlock, kDipoleSmemBins * 36, b->stream>>>(d);
             } else {
                 HistArgs h;
-                h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1;
+                h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1; h.prof_kind = b->prof_on ? ELG_K_HIST : -1;
                 h.inv_bc = b->inv_bc; h.t_lo = 0; h.inv_dt = 0; h.nb = e.nb; h.counts = b->counts;
                 h.aggregate = b->hist_aggregate < 0 ? 0 : b->hist_aggregate;
                 // one private copy per warp needs 8 nb bins: small histograms take less shared memory and get more
@@ -1157,7 +1211,7 @@ extern "C" int32_t elg_moments(elg_bunch* b, int64_t* n_alive, double h_centroid
     if (!b) return fail(ELG_EINVAL, "elg_moments: NULL bunch");
     MomArgs m;
     for (int k = 0; k < 6; k++) m.src[k] = b->coord(b->cur_buf, k);
-    m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial;
+    m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial; m.prof_kind = -1;
     m.record = b->records + 43 * kRecCap;
     moments_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(m);
     g_launches++;

@@ -61,7 +61,18 @@ struct DevState {
     unsigned long long fid_acc[2];   // exact fixed-point sum of s - s_design (G36)
     double s_ref;              // fiducial path length of the bunch, read by RFKICK ops with the fiducial flag
     long long zero_bits;       // always 0: a value the compiler cannot see through (matrix_map_uniform)
+    unsigned long long work[16];     // per kernel kind (ELG_K_*): algorithmic bytes, flops of the launches since the last
+                                     // elg_profile_read (only counted while profiling is on)
 };
+
+// work accounting for elg_profile_read: one thread adds what this launch moves and computes, from the live count
+// the launch itself sees (the host never knows it).  kind < 0: profiling off.
+__device__ __forceinline__ void account_work(DevState* st, int kind, long long n, unsigned int bytes_pp, unsigned int flops_pp) {
+    if (kind >= 0 && blockIdx.x == 0 && threadIdx.x == 0 && n > 0) {
+        atomicAdd(&st->work[2 * kind], (unsigned long long)n * bytes_pp);
+        atomicAdd(&st->work[2 * kind + 1], (unsigned long long)n * flops_pp);
+    }
+}
 
 struct ChainCommon {
     double* src[6];
@@ -94,6 +105,8 @@ struct ChainCommon {
     long long range_hi;        // (pipelined upload: one range per chunk, elg_upload_and_track)
     double* mom_partial;       // moment epilogue (MOM instantiations): per-block partials [kNMom][gridDim.x]
     double* mom_record;        //   and the 43-double record to fill (n, centroid, Sigma), a13 / G26
+    int prof_kind;             // work accounting (account_work): ELG_K_* or -1
+    unsigned int bytes_pp, flops_pp;     // algorithmic bytes / flops of this run per live particle
 };
 
 template <int MAXOPS>
@@ -568,6 +581,7 @@ __global__ void __launch_bounds__(kBlock, ((P >= 4 || MOM) ? 2 : 3)) chain_kerne
     const long long n_tiles = (n > c.range_lo) ? (n - c.range_lo + kTileP - 1) / kTileP : 0;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double mn = INFINITY, mx = -INFINITY;
+    account_work(c.st, c.prof_kind, n - c.range_lo, c.bytes_pp, c.flops_pp);
     double K[MOM ? 6 : 1], acc[MOM ? kNMom : 1];
     if constexpr (MOM) {
         moment_shift<MAXOPS, EXT>(a, n, K);
@@ -756,6 +770,7 @@ __global__ void __maxnreg__(LongCfg<LEVEL>::REGS) chain_long_kernel(const __grid
     const long long n_tiles = (n > c.range_lo) ? (n - c.range_lo + kTileL - 1) / kTileL : 0;
     __shared__ double s_mn[NT], s_mx[NT];                        // running min / max of s per thread: not in registers,
     if (c.want_minmax) { s_mn[threadIdx.x] = INFINITY; s_mx[threadIdx.x] = -INFINITY; }     // the map loop needs them all
+    account_work(c.st, c.prof_kind, n - c.range_lo, c.bytes_pp, c.flops_pp);
 
     auto prefetch = [&](long long tile) {
         const long long t0 = c.range_lo + tile * kTileL + (long long)threadIdx.x * 2;
@@ -901,6 +916,7 @@ __global__ void __launch_bounds__(kC2Threads, (MOM ? 1 : ELG_C2_BLOCKS)) compact
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const unsigned int lt_mask = (1u << lane) - 1u;
     double mn = INFINITY, mx = -INFINITY;
+    account_work(c.st, c.prof_kind, n, c.bytes_pp, c.flops_pp);
 
     extern __shared__ __align__(16) double c2_ring[];           // [S][7][TILE]; row 6 holds the IDs (bit patterns)
     __shared__ int s_wtot[2][PP][NW];                            // per iteration parity, sub-tile, warp: survivors
@@ -1172,7 +1188,8 @@ __global__ void __launch_bounds__(kBlock) window_kernel(const WindowArgs a) {
 // ---------------------------------------------------------------------------------------------------
 struct HistArgs {
     const double* s;
-    const DevState* st;
+    DevState* st;
+    int prof_kind;
     int cur;
     long long n_fixed;     // >= 0: use this n and the explicit window below (test hook); < 0: device state
     double inv_bc, t_lo, inv_dt;
@@ -1188,6 +1205,7 @@ __global__ void __launch_bounds__(kBlock) hist_kernel(const HistArgs a) {
     double t_lo, inv_dt;
     if (a.n_fixed >= 0) { n = a.n_fixed; blo = 0; bhi = a.nb - 1; t_lo = a.t_lo; inv_dt = a.inv_dt; }
     else { n = a.st->n_alive[a.cur]; blo = a.st->bin_lo; bhi = a.st->bin_hi; t_lo = a.st->win[0]; inv_dt = a.st->win[2]; }
+    if (a.st) account_work(a.st, a.prof_kind, n, 8u, 4u);
     long long span = bhi - blo + 1;
     if (span < 1) span = 1;
     const int S = (int)(span < a.smem_bins ? span : a.smem_bins);
@@ -1256,7 +1274,8 @@ struct DipoleArgs {
     const double* s;
     const double* x;
     const double* y;
-    const DevState* st;
+    DevState* st;
+    int prof_kind;
     int cur;
     double inv_bc;
     int nb;
@@ -1289,6 +1308,7 @@ __global__ void __launch_bounds__(kBlock) dipole_hist_kernel(const DipoleArgs a)
     const long long n = a.st->n_alive[a.cur];
     const long long blo = a.st->bin_lo, bhi = a.st->bin_hi;
     const double t_lo = a.st->win[0], inv_dt = a.st->win[2];
+    account_work(a.st, a.prof_kind, n, 24u, 12u);
     long long span = bhi - blo + 1;
     if (span < 1) span = 1;
     const int S = (int)(span < kDipoleSmemBins ? span : kDipoleSmemBins);
@@ -1557,12 +1577,14 @@ struct MomArgs {
     const double* src[6];
     DevState* st;
     int cur;
+    int prof_kind;
     double* partial;       // [kNMom][gridDim.x]
     double* record;        // 43 doubles: n, C[6], Sigma[36]
 };
 
 __global__ void __launch_bounds__(kBlock) moments_kernel(const MomArgs a) {
     const long long n = a.st->n_alive[a.cur];
+    account_work(a.st, a.prof_kind, n, 48u, 60u);
     double K[6];
 #pragma unroll
     for (int c = 0; c < 6; c++) K[c] = (n > 0) ? __ldg(a.src[c]) : 0.0;
@@ -1590,6 +1612,30 @@ __global__ void __launch_bounds__(kBlock) moments_kernel(const MomArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// fp64_peak_kernel: the denominator of the fp64 roofline, measured instead of derived: eight independent DFMA chains
+// per thread, nothing else in the loop.  Operand form DFMA R, R, R, c[..] (two vector registers + one constant-bank
+// operand): the fastest form on sm_100 (63.5 DFMA/clk/SM; three vector registers or two uniform operands give 58.5)
+// and the form of the long-run kernel's own DFMAs (two registers + one uniform).  elg_dbg_fp64_peak times it.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kPeakIlp = 8, kPeakUnroll = 16;
+__global__ void __launch_bounds__(kBlock) fp64_peak_kernel(double* out, long long iters, double b, double c) {
+    double a[kPeakIlp];
+#pragma unroll
+    for (int i = 0; i < kPeakIlp; i++) a[i] = 1e-3 * (threadIdx.x + i);
+    const double bb = b + 1e-9 * threadIdx.x;                                    // a per-thread value: vector operand
+    for (long long it = 0; it < iters; it++) {
+#pragma unroll
+        for (int r = 0; r < kPeakUnroll; r++)
+#pragma unroll
+            for (int i = 0; i < kPeakIlp; i++) a[i] = fma(a[i], bb, c);         // c: kernel parameter = constant-bank operand
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < kPeakIlp; i++) s += a[i];
+    if (s == 123.456) out[threadIdx.x] = s;                                     // never true: keeps the chains alive
+}
+
+// ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlock) iota_kernel(long long* id, long long n) {
     const long long stride = (long long)gridDim.x * kBlock;
     for (long long i = (long long)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) id[i] = i;
@@ -1603,7 +1649,7 @@ __global__ void init_state_kernel(DevState* st, long long n0) {
     st->bin_lo = 0; st->bin_hi = -1;
     st->tile_counter = 0; st->done_counter = 0; st->mom_done = 0; st->fid_done = 0;
     st->fid_acc[0] = 0ull; st->fid_acc[1] = 0ull; st->s_ref = 0.0;
-    st->zero_bits = 0;
+    st->zero_bits = 0;                                           // (work[] is not touched: it belongs to elg_profile_read)
 }
 
 }  // namespace elg

@@ -35,7 +35,7 @@ EXPORTS = (
     "elg_moments", "elg_lost", "elg_n_alive", "elg_bunch_read", "elg_bunch_device_array",
     "elg_profile_enable", "elg_profile_read",
     "elg_dbg_histogram", "elg_dbg_dipole_histogram", "elg_dbg_kick", "elg_dbg_tkick", "elg_dbg_compact",
-    "elg_dbg_wake_samples", "elg_dbg_convolve",
+    "elg_dbg_wake_samples", "elg_dbg_convolve", "elg_dbg_fp64_peak",
 )
 KERNEL_KINDS = ("chain", "chain_compact", "window", "hist", "wake_samples", "conv", "moments", "chain_long")
 
@@ -115,7 +115,8 @@ def lib():
     L.elg_bunch_read.argtypes = [vp, v6, _i64p, C.c_int64]; L.elg_bunch_read.restype = C.c_int32
     L.elg_bunch_device_array.argtypes = [vp, C.c_int32, C.POINTER(vp)]; L.elg_bunch_device_array.restype = C.c_int32
     L.elg_profile_enable.argtypes = [vp, C.c_int32]; L.elg_profile_enable.restype = C.c_int32
-    L.elg_profile_read.argtypes = [vp, _i64p, _dp]; L.elg_profile_read.restype = C.c_int32
+    L.elg_profile_read.argtypes = [vp, _i64p, _dp, _dp, _dp]; L.elg_profile_read.restype = C.c_int32
+    L.elg_dbg_fp64_peak.argtypes = [vp, C.c_int64, _dp, _dp, vp]; L.elg_dbg_fp64_peak.restype = C.c_int32
     L.elg_dbg_histogram.argtypes = [vp, C.c_double, C.c_double, C.c_int32, vp]; L.elg_dbg_histogram.restype = C.c_int32
     L.elg_dbg_dipole_histogram.argtypes = [vp, C.c_double, C.c_double, C.c_int32, vp, vp]
     L.elg_dbg_dipole_histogram.restype = C.c_int32
@@ -411,11 +412,15 @@ class Bunch:
         """elg_profile_enable: bracket every kernel launch of this bunch with CUDA events."""
         _ck(lib().elg_profile_enable(self._h, 1 if on else 0))
 
-    def profile_read(self) -> dict:
-        """elg_profile_read: {kernel kind: (launches, summed device ms)} since the last read."""
+    def profile_read(self, work: bool = False) -> dict:
+        """elg_profile_read: {kernel kind: (launches, summed device ms)} since the last read; with work=True
+        {kind: (launches, ms, algorithmic bytes, algorithmic flops)}."""
         n = len(KERNEL_KINDS)
         cnt = np.zeros(n, dtype=np.int64); ms = np.zeros(n, dtype=np.float64)
-        _ck(lib().elg_profile_read(self._h, _p(cnt, _i64p), _p(ms)))
+        by = np.zeros(n, dtype=np.float64); fl = np.zeros(n, dtype=np.float64)
+        _ck(lib().elg_profile_read(self._h, _p(cnt, _i64p), _p(ms), _p(by), _p(fl)))
+        if work:
+            return {k: (int(cnt[i]), float(ms[i]), float(by[i]), float(fl[i])) for i, k in enumerate(KERNEL_KINDS)}
         return {k: (int(cnt[i]), float(ms[i])) for i, k in enumerate(KERNEL_KINDS)}
 
     def device_array(self, c: int):
@@ -518,3 +523,12 @@ def dbg_convolve(counts, W, q: float) -> np.ndarray:
     st = torch.cuda.current_stream().cuda_stream
     _ck(lib().elg_dbg_convolve(d_c.data_ptr(), d_W.data_ptr(), d_c.numel(), q, d_V.data_ptr(), st))
     return d_V.cpu().numpy()
+
+
+def dbg_fp64_peak(iters: int = 20000):
+    """elg_dbg_fp64_peak: (TFLOP/s, ms) of the DFMA-only kernel -- the measured fp64 roofline denominator."""
+    torch = _torch()
+    scratch = torch.empty(512, dtype=torch.float64, device="cuda")
+    tf = C.c_double(); ms = C.c_double()
+    _ck(lib().elg_dbg_fp64_peak(scratch.data_ptr(), iters, C.byref(tf), C.byref(ms), torch.cuda.current_stream().cuda_stream))
+    return tf.value, ms.value

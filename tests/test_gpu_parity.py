@@ -738,3 +738,47 @@ def test_track_in_two_calls_equals_one(elg, elgo):
     # rewind + re-upload gives the same answer again (workspace reuse)
     a.upload(v0); a.track(bl, 6)
     assert np.array_equal(a.read()[0], b.read()[0])
+
+
+def test_profile_reports_algorithmic_work(elg):
+    """elg_profile_read's bytes / flops (what bench.py's roofline uses): coordinates read + written x live particles of
+    every launch, counted on the device.  DRIFT + MATRIX reads 6 and writes 6 coordinates (96 B); a compacting run
+    moves all seven arrays (112 B); 10 matrices are 720 flop per particle; lossy lines use the live count of each launch."""
+    n = 300_001
+    w = make_workload("p1-chain", n=n)
+    v0 = w.particles()
+    bl = elg.Beamline(w.elements); b = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=bl)
+    b.profile(True); b.profile_read()
+    b.track(bl, 1)
+    p = b.profile_read(work=True)
+    assert p["chain"][0] == 1 and p["chain"][2] == 96.0 * n and p["chain"][3] == (11 + 72) * n
+    b.upload(v0)                                           # rewinds: the counters survive a rewind
+    b.track(bl, 1); b.upload(v0); b.track(bl, 1)
+    p = b.profile_read(work=True)
+    assert p["chain"][0] == 2 and p["chain"][2] == 2 * 96.0 * n
+    w2 = make_workload("cfg4", n=n)
+    bl2 = elg.Beamline(w2.elements); b2 = elg.Bunch(w2.particles(), w2.p0c_eV, w2.charge_C, beamline=bl2)
+    b2.profile(True); b2.profile_read()
+    b2.track(bl2, 1)
+    p2 = b2.profile_read(work=True)
+    _, _, elem, _ = b2.lost()
+    n_in = n - np.array([(elem < 3 * i).sum() for i in range(20)])          # live count entering collimator i
+    assert p2["chain_compact"][0] == 20 and p2["chain_compact"][2] == 112.0 * n_in.sum()
+    n_hist = n - np.array([(elem <= 3 * i).sum() for i in range(20)])
+    assert p2["hist"][0] == 20 and p2["hist"][2] == 8.0 * n_hist.sum()
+    w3 = make_workload("p3-matrices", n=n, n_matrices=10)
+    bl3 = elg.Beamline(w3.elements, ring=True); b3 = elg.Bunch(w3.particles(), w3.p0c_eV, w3.charge_C, beamline=bl3)
+    b3.profile(True); b3.profile_read()
+    b3.track(bl3, 2)                                       # the planner fuses the two turns into one 20-matrix run
+    p3 = b3.profile_read(work=True)
+    assert p3["chain_long"][0] == 1 and p3["chain_long"][3] == 2 * 720.0 * n and p3["chain_long"][2] == 96.0 * n
+    b3.profile(False)
+    b3.track(bl3, 1)
+    assert b3.profile_read(work=True)["chain_long"] == (0, 0.0, 0.0, 0.0)   # nothing is counted while profiling is off
+
+
+def test_fp64_peak_hook(elg):
+    """elg_dbg_fp64_peak (the measured denominator of the fp64 roofline): a DFMA-only kernel must land near the nominal
+    148 SMs x 64 DFMA/clk x 2 x clock."""
+    tf, ms = elg.dbg_fp64_peak(5000)
+    assert ms > 0 and 25.0 < tf < 45.0
