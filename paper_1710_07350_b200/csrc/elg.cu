@@ -102,7 +102,8 @@ struct elg_bunch {
     std::map<int, int> hist_grids;                      // hist_kernel grid per shared-memory size
     std::map<const void*, int> grids;                   // persistent grid size per chain kernel instantiation
     int force_p = 0;                                    // ELG_CHAIN_P = 2 | 4 overrides the planner's choice
-    int grid_mom = 0, grid_dipole = 0;
+    int grid_mom = 0;
+    std::map<int, int> dipole_grids;                    // dipole_hist_kernel grid per shared-memory size
     int hist_aggregate = 0;
     // pipelined upload (elg_upload_and_track): the library's own copy stream and one event per chunk
     cudaStream_t copy_stream = nullptr;
@@ -231,7 +232,8 @@ int32_t long_setup_once() {
 int32_t hist_setup_once() {
     static bool done = false;
     if (!done) {
-        ELG_CK(cudaFuncSetAttribute(hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kHistSmemBins * 4));
+        ELG_CK(cudaFuncSetAttribute(hist_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kHistSmemBins * 4));
+        ELG_CK(cudaFuncSetAttribute(hist_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kHistSmemBins * 4));
         ELG_CK(cudaFuncSetAttribute(dipole_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDipoleSmemBins * 36));
         done = true;
     }
@@ -407,7 +409,6 @@ extern "C" int32_t elg_bunch_create(elg_bunch** out, int64_t n0, void* d_soa, vo
     if (rc == ELG_OK) rc = long_setup_once();
     if (rc == ELG_OK) rc = hist_setup_once();
     if (rc == ELG_OK) rc = grid_for(moments_kernel, sms, 0, kBlock, &b->grid_mom);
-    if (rc == ELG_OK) rc = grid_for(dipole_hist_kernel, sms, kDipoleSmemBins * 36, kBlock, &b->grid_dipole);
     if (rc != ELG_OK) { delete b; return rc; }
     const char* agg = std::getenv("ELG_HIST_AGGREGATE");
     b->hist_aggregate = agg ? std::atoi(agg) : -1;                 // -1: automatic
@@ -536,10 +537,21 @@ struct Tracker {
         auto it = b->hist_grids.find(smem_bins);
         if (it != b->hist_grids.end()) return it->second;
         int occ = 0;
-        check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_kernel, kBlock, (size_t)smem_bins * 4), "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+        check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, hist_kernel<false>, kBlock, (size_t)smem_bins * 4), "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
         if (occ < 1) occ = 1;
         const int g = occ * b->sms;
         b->hist_grids[smem_bins] = g;
+        return g;
+    }
+
+    int dipole_grid(int smem_bins) {
+        auto it = b->dipole_grids.find(smem_bins);
+        if (it != b->dipole_grids.end()) return it->second;
+        int occ = 0;
+        check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dipole_hist_kernel, kBlock, (size_t)smem_bins * 36), "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+        if (occ < 1) occ = 1;
+        const int g = occ * b->sms;
+        b->dipole_grids[smem_bins] = g;
         return g;
     }
 
@@ -862,8 +874,10 @@ struct Tracker {
                 d.s = b->coord(b->cur_buf, 4); d.x = b->coord(b->cur_buf, 0); d.y = b->coord(b->cur_buf, 2);
                 d.st = b->st; d.cur = b->cur_slot; d.inv_bc = b->inv_bc; d.nb = e.nb; d.counts = b->counts; d.dacc = b->dacc;
                 d.prof_kind = b->prof_on ? ELG_K_HIST : -1;
+                // shared memory for the bins this element can occupy: small histograms get more resident blocks
+                d.smem_bins = e.nb < kDipoleSmemBins ? (e.nb + 31) / 32 * 32 : kDipoleSmemBins;
                 ProfScope ps(b, ELG_K_HIST);
-                dipole_hist_kernel<<<b->grid_dipole, kBlock, kDipoleSmemBins * 36, b->stream>>>(d);
+                dipole_hist_kernel<<<dipole_grid(d.smem_bins), kBlock, (size_t)d.smem_bins * 36, b->stream>>>(d);
             } else {
                 HistArgs h;
                 h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1; h.prof_kind = b->prof_on ? ELG_K_HIST : -1;
@@ -873,7 +887,8 @@ struct Tracker {
                 // resident blocks (more loads in flight)
                 h.smem_bins = (8LL * e.nb < kHistSmemBins) ? 8 * e.nb : kHistSmemBins;
                 ProfScope ps(b, ELG_K_HIST);
-                hist_kernel<<<hist_grid(h.smem_bins), kBlock, h.smem_bins * 4, b->stream>>>(h);
+                if (h.aggregate) hist_kernel<true><<<hist_grid(h.smem_bins), kBlock, h.smem_bins * 4, b->stream>>>(h);
+                else hist_kernel<false><<<hist_grid(h.smem_bins), kBlock, h.smem_bins * 4, b->stream>>>(h);
 
             }
             check(cudaGetLastError(), "hist_kernel launch");

@@ -31,6 +31,9 @@ constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
 #define ELG_L1_PL 6
 #define ELG_L1_REGS 200
 #endif
+#ifndef ELG_BIN_MAGIC
+#define ELG_BIN_MAGIC 1          // bin_of: floor by adding 1.5 x 2^52 instead of FRND / F2I (0: conversions)
+#endif
 #ifndef ELG_L2_NT
 #define ELG_L2_NT 384
 #define ELG_L2_PL 4
@@ -184,14 +187,23 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 template <int ID, int N>
 __device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(N) : "memory"); }
 
-// bin of a time coordinate (G10): floor((s*inv_bc - t_lo)*inv_dt) in [0, nb) else -1
+// bin of a time coordinate (G10): floor((s*inv_bc - t_lo)*inv_dt) in [0, nb) else -1.  For 0 <= u < nb <= 2^24 the
+// floor is taken without FRND.F64 / F2I.F64 (quarter-rate conversions): u + 1.5 x 2^52 lies in [2^52, 2^53), where
+// doubles are the integers, so the addition rounds u to the nearest integer r, the low word of the sum's bit pattern IS
+// r, and floor(u) = r - (r > u).  floor(u) >= 0 <=> u >= 0 and floor(u) < nb <=> u < nb, so the range test is the
+// definition's; NaN fails it.
 __device__ __forceinline__ int bin_of(double s, double inv_bc, double t_lo, double inv_dt, int nb, double* u_out) {
     const double t = s * inv_bc;
     const double u = (t - t_lo) * inv_dt;
-    const double fl = floor(u);
     *u_out = u;
-    if (!(fl >= 0.0) || !(fl < (double)nb)) return -1;
-    return (int)fl;
+    if (!(u >= 0.0) || !(u < (double)nb)) return -1;
+#if !ELG_BIN_MAGIC
+    return (int)floor(u);
+#endif
+    constexpr double kMagic = 6755399441055744.0;                // 1.5 x 2^52
+    const double m = u + kMagic;
+    const double r = m - kMagic;
+    return __double2loint(m) - ((r > u) ? 1 : 0);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -1194,12 +1206,13 @@ struct HistArgs {
     long long n_fixed;     // >= 0: use this n and the explicit window below (test hook); < 0: device state
     double inv_bc, t_lo, inv_dt;
     int nb;
-    int aggregate;         // 1: warp-aggregate equal bins with match.any before the shared atomic
+    int aggregate;         // 1: warp-aggregate equal bins with match.any before the shared atomic (hist_kernel<true>)
     int smem_bins;         // bins of dynamic shared memory this launch was given (<= kHistSmemBins)
     unsigned int* counts;
 };
 
-__global__ void __launch_bounds__(kBlock) hist_kernel(const HistArgs a) {
+template <bool AGG>
+__global__ void __launch_bounds__(kBlock, 6) hist_kernel(const HistArgs a) {
     extern __shared__ unsigned int sh[];
     long long n, blo, bhi;
     double t_lo, inv_dt;
@@ -1211,44 +1224,53 @@ __global__ void __launch_bounds__(kBlock) hist_kernel(const HistArgs a) {
     const int S = (int)(span < a.smem_bins ? span : a.smem_bins);
     int R = a.smem_bins / S;
     if (R > kWarps) R = kWarps;
-    const int wid = threadIdx.x >> 5;
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned int* mine = sh + (wid % R) * S;
     for (int i = threadIdx.x; i < R * S; i += kBlock) sh[i] = 0u;
     __syncthreads();
+    const int lo32 = (int)blo;                                   // 0 <= bin_lo <= nb - 1 < 2^24
 
     constexpr int kPer = 8;                                      // 4 x 128-bit loads in flight per thread
     const long long stride = (long long)gridDim.x * kBlock * kPer;
     // warp-uniform trip count (the aggregated path uses full-mask warp votes)
     for (long long w0 = ((long long)blockIdx.x * kBlock + (threadIdx.x & ~31)) * kPer; w0 < n; w0 += stride) {
         // lane l owns particles w0 + 2l + 64k + {0, 1}, k < 4: every load is a 512-byte warp access
-        const long long i0 = w0 + (long long)(threadIdx.x & 31) * 2;
+        const long long i0 = w0 + (long long)lane * 2;
         double sv[kPer];
         bool have[kPer];
+        if (w0 + 32 * kPer <= n) {                               // the whole warp chunk is live: no per-load tests
 #pragma unroll
-        for (int k = 0; k < kPer / 2; k++) {
-            const long long i = i0 + 64 * k;
-            have[2 * k] = i < n; have[2 * k + 1] = i + 1 < n;
-            sv[2 * k] = 0.0; sv[2 * k + 1] = 0.0;
-            if (have[2 * k + 1]) { const double2 t = ld_stream2(a.s + i); sv[2 * k] = t.x; sv[2 * k + 1] = t.y; }
-            else if (have[2 * k]) sv[2 * k] = ld_stream1(a.s + i);
+            for (int k = 0; k < kPer / 2; k++) {
+                const double2 t = ld_stream2(a.s + i0 + 64 * k);
+                sv[2 * k] = t.x; sv[2 * k + 1] = t.y; have[2 * k] = true; have[2 * k + 1] = true;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < kPer / 2; k++) {
+                const long long i = i0 + 64 * k;
+                have[2 * k] = i < n; have[2 * k + 1] = i + 1 < n;
+                sv[2 * k] = 0.0; sv[2 * k + 1] = 0.0;
+                if (have[2 * k + 1]) { const double2 t = ld_stream2(a.s + i); sv[2 * k] = t.x; sv[2 * k + 1] = t.y; }
+                else if (have[2 * k]) sv[2 * k] = ld_stream1(a.s + i);
+            }
         }
 #pragma unroll
         for (int p = 0; p < kPer; p++) {
             double u;
             const int b = have[p] ? bin_of(sv[p], a.inv_bc, t_lo, inv_dt, a.nb, &u) : -1;
-            if (a.aggregate) {
+            const unsigned int rel = (unsigned int)(b - lo32);   // b < bin_lo cannot happen (monotone bin function); if it
+                                                                 // did, rel wraps past S and the global path takes it
+            if constexpr (AGG) {
                 const unsigned int act = __ballot_sync(0xffffffffu, b >= 0);   // loop trip count is warp-uniform
                 if (b >= 0) {
                     const unsigned int peers = __match_any_sync(act, b);
-                    if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) {
-                        const long long rel = (long long)b - blo;
-                        if (rel < S) atomicAdd(mine + rel, (unsigned int)__popc(peers));
+                    if ((int)(__ffs(peers) - 1) == lane) {
+                        if (rel < (unsigned int)S) atomicAdd(mine + rel, (unsigned int)__popc(peers));
                         else atomicAdd(a.counts + b, (unsigned int)__popc(peers));
                     }
                 }
             } else if (b >= 0) {
-                const long long rel = (long long)b - blo;
-                if (rel < S) atomicAdd(mine + rel, 1u);
+                if (rel < (unsigned int)S) atomicAdd(mine + rel, 1u);
                 else atomicAdd(a.counts + b, 1u);
             }
         }
@@ -1264,11 +1286,28 @@ __global__ void __launch_bounds__(kBlock) hist_kernel(const HistArgs a) {
 // ---------------------------------------------------------------------------------------------------
 // dipole_hist_kernel (TRWAKE, G32-G33): bin counts and per-bin dipole sums of x and y.  A sum of doubles
 // accumulated with atomics would depend on the order of arrival; here every coordinate is split exactly into
-// two integers (hi = rint(x 2^32), lo = rint((x - hi 2^-32) 2^64)) which are summed with 64-bit INTEGER
-// atomics: exact, order-independent, run-to-run reproducible, and bit-identical to the sequential CPU sum.
-// Shared-memory privatisation of the occupied bin range as in hist_kernel (36 bytes per bin).
+// two integers (hi = rint(x 2^36), lo = rint((x - hi 2^-36) 2^64)) which are summed with 64-bit
+// INTEGER arithmetic: exact to 2^-64 m per particle, order-independent, run-to-run reproducible.
+// Shared-memory privatisation of the occupied bin range as in hist_kernel, 36 bytes per bin, laid out as NINE
+// PLANES of 32-bit words (count | low and high words of the four 64-bit sums): the word of bin b in a plane sits in
+// bank b mod 32, so the 32 lanes of an atomic spread over all banks (round 1 kept the four 64-bit sums of a bin side by
+// side: every atomic of a warp fell into 4 of the 32 banks, 85 % of the shared-memory wavefront peak, 0.74 ms per
+// 1e8 particles; profiles/r02_dipole.md).  The split point 2^36 (round 1: 2^32) leaves both integers of a
+// millimetre-sized offset below 2^28, so the low word of a sum rarely wraps and an add is ONE native 32-bit atomic
+// (the carry into the high word follows in 1-3 % of the adds): 5.1 shared atomics per particle instead of 9.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kDipoleSmemBins = 1792;                   // 1792 x 36 B = 63 KB
+constexpr int kDipoleSmemBins = 1792;                   // 1792 x 36 B = 63 KB: the most bins a block privatises
+#ifndef ELG_DIP_PER
+#define ELG_DIP_PER 4
+#endif
+#ifndef ELG_DIP_BLOCKS
+#define ELG_DIP_BLOCKS 4
+#endif
+constexpr int kDipolePer = ELG_DIP_PER;                 // particles per thread and iteration: 6 x 128-bit loads in flight
+constexpr int kFixDipole = 36;                          // split point of the dipole sums: |sum of x over a bin| < 2^27 m
+constexpr int kFixFiducial = 32;                        // split point of the fiducial sum (no shared atomics there: keep the
+                                                        // larger range, |sum of s - s_design| < 2^31 m)
+constexpr double kFixLo = 18446744073709551616.0;       // 2^64
 
 struct DipoleArgs {
     const double* s;
@@ -1279,69 +1318,90 @@ struct DipoleArgs {
     int cur;
     double inv_bc;
     int nb;
+    int smem_bins;                 // bins of dynamic shared memory this launch was given (<= kDipoleSmemBins)
     unsigned int* counts;
     unsigned long long* dacc;      // [nb][4]: x hi, x lo, y hi, y lo
 };
 
+template <int BITS>
 __device__ __forceinline__ bool fixed_split(double x, long long* hi, long long* lo) {
+    constexpr double kHi = (double)(1ull << BITS);
     if (!(fabs(x) < 1048576.0)) return false;
-    const double h = rint(x * 4294967296.0);
-    const double r = x - h * (1.0 / 4294967296.0);               // exact
+    const double h = rint(x * kHi);
+    const double r = x - h * (1.0 / kHi);                        // exact
     *hi = (long long)h;
-    *lo = (long long)rint(r * 18446744073709551616.0);
-    return true;
+    *lo = (long long)rint(r * kFixLo);                           // (rounding by adding 1.5 x 2^52 as in bin_of was
+    return true;                                                 //  measured here too: slower, the fp64 pipe is the busier one)
+}
+template <int BITS>
+__device__ __forceinline__ double fixed_join(long long H, long long L) {
+    constexpr double kHi = (double)(1ull << BITS);
+    return fma((double)H, 1.0 / kHi, (double)L * (1.0 / kFixLo));
 }
 
-// 64-bit integer add in shared memory from two native 32-bit atomics (a 64-bit shared atomicAdd compiles to a
+// 64-bit integer adds in shared memory from native 32-bit atomics (a 64-bit shared atomicAdd compiles to a
 // compare-and-swap spin loop): add the low word, carry into the high word when the low word wrapped.  Addition
-// modulo 2^64 commutes, so the result does not depend on the interleaving.
-__device__ __forceinline__ void smem_add64(unsigned long long* p, unsigned long long v) {
-    unsigned int* w = reinterpret_cast<unsigned int*>(p);
-    const unsigned int lo = (unsigned int)v, hi = (unsigned int)(v >> 32);
-    const unsigned int old = atomicAdd(w, lo);
-    const unsigned int carry = (old + lo < old) ? 1u : 0u;
-    if (hi + carry) atomicAdd(w + 1, hi + carry);
+// modulo 2^64 commutes, so the result does not depend on the interleaving.  A small negative value has high word
+// 0xffffffff and nearly always produces a carry: hi + carry = 0, one atomic as well.  The four low-word atomics of a
+// particle are issued back to back (independent), the rare high-word ones follow.
+__device__ __forceinline__ void smem_add64x4(unsigned int* planes, int S, int rel, const unsigned long long (&v)[4]) {
+    unsigned int old[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) old[k] = atomicAdd(planes + (1 + 2 * k) * S + rel, (unsigned int)v[k]);
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const unsigned int lo = (unsigned int)v[k], hi = (unsigned int)(v[k] >> 32);
+        const unsigned int up = hi + ((old[k] + lo < old[k]) ? 1u : 0u);
+        if (up) atomicAdd(planes + (2 + 2 * k) * S + rel, up);
+    }
 }
 
-__global__ void __launch_bounds__(kBlock) dipole_hist_kernel(const DipoleArgs a) {
-    extern __shared__ __align__(8) unsigned char sh_raw[];
+__global__ void __launch_bounds__(kBlock, ELG_DIP_BLOCKS) dipole_hist_kernel(const DipoleArgs a) {
+    extern __shared__ __align__(16) unsigned int sh_dip[];       // [9][S]
     const long long n = a.st->n_alive[a.cur];
     const long long blo = a.st->bin_lo, bhi = a.st->bin_hi;
     const double t_lo = a.st->win[0], inv_dt = a.st->win[2];
     account_work(a.st, a.prof_kind, n, 24u, 12u);
     long long span = bhi - blo + 1;
     if (span < 1) span = 1;
-    const int S = (int)(span < kDipoleSmemBins ? span : kDipoleSmemBins);
-    unsigned long long* sd = reinterpret_cast<unsigned long long*>(sh_raw);          // [S][4]
-    unsigned int* sc = reinterpret_cast<unsigned int*>(sh_raw + (size_t)S * 32);      // [S]
-    for (int i = threadIdx.x; i < S * 4; i += kBlock) sd[i] = 0ull;
-    for (int i = threadIdx.x; i < S; i += kBlock) sc[i] = 0u;
+    const int S = (int)(span < a.smem_bins ? span : a.smem_bins);
+    for (int i = threadIdx.x; i < 9 * S; i += kBlock) sh_dip[i] = 0u;
     __syncthreads();
-    const long long stride = (long long)gridDim.x * kBlock * 2;
-    for (long long i0 = ((long long)blockIdx.x * kBlock + threadIdx.x) * 2; i0 < n; i0 += stride) {
-        double sv[2], xv[2], yv[2];
-        const bool two = i0 + 2 <= n;
-        if (two) {
-            const double2 ts = ld_stream2(a.s + i0), tx = ld_stream2(a.x + i0), ty = ld_stream2(a.y + i0);
-            sv[0] = ts.x; sv[1] = ts.y; xv[0] = tx.x; xv[1] = tx.y; yv[0] = ty.x; yv[1] = ty.y;
-        } else {
-            sv[0] = ld_stream1(a.s + i0); xv[0] = ld_stream1(a.x + i0); yv[0] = ld_stream1(a.y + i0);
-            sv[1] = 0.0; xv[1] = 0.0; yv[1] = 0.0;
+    unsigned int* const sc = sh_dip;
+    constexpr int kPer = kDipolePer;
+    const long long stride = (long long)gridDim.x * kBlock * kPer;
+    // lane l of a warp owns particles w0 + 2l + 64k + {0, 1}, k < kPer / 2: every load is a 512-byte warp access
+    for (long long w0 = ((long long)blockIdx.x * kBlock + (threadIdx.x & ~31)) * kPer; w0 < n; w0 += stride) {
+        const long long i0 = w0 + (long long)(threadIdx.x & 31) * 2;
+        double sv[kPer], xv[kPer], yv[kPer];
+        bool have[kPer];
+#pragma unroll
+        for (int k = 0; k < kPer / 2; k++) {
+            const long long i = i0 + 64 * k;
+            have[2 * k] = i < n; have[2 * k + 1] = i + 1 < n;
+            sv[2 * k] = 0.0; sv[2 * k + 1] = 0.0; xv[2 * k] = 0.0; xv[2 * k + 1] = 0.0; yv[2 * k] = 0.0; yv[2 * k + 1] = 0.0;
+            if (have[2 * k + 1]) {
+                const double2 ts = ld_stream2(a.s + i), tx = ld_stream2(a.x + i), ty = ld_stream2(a.y + i);
+                sv[2 * k] = ts.x; sv[2 * k + 1] = ts.y; xv[2 * k] = tx.x; xv[2 * k + 1] = tx.y; yv[2 * k] = ty.x; yv[2 * k + 1] = ty.y;
+            } else if (have[2 * k]) {
+                sv[2 * k] = ld_stream1(a.s + i); xv[2 * k] = ld_stream1(a.x + i); yv[2 * k] = ld_stream1(a.y + i);
+            }
         }
 #pragma unroll
-        for (int p = 0; p < 2; p++) {
-            if (p == 1 && !two) break;
+        for (int p = 0; p < kPer; p++) {
+            if (!have[p]) continue;
             double u;
             const int b = bin_of(sv[p], a.inv_bc, t_lo, inv_dt, a.nb, &u);
             if (b < 0) continue;
             long long xh, xl, yh, yl;
-            const bool ok = fixed_split(xv[p], &xh, &xl) & fixed_split(yv[p], &yh, &yl);
+            const bool ok = fixed_split<kFixDipole>(xv[p], &xh, &xl) & fixed_split<kFixDipole>(yv[p], &yh, &yl);
             const long long rel = (long long)b - blo;
             if (rel < S) {
-                atomicAdd(sc + rel, 1u);
+                const int r = (int)rel;
+                atomicAdd(sc + r, 1u);
                 if (ok) {
-                    smem_add64(sd + 4 * rel + 0, (unsigned long long)xh); smem_add64(sd + 4 * rel + 1, (unsigned long long)xl);
-                    smem_add64(sd + 4 * rel + 2, (unsigned long long)yh); smem_add64(sd + 4 * rel + 3, (unsigned long long)yl);
+                    const unsigned long long v4[4] = {(unsigned long long)xh, (unsigned long long)xl, (unsigned long long)yh, (unsigned long long)yl};
+                    smem_add64x4(sh_dip, S, r, v4);
                 }
             } else {
                 atomicAdd(a.counts + b, 1u);
@@ -1359,21 +1419,21 @@ __global__ void __launch_bounds__(kBlock) dipole_hist_kernel(const DipoleArgs a)
             atomicAdd(a.counts + blo + i, cnt);
 #pragma unroll
             for (int k = 0; k < 4; k++) {
-                const unsigned long long v = sd[4 * i + k];
+                const unsigned long long v = (unsigned long long)sh_dip[(1 + 2 * k) * S + i] | ((unsigned long long)sh_dip[(2 + 2 * k) * S + i] << 32);
                 if (v) atomicAdd(a.dacc + 4 * (blo + i) + k, v);
             }
         }
     }
 }
 
-// D = fma((double)H, 2^-32, (double)L 2^-64) (G33), Dx then Dy
+// D = fma((double)H, 2^-36, (double)L 2^-64) (G33), Dx then Dy
 __global__ void __launch_bounds__(kBlock) dipole_finalize_kernel(const unsigned long long* dacc, int nb, double* D) {
     const int k = blockIdx.x * kBlock + threadIdx.x;
     if (k >= nb) return;
     const long long xh = (long long)dacc[4 * k + 0], xl = (long long)dacc[4 * k + 1];
     const long long yh = (long long)dacc[4 * k + 2], yl = (long long)dacc[4 * k + 3];
-    D[k] = fma((double)xh, 1.0 / 4294967296.0, (double)xl * (1.0 / 18446744073709551616.0));
-    D[nb + k] = fma((double)yh, 1.0 / 4294967296.0, (double)yl * (1.0 / 18446744073709551616.0));
+    D[k] = fixed_join<kFixDipole>(xh, xl);
+    D[nb + k] = fixed_join<kFixDipole>(yh, yl);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -1391,8 +1451,8 @@ __global__ void __launch_bounds__(kBlock) fiducial_kernel(const double* s, DevSt
         if (two) { const double2 t = ld_stream2(s + i0); a = t.x; b = t.y; }
         else a = ld_stream1(s + i0);
         long long h, l;
-        if (fixed_split(a - s_design, &h, &l)) { H += h; L += l; }
-        if (two && fixed_split(b - s_design, &h, &l)) { H += h; L += l; }
+        if (fixed_split<kFixFiducial>(a - s_design, &h, &l)) { H += h; L += l; }
+        if (two && fixed_split<kFixFiducial>(b - s_design, &h, &l)) { H += h; L += l; }
     }
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
@@ -1413,7 +1473,7 @@ __global__ void __launch_bounds__(kBlock) fiducial_kernel(const double* s, DevSt
         if (s_last) {
             __threadfence();
             const long long Ht = (long long)atomicAdd(&st->fid_acc[0], 0ull), Lt = (long long)atomicAdd(&st->fid_acc[1], 0ull);
-            const double sum = fma((double)Ht, 1.0 / 4294967296.0, (double)Lt * (1.0 / 18446744073709551616.0));
+            const double sum = fixed_join<kFixFiducial>(Ht, Lt);
             st->s_ref = (n > 0) ? s_design + sum / (double)n : s_design;
             st->fid_acc[0] = 0ull; st->fid_acc[1] = 0ull; st->fid_done = 0;
         }

@@ -370,6 +370,14 @@ def test_dipole_histogram_stage(elg, elgo):
     assert np.array_equal(gc4, oc4) and gc4.sum() == 4
     assert np.max(np.abs(gDx4 - oDx4)) <= 2.0 ** -64 and np.max(np.abs(gDy4 - oDy4)) <= 2.0 ** -64     # G33 resolution
     assert abs(gDx4.sum() - 1e-4) <= 2.0 ** -64 and oDx4.sum() == 1e-4 and abs(gDy4.sum() - 1e-5) <= 2.0 ** -64
+    # offsets of kilometres take the other branch of the device's split (|x| >= 2^14 m): one particle per bin, so the
+    # sum is the value itself
+    big = np.array([5e4 + 1e-7, -7e5 - 1.0 / 3, 16384.0, -16383.999999, 1048575.9])
+    s5 = v[4, 0] + (np.arange(5) - 2) * 3 * dt / ibc
+    oc5, oDx5, oDy5, _ = elgo.dipole_histogram(s5, big, -big, ibc, t_lo, inv_dt, nb)
+    gc5, gDx5, gDy5 = elg.dbg_dipole_histogram(s5, big, -big, w.p0c_eV, t_lo, dt, nb)
+    assert np.array_equal(gc5, oc5) and gc5.sum() == 5 and gc5.max() == 1
+    assert np.array_equal(gDx5, oDx5) and np.array_equal(gDy5, oDy5) and np.array_equal(np.sort(gDx5[gc5 > 0]), np.sort(big))
 
 
 # ------------------------------------------------------------------------------------ (iv) wake, convolution
