@@ -157,5 +157,9 @@ def test_long_run_kernels_use_uniform_coefficient_operands():
         spills = [l for l in body if " LDL" in l or " STL" in l]
         assert len(uniform) >= 0.85 * len(dfma), f"level {level}: {len(uniform)} of {len(dfma)} DFMA take a uniform operand"
         assert sum("LDCU" in l and "UR" in l.split("c[0x0]")[-1] for l in body) >= 40, f"level {level}: UR-indexed LDCU missing"
-        assert len(spills) <= 8, f"level {level}: {len(spills)} local-memory instructions (register spills)"
+        # levels 0 and 3 are compiled at the register cap of 384 threads (168): ptxas then parks 4 doubles per matrix
+        # PAIR in local memory (8 of the ~560 instructions of the pair loop) and schedules the DFMA chains 4 % faster
+        # than the spill-free 152-register form (cfg3: 44.1 -> 42.4 ms); more than that would be a regression
+        limit = 32 if level in (0, 3) else 8
+        assert len(spills) <= limit, f"level {level}: {len(spills)} local-memory instructions (register spills)"
     assert seen == 4
