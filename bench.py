@@ -389,8 +389,11 @@ def run_ours(args):
 
     # ---- HBM-bound probes at the same particle count (north_star target kernels)
     probes = []
+    other_configs = None
     if want_probes:
         probes = run_probes(elg, gb, restore, n0, w, hbm_peak, stream, dev, args)
+        if w.name == "cfg3":
+            other_configs = run_other_configs(elg, stream, dev)
 
     if roofline is not None and probes:
         # north_star's target sentence: ">= 70 % of B200 HBM bandwidth on the fused element-chain and compaction kernels at
@@ -423,7 +426,7 @@ def run_ours(args):
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "kernel_ms_per_step": {k: round(v[1] / args.steps, 4) for k, v in kinds.items()},
         "kernel_share": shares,
-        "roofline": roofline, "probes": probes, "cpu_baseline": cpu,
+        "roofline": roofline, "configs": other_configs, "probes": probes, "cpu_baseline": cpu,
         "hbm_peak_gbs": hbm_peak, "hbm_peak_source": peak_src,
     }
     print(json.dumps(line), flush=True)
@@ -442,6 +445,44 @@ def line_passes(gb, w):
             total += n
         n -= int(lost_at[k])
     return float(total)
+
+
+def run_other_configs(elg, stream, dev, steps=10, warmup=3):
+    """BASELINE.json's configs 0, 1, 2 and 4 at their own sizes (1e5 ... 1e7 particles: launch-latency-sized and
+    largely L2-resident): one step = the whole job of the config (cfg2: its 10 passes), median of `steps`
+    CUDA-event timings, inputs resident.  Parity at these sizes: tests/test_gpu_parity.py, tests/test_gpu_fullsize.py."""
+    import torch
+    from elg_inputs import make_workload
+    out = {}
+    for name in ("cfg0", "cfg1", "cfg2", "cfg4"):
+        w = make_workload(name)
+        n0 = w.n0
+        hp = torch.empty((6, n0), dtype=torch.float64, pin_memory=True)
+        w.particles(n0, out=hp.numpy())
+        gb = elg.Bunch(None, w.p0c_eV, w.charge_C, beamline=None, n0=n0, device=str(dev), lost_capacity=n0)
+        bl = elg.Beamline(w.elements, ring=w.ring)
+        gb.upload(hp); gb.synchronize()
+        keep = gb.soa.clone()
+        times = []
+        launches = 0
+        for rep in range(warmup + steps):
+            gb.soa.copy_(keep); gb.rewind(); gb.synchronize()
+            l0 = elg.launch_count()
+            ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+            ev0.record(stream)
+            gb.track(bl, w.n_turns, moments_every=w.moments_every, records=False)
+            ev1.record(stream)
+            torch.cuda.synchronize(dev)
+            launches = elg.launch_count() - l0
+            if rep >= warmup:
+                times.append(ev0.elapsed_time(ev1))
+        ms = float(np.median(times))
+        passes = line_passes(gb, w) if not w.ring else float(n0) * w.n_pass_elements * w.n_turns
+        out[name] = {"particles": n0, "elements_per_pass": w.n_pass_elements, "passes_per_step": w.n_turns,
+                     "moments_every": w.moments_every, "ms_per_step": ms, "launches_per_step": int(launches),
+                     "value": passes / (ms * 1e-3) / 1e6, "unit": UNIT, "n_alive_after": int(gb.n_alive)}
+        del gb, keep, hp
+    return out
 
 
 def run_probes(elg, gb, restore, n0, w_main, hbm_peak, stream, dev, args):

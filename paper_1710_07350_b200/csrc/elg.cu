@@ -11,7 +11,9 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <cstdlib>
 #include <string>
+#include <utility>
 #include <vector>
 
 using namespace elg;
@@ -29,6 +31,24 @@ int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
         if (e_ != cudaSuccess)                                                                 \
             return fail(ELG_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
     } while (0)
+
+// Every kernel is launched with the programmatic-stream-serialization attribute (programmatic dependent launch): the
+// kernels' first statement is pdl_begin() = griddepcontrol.wait (elg_kernels.cuh), so the ordering is that of the stream
+// and only the launch latency between dependent kernels overlaps.  ELG_PDL=0 launches without it.
+bool pdl_enabled() {
+    static const bool on = [] { const char* e = std::getenv("ELG_PDL"); return !(e && std::atoi(e) == 0); }();
+    return on;
+}
+template <class... KArgs, class... Args>
+void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);      // errors surface in the caller's cudaGetLastError
+}
 
 constexpr double kCLight = 299792458.0;                 // m/s
 constexpr double kTwoPi = 6.283185307179586476925286766559;
@@ -355,7 +375,7 @@ extern "C" int32_t elg_workspace_bytes(int64_t n0, const elg_beamline* bl, int64
 
 extern "C" int32_t elg_bunch_rewind(elg_bunch* b) {
     if (!b) return fail(ELG_EINVAL, "elg_bunch_rewind: NULL bunch");
-    init_state_kernel<<<1, 1, 0, b->stream>>>(b->st, b->n0);
+    launch_k(init_state_kernel, 1, 1, 0, b->stream, b->st, b->n0);
     g_launches++;
     ELG_CK(cudaGetLastError());
     b->cur_buf = 0; b->cur_slot = 0; b->turn = 0; b->rec_count = 0;
@@ -470,7 +490,7 @@ extern "C" int32_t elg_dbg_fp64_peak(double* d_scratch, int64_t iters, double* h
     float ms = 0.f;
     for (int rep = 0; rep < 4; rep++) {                                // rep 0 warms the clocks up; best of the other three
         ELG_CK(cudaEventRecord(e0, st));
-        fp64_peak_kernel<<<grid, kBlock, 0, st>>>(d_scratch, iters, 0.999, 1e-7);
+        launch_k(fp64_peak_kernel, grid, kBlock, 0, st, d_scratch, iters, 0.999, 1e-7);
         ELG_CK(cudaEventRecord(e1, st));
         g_launches++;
         ELG_CK(cudaGetLastError());
@@ -494,7 +514,7 @@ extern "C" int32_t elg_bunch_upload(elg_bunch* b, const double* const h_coords[6
     }
     if (h_ids) ELG_CK(cudaMemcpyAsync(b->ids(0), h_ids, b->n0 * 8, cudaMemcpyHostToDevice, b->stream));
     else if (b->n0 > 0) {
-        iota_kernel<<<b->sms * 4, kBlock, 0, b->stream>>>(b->ids(0), b->n0);
+        launch_k(iota_kernel, b->sms * 4, kBlock, 0, b->stream, b->ids(0), b->n0);
         g_launches++;
         ELG_CK(cudaGetLastError());
     }
@@ -635,16 +655,19 @@ struct Tracker {
         {
             ProfScope ps(b, MAXOPS == kMaxOpsLarge ? ELG_K_CHAIN_LONG : (COMPACT ? ELG_K_CHAIN_COMPACT : ELG_K_CHAIN));
             if constexpr (MAXOPS == kMaxOpsLarge)
-                chain_long_kernel<MAXOPS, EXT><<<grid, LongCfg<EXT>::NT, chain_long_smem_bytes<EXT>(), b->stream>>>(a);
+                launch_k(chain_long_kernel<MAXOPS, EXT>, grid, LongCfg<EXT>::NT, chain_long_smem_bytes<EXT>(), b->stream, a);
             else if constexpr (COMPACT)
             {
-                void* kargs[] = {(void*)&a};                     // cooperative: every block resident (static tiles)
-                check(cudaLaunchCooperativeKernel((const void*)compact_kernel<MAXOPS, (EXT != 0), MOM>, dim3(grid), dim3(kC2Threads), kargs,
-                                                  compact_smem_bytes(), b->stream),
-                      "compact_kernel cooperative launch");
+                cudaLaunchConfig_t cfg{};                        // cooperative: every block resident (static tiles)
+                cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kC2Threads); cfg.dynamicSmemBytes = compact_smem_bytes(); cfg.stream = b->stream;
+                cudaLaunchAttribute attr[2];
+                attr[0].id = cudaLaunchAttributeCooperative; attr[0].val.cooperative = 1;
+                attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[1].val.programmaticStreamSerializationAllowed = 1;
+                cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 2 : 1;
+                check(cudaLaunchKernelEx(&cfg, compact_kernel<MAXOPS, (EXT != 0), MOM>, a), "compact_kernel cooperative launch");
             }
             else
-                chain_kernel<MAXOPS, P, (EXT != 0), MOM><<<grid, kBlock, 0, b->stream>>>(a);
+                launch_k(chain_kernel<MAXOPS, P, (EXT != 0), MOM>, grid, kBlock, 0, b->stream, a);
         }
         check(cudaGetLastError(), "chain_kernel launch");
         if (COMPACT) { b->cur_buf ^= 1; b->cur_slot ^= 1; }
@@ -803,7 +826,7 @@ struct Tracker {
         m.record = b->records + 43 * b->rec_count;
         {
             ProfScope ps(b, ELG_K_MOMENTS);
-            moments_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(m);
+            launch_k(moments_kernel, b->grid_mom, kBlock, 0, b->stream, m);
         }
         check(cudaGetLastError(), "moments_kernel launch");
         b->rec_count++;
@@ -877,7 +900,7 @@ struct Tracker {
                 // shared memory for the bins this element can occupy: small histograms get more resident blocks
                 d.smem_bins = e.nb < kDipoleSmemBins ? (e.nb + 31) / 32 * 32 : kDipoleSmemBins;
                 ProfScope ps(b, ELG_K_HIST);
-                dipole_hist_kernel<<<dipole_grid(d.smem_bins), kBlock, (size_t)d.smem_bins * 36, b->stream>>>(d);
+                launch_k(dipole_hist_kernel, dipole_grid(d.smem_bins), kBlock, (size_t)d.smem_bins * 36, b->stream, d);
             } else {
                 HistArgs h;
                 h.s = b->coord(b->cur_buf, 4); h.st = b->st; h.cur = b->cur_slot; h.n_fixed = -1; h.prof_kind = b->prof_on ? ELG_K_HIST : -1;
@@ -887,8 +910,8 @@ struct Tracker {
                 // resident blocks (more loads in flight)
                 h.smem_bins = (8LL * e.nb < kHistSmemBins) ? 8 * e.nb : kHistSmemBins;
                 ProfScope ps(b, ELG_K_HIST);
-                if (h.aggregate) hist_kernel<true><<<hist_grid(h.smem_bins), kBlock, h.smem_bins * 4, b->stream>>>(h);
-                else hist_kernel<false><<<hist_grid(h.smem_bins), kBlock, h.smem_bins * 4, b->stream>>>(h);
+                if (h.aggregate) launch_k(hist_kernel<true>, hist_grid(h.smem_bins), kBlock, h.smem_bins * 4, b->stream, h);
+                else launch_k(hist_kernel<false>, hist_grid(h.smem_bins), kBlock, h.smem_bins * 4, b->stream, h);
 
             }
             check(cudaGetLastError(), "hist_kernel launch");
@@ -907,14 +930,14 @@ struct Tracker {
         w.dacc = dipole ? reinterpret_cast<long long*>(b->dacc) : nullptr;
         {
             ProfScope ps(b, ELG_K_WINDOW);
-            window_kernel<<<(e.nb + 4 * kBlock - 1) / (4 * kBlock), kBlock, 0, b->stream>>>(w);
+            launch_k(window_kernel, (e.nb + 4 * kBlock - 1) / (4 * kBlock), kBlock, 0, b->stream, w);
         }
         check(cudaGetLastError(), "window_kernel launch");
     }
 
     void dipole_finalize(int nb) {                                    // fixed-point accumulators -> Dx, Dy (G33)
         ProfScope ps(b, ELG_K_CONV);
-        dipole_finalize_kernel<<<(nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(b->dacc, nb, b->D);
+        launch_k(dipole_finalize_kernel, (nb + kBlock - 1) / kBlock, kBlock, 0, b->stream, b->dacc, nb, b->D);
         check(cudaGetLastError(), "dipole_finalize_kernel launch");
     }
 
@@ -943,7 +966,7 @@ struct Tracker {
         wa.table = b->table + bl->table_off[k]; wa.n_table = e.n_table; wa.dt_table = e.dt_table; wa.W = b->W;
         {
             ProfScope ps(b, ELG_K_WAKE_SAMPLES);
-            wake_samples_kernel<<<(e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream>>>(wa);
+            launch_k(wake_samples_kernel, (e.nb + kBlock - 1) / kBlock, kBlock, 0, b->stream, wa);
         }
         check(cudaGetLastError(), "wake_samples_kernel launch");
     }
@@ -959,7 +982,7 @@ struct Tracker {
             cr.kloss = r.kloss; cr.alpha = r.alpha; cr.wbar = r.wbar; cr.ratio = r.ratio; cr.V = b->V;
             {
                 ProfScope ps(b, ELG_K_CONV);
-                conv_rec_kernel<<<1, kBlock, 0, b->stream>>>(cr);
+                launch_k(conv_rec_kernel, 1, kBlock, 0, b->stream, cr);
             }
             check(cudaGetLastError(), "conv_rec_kernel launch");
             if (o && o->V_out && o->V_written + e.nb <= o->V_capacity)
@@ -970,7 +993,7 @@ struct Tracker {
             cv.counts = b->counts; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro; cv.V = b->V;
             {
                 ProfScope ps(b, ELG_K_CONV);
-                conv_kernel<unsigned int><<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
+                launch_k(conv_kernel<unsigned int>, (e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream, cv);
             }
             check(cudaGetLastError(), "conv_kernel launch");
             if (o && o->V_out && o->V_written + e.nb <= o->V_capacity)
@@ -991,7 +1014,7 @@ struct Tracker {
                 cv.counts = b->D + (size_t)plane * e.nb; cv.W = b->W; cv.st = b->st; cv.nb = e.nb; cv.q = b->q_macro;
                 cv.V = b->Vt + (size_t)plane * e.nb;
                 ProfScope ps(b, ELG_K_CONV);
-                conv_kernel<double><<<(e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream>>>(cv);
+                launch_k(conv_kernel<double>, (e.nb + kWarps - 1) / kWarps, kBlock, 0, b->stream, cv);
             }
             check(cudaGetLastError(), "conv_kernel launch");
             if (o && o->V_out && o->V_written + 4LL * e.nb <= o->V_capacity) {
@@ -1032,7 +1055,7 @@ struct Tracker {
                         count();
                         if (b && ok()) {
                             ProfScope ps(b, ELG_K_MOMENTS);
-                            fiducial_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(b->coord(b->cur_buf, 4), b->st, b->cur_slot, s_here);
+                            launch_k(fiducial_kernel, b->grid_mom, kBlock, 0, b->stream, b->coord(b->cur_buf, 4), b->st, b->cur_slot, s_here);
                             check(cudaGetLastError(), "fiducial_kernel launch");
                         }
                         op.coef[5] = 1.0;
@@ -1178,7 +1201,7 @@ extern "C" int32_t elg_upload_and_track(elg_bunch* b, const elg_beamline* bl, co
     ELG_CK(cudaStreamWaitEvent(b->copy_stream, b->entry_ev, 0));
     if (h_ids) ELG_CK(cudaMemcpyAsync(b->ids(0), h_ids, b->n0 * 8, cudaMemcpyHostToDevice, b->stream));
     else {
-        iota_kernel<<<b->sms * 4, kBlock, 0, b->stream>>>(b->ids(0), b->n0);
+        launch_k(iota_kernel, b->sms * 4, kBlock, 0, b->stream, b->ids(0), b->n0);
         g_launches++;
         ELG_CK(cudaGetLastError());
     }
@@ -1228,7 +1251,7 @@ extern "C" int32_t elg_moments(elg_bunch* b, int64_t* n_alive, double h_centroid
     for (int k = 0; k < 6; k++) m.src[k] = b->coord(b->cur_buf, k);
     m.st = b->st; m.cur = b->cur_slot; m.partial = b->mom_partial; m.prof_kind = -1;
     m.record = b->records + 43 * kRecCap;
-    moments_kernel<<<b->grid_mom, kBlock, 0, b->stream>>>(m);
+    launch_k(moments_kernel, b->grid_mom, kBlock, 0, b->stream, m);
     g_launches++;
     ELG_CK(cudaGetLastError());
     double rec[43];
@@ -1391,7 +1414,7 @@ extern "C" int32_t elg_dbg_wake_samples(int32_t kind, int32_t nb, double dt, dou
         if (!d_table || n_table < 1 || !(dt_table > 0.0)) return fail(ELG_EINVAL, "elg_dbg_wake_samples: bad table");
     } else return fail(ELG_EINVAL, "elg_dbg_wake_samples: bad kind");
     wa.table = d_table; wa.n_table = n_table; wa.dt_table = dt_table; wa.W = d_W;
-    wake_samples_kernel<<<(nb + kBlock - 1) / kBlock, kBlock, 0, (cudaStream_t)stream>>>(wa);
+    launch_k(wake_samples_kernel, (nb + kBlock - 1) / kBlock, kBlock, 0, (cudaStream_t)stream, wa);
     g_launches++;
     ELG_CK(cudaGetLastError());
     return ELG_OK;
@@ -1402,7 +1425,7 @@ extern "C" int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W,
     if (nb < 1 || !d_counts || !d_W || !d_V) return fail(ELG_EINVAL, "elg_dbg_convolve: bad arguments");
     ConvArgs<unsigned int> cv;
     cv.counts = d_counts; cv.W = d_W; cv.st = nullptr; cv.nb = nb; cv.q = q; cv.V = d_V;
-    conv_kernel<unsigned int><<<(nb + kWarps - 1) / kWarps, kBlock, 0, (cudaStream_t)stream>>>(cv);
+    launch_k(conv_kernel<unsigned int>, (nb + kWarps - 1) / kWarps, kBlock, 0, (cudaStream_t)stream, cv);
     g_launches++;
     ELG_CK(cudaGetLastError());
     return ELG_OK;
