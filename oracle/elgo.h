@@ -29,8 +29,11 @@
  *   elgo_track record placement (ELGO_MOM_ELEMENT / ELGO_MOM_TURN, G26)  pinned - three-particle hand case, 77 records
  *                               for cfg1; ring flag (G8): RF reference advances per turn on a ring only
  *   elgo_moments      pinned  - symmetric hand sets, shift invariance, Gaussian statistics
- *   elgo_track on whole configs: PARITY UNPINNED by the paper (no published end-to-end values);
- *                     it is the composition of the pinned stages in the order of PAPER.md:51.
+ *   elgo_track        pinned  - equals the composition, by hand, of the pinned stage functions in the order of
+ *                               PAPER.md:51 (test_track_is_the_composition_of_stages, test_trwake_track_is_...),
+ *                               turn advance and thread-count invariance, loss sequence of a small cfg4, record
+ *                               placement (above).  The paper prints no end-to-end values for whole beamlines, so
+ *                               nothing beyond the composition can be pinned to it.
  *
  * Precision: the paper computes in double precision; so does the oracle.  Sums
  * (convolution, moments) are accumulated in long double so that the oracle is closer to the exact
