@@ -713,7 +713,7 @@ struct Tracker {
         int ext = 0;                                                  // rarely used maps: higher EXT instantiations
         bool has_unc = false;
         for (const HostOp& op : pending) {
-            if (op.type == OP_MATRIX2 || op.type == OP_TKICK) ext = ext < 1 ? 1 : ext;
+            if (op.type == OP_MATRIX2 || (op.type == OP_TKICK && (large || compact || !ELG_TKICK_BASE))) ext = ext < 1 ? 1 : ext;
             if (op.type == OP_MATRIX3) ext = 2;
             has_unc = has_unc || op.type == OP_MATRIX_UNC;
         }

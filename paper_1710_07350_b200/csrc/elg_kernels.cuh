@@ -39,6 +39,9 @@ constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
 #define ELG_L1_PL 6
 #define ELG_L1_REGS 200
 #endif
+#ifndef ELG_TKICK_BASE
+#define ELG_TKICK_BASE 1         // 1: the base (fully unrolled) chain_kernel instantiations also hold the transverse wake kick
+#endif
 #ifndef ELG_BIN_MAGIC
 #define ELG_BIN_MAGIC 1          // bin_of: floor by adding 1.5 x 2^52 instead of FRND / F2I (0: conversions)
 #endif
@@ -419,13 +422,18 @@ __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, 
     }
 }
 
-// EXT = false leaves out the rarely used maps (MATRIX2, TKICK): the HBM-bound short kernels stay at ~60 registers
-// (4 blocks per SM); the planner picks the EXT = true instantiation when a run holds one of them.
-// Without the rarely used maps the loop over the MAXOPS parameter slots is fully unrolled, so every coefficient has a
+// EXT = false leaves out the second-order map: the HBM-bound short kernels stay at 72 registers (3 blocks per SM); the
+// planner picks the EXT = true instantiation when a run holds a MATRIX2.  TK: the transverse wake kick is compiled in
+// (chain_kernel always; compact_kernel only with EXT: with the kick in its base form the compaction measured 1.5 %
+// slower at 1e8 particles, and a TKICK directly in front of an aperture is rare).
+// Without the second-order map the loop over the MAXOPS parameter slots is fully unrolled, so every coefficient has a
 // compile-time offset in the constant bank and reaches its DFMA as a uniform-register operand (LDCU + DFMA R, R, UR, R):
 // no per-coefficient LDC through the MIO (profiles/r01d: 6 -> 53 DFMA/clk/SM at two particles per thread in a
-// register-only loop).  Only the slots a run uses are ever fetched, so the larger code does not cost instruction cache.
-template <int MAXOPS, int P, bool EXT>
+// register-only loop), no register copy-back after a matrix, no type dispatch at run time (an RFCW cavity's fused run
+// -- KICK, TKICK, MATRIX, RFKICK -- ran 443 instructions per particle in the EXT form, 25 % of them moves: 1.99 -> 1.87
+// ms per cavity at 1e8 particles).  Only the slots a run uses are ever fetched, so the larger code does not cost
+// instruction cache.
+template <int MAXOPS, int P, bool EXT, bool TK = false>
 __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
     const int n_ops = a.c.n_ops;
     if constexpr (!EXT) {
@@ -442,7 +450,7 @@ __device__ __forceinline__ void apply_ops(const ChainArgs<MAXOPS>& a, double (&v
 #pragma unroll
                     for (int r = 0; r < 6; r++) v[p][r] = w[p][r];
             } else {
-                other_map<P, false>(ty, c, a.c, v);
+                other_map<P, TK>(ty, c, a.c, v);
             }
         }
     } else {                                                     // with the second-order code per slot the unrolled form spills
@@ -589,12 +597,12 @@ __device__ __forceinline__ void moments_finish(const double (&acc)[kNMom], const
 // The shift K of the moment epilogue: the run's maps applied to particle 0 of the store (every thread computes the
 // same K; non-finite components become 0).  It only has to lie inside the distribution (conditioning of the
 // one-pass formula: s is an absolute path length), it need not be a survivor.
-template <int MAXOPS, bool EXT>
+template <int MAXOPS, bool EXT, bool TK = false>
 __device__ __forceinline__ void moment_shift(const ChainArgs<MAXOPS>& a, long long n, double (&K)[6]) {
     double k2[2][6];
 #pragma unroll
     for (int cc = 0; cc < 6; cc++) { k2[0][cc] = (n > 0) ? __ldg(a.c.src[cc]) : 0.0; k2[1][cc] = k2[0][cc]; }
-    apply_ops<MAXOPS, 2, EXT>(a, k2);
+    apply_ops<MAXOPS, 2, EXT, TK>(a, k2);
 #pragma unroll
     for (int cc = 0; cc < 6; cc++) K[cc] = (fabs(k2[0][cc]) < INFINITY) ? k2[0][cc] : 0.0;
 }
@@ -616,7 +624,7 @@ __global__ void __launch_bounds__(kBlock, ((P >= 4 || MOM) ? 2 : 3)) chain_kerne
     account_work(c.st, c.prof_kind, n - c.range_lo, c.bytes_pp, c.flops_pp);
     double K[MOM ? 6 : 1], acc[MOM ? kNMom : 1];
     if constexpr (MOM) {
-        moment_shift<MAXOPS, EXT>(a, n, K);
+        moment_shift<MAXOPS, EXT, (ELG_TKICK_BASE != 0)>(a, n, K);
 #pragma unroll
         for (int q = 0; q < kNMom; q++) acc[q] = 0.0;
     }
@@ -642,7 +650,7 @@ __global__ void __launch_bounds__(kBlock, ((P >= 4 || MOM) ? 2 : 3)) chain_kerne
             }
         }
 
-        apply_ops<MAXOPS, P, EXT>(a, v);
+        apply_ops<MAXOPS, P, EXT, (ELG_TKICK_BASE != 0)>(a, v);
 
 #pragma unroll
         for (int h = 0; h < H; h++) {
