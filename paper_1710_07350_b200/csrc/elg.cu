@@ -628,6 +628,7 @@ struct Tracker {
                 case OP_RFKICK: c.flops_pp += 6u; break;
                 case OP_KICK: c.flops_pp += 10u; break;
                 case OP_TKICK: c.flops_pp += 14u; break;
+                case OP_KICK3: c.flops_pp += 18u; break;
                 default: break;
             }
         }
@@ -694,6 +695,7 @@ struct Tracker {
                 case OP_MATRIX: case OP_MATRIX2: case OP_MATRIX3: case OP_MATRIX_UNC: rmask |= 0x3F; wmask |= 0x3F; break;
                 case OP_RFKICK: case OP_KICK: rmask |= 0x30; wmask |= 0x20; break;   // reads s delta, writes delta
                 case OP_TKICK: rmask |= 0x1A; wmask |= 0x0A; break;                  // reads x' y' s, writes x' y'
+                case OP_KICK3: rmask |= 0x3A; wmask |= 0x2A; break;                  // both
             }
         }
         if (want_mm) rmask |= 0x10;
@@ -713,7 +715,7 @@ struct Tracker {
         int ext = 0;                                                  // rarely used maps: higher EXT instantiations
         bool has_unc = false;
         for (const HostOp& op : pending) {
-            if (op.type == OP_MATRIX2 || (op.type == OP_TKICK && (large || compact || !ELG_TKICK_BASE))) ext = ext < 1 ? 1 : ext;
+            if (op.type == OP_MATRIX2 || ((op.type == OP_TKICK || op.type == OP_KICK3) && (large || compact || !ELG_TKICK_BASE))) ext = ext < 1 ? 1 : ext;
             if (op.type == OP_MATRIX3) ext = 2;
             has_unc = has_unc || op.type == OP_MATRIX_UNC;
         }
@@ -874,6 +876,12 @@ struct Tracker {
                 else if (o) { o->window_written++; o->hist_written += e.nb; }
                 trwake_part(k + 1);
                 skip_next = true;
+                // both kicks look the same bin up: one op (identical arithmetic per coordinate, one bin_of)
+                const size_t np = pending.size();
+                if (np >= 2 && pending[np - 2].type == OP_KICK && pending[np - 1].type == OP_TKICK && kick_nb == tk_nb && kick_interp == tk_interp) {
+                    pending.pop_back();
+                    pending.back().type = OP_KICK3;
+                }
             }
         } else {
             trwake_part(k);

@@ -56,7 +56,8 @@ enum : uint8_t { OP_DRIFT = 1, OP_MATRIX = 2, OP_RFKICK = 3, OP_KICK = 4,
                  OP_CONT = 6,
                  OP_TKICK = 7,        // transverse wake kick of the preceding TRWAKE (G32)
                  OP_MATRIX3 = 8,      // third-order map: R, C | 3 slots Tt[21][6] | 8 slots Ut[56][6] (12 slots, G35)
-                 OP_MATRIX_UNC = 9 }; // MATRIX whose zero pattern is that of an uncoupled element (flagged option)
+                 OP_MATRIX_UNC = 9,   // MATRIX whose zero pattern is that of an uncoupled element (flagged option)
+                 OP_KICK3 = 10 };     // OP_KICK + OP_TKICK of an RFCW composite (same binning): one bin look-up for both
 enum { AP_NONE = 0, AP_RCOL = 1, AP_ECOL = 2 };
 
 // Device-resident tracking state (first bytes of the workspace).  Nothing here is read by the host
@@ -416,6 +417,38 @@ __device__ __forceinline__ void other_map(int ty, const double* __restrict__ c, 
                 vx = fma(fr, x1 - x0, x0);
                 vy = fma(fr, y1 - y0, y0);
             }
+            v[p][1] = fma(vx, inv_E, v[p][1]);
+            v[p][3] = fma(vy, inv_E, v[p][3]);
+        }
+    } else if (EXT && ty == OP_KICK3) {                          // G14 + G32 with a shared bin and interpolation weight:
+        const double inv_bc = c[0], inv_E = c[1];                //   the same operations on each coordinate as OP_KICK
+        const double t_lo = cm.st->win[0], inv_dt = cm.st->win[2];   // followed by OP_TKICK (neither changes s)
+        const int nb = cm.nb;
+#pragma unroll
+        for (int p = 0; p < P; p++) {
+            double u0;
+            const int b = bin_of(v[p][4], inv_bc, t_lo, inv_dt, nb, &u0);
+            if (b < 0) continue;
+            double Vt, vx, vy;
+            if (!cm.interp || nb < 2) {
+                Vt = __ldg(cm.V + b); vx = __ldg(cm.Vx + b); vy = __ldg(cm.Vy + b);
+            } else {
+                const double u = u0 - 0.5;
+                double k = floor(u);
+                if (k < 0.0) k = 0.0;
+                if (k > (double)(nb - 2)) k = (double)(nb - 2);
+                double fr = u - k;
+                if (fr < 0.0) fr = 0.0;
+                if (fr > 1.0) fr = 1.0;
+                const int ki = (int)k;
+                const double V0 = __ldg(cm.V + ki), V1 = __ldg(cm.V + ki + 1);
+                const double x0 = __ldg(cm.Vx + ki), x1 = __ldg(cm.Vx + ki + 1);
+                const double y0 = __ldg(cm.Vy + ki), y1 = __ldg(cm.Vy + ki + 1);
+                Vt = fma(fr, V1 - V0, V0);
+                vx = fma(fr, x1 - x0, x0);
+                vy = fma(fr, y1 - y0, y0);
+            }
+            v[p][5] = fma(-Vt, inv_E, v[p][5]);
             v[p][1] = fma(vx, inv_E, v[p][1]);
             v[p][3] = fma(vy, inv_E, v[p][3]);
         }
