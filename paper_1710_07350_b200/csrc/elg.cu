@@ -35,6 +35,11 @@ int32_t fail(int32_t code, const std::string& msg) { g_err = msg; return code; }
 // Every kernel is launched with the programmatic-stream-serialization attribute (programmatic dependent launch): the
 // kernels' first statement is pdl_begin() = griddepcontrol.wait (elg_kernels.cuh), so the ordering is that of the stream
 // and only the launch latency between dependent kernels overlaps.  ELG_PDL=0 launches without it.
+// ELG_CHAIN_RING=0: short runs through chain_kernel (loads held in registers) instead of chain_ring_kernel
+bool ring_enabled() {
+    static const bool on = [] { const char* e = std::getenv("ELG_CHAIN_RING"); return !(e && std::atoi(e) == 0); }();
+    return on;
+}
 bool pdl_enabled() {
     static const bool on = [] { const char* e = std::getenv("ELG_PDL"); return !(e && std::atoi(e) == 0); }();
     return on;
@@ -241,6 +246,7 @@ int32_t long_setup_once() {
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<1>()));
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<2>()));
         ELG_CK(cudaFuncSetAttribute(chain_long_kernel<kMaxOpsLarge, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_long_smem_bytes<3>()));
+        ELG_CK(cudaFuncSetAttribute(chain_ring_kernel<kMaxOpsSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize, chain_ring_smem_bytes()));
         ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
         ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
         ELG_CK(cudaFuncSetAttribute(compact_kernel<kMaxOpsSmall, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, compact_smem_bytes()));
@@ -648,6 +654,9 @@ struct Tracker {
         else if constexpr (COMPACT) {
             grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0), MOM>, compact_smem_bytes(), kC2Threads);
             if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
+        } else if constexpr (P == 2 && EXT == 0 && !MOM) {
+            if (ring_enabled()) grid = cached_grid((const void*)chain_ring_kernel<MAXOPS>, chain_ring_smem_bytes(), kCrThreads);
+            else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, false, MOM>, 0);
         } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, (EXT != 0), MOM>, 0);
         if (!ok()) return;
         if ((long long)(mm_slot + 1) * grid > kMmPartials) { rc = fail(ELG_ECAPACITY, "elg_upload_and_track: too many chunks for the min/max partial slots"); return; }
@@ -666,6 +675,10 @@ struct Tracker {
                 attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[1].val.programmaticStreamSerializationAllowed = 1;
                 cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 2 : 1;
                 check(cudaLaunchKernelEx(&cfg, compact_kernel<MAXOPS, (EXT != 0), MOM>, a), "compact_kernel cooperative launch");
+            }
+            else if constexpr (P == 2 && EXT == 0 && !MOM) {
+                if (ring_enabled()) launch_k(chain_ring_kernel<MAXOPS>, grid, kCrThreads, chain_ring_smem_bytes(), b->stream, a);
+                else launch_k(chain_kernel<MAXOPS, P, false, MOM>, grid, kBlock, 0, b->stream, a);
             }
             else
                 launch_k(chain_kernel<MAXOPS, P, (EXT != 0), MOM>, grid, kBlock, 0, b->stream, a);

@@ -1188,6 +1188,121 @@ __global__ void __launch_bounds__(kC2Threads, (MOM ? 1 : ELG_C2_BLOCKS)) compact
 }
 
 // ---------------------------------------------------------------------------------------------------
+// chain_ring_kernel: the HBM-bound short run (at most two matrices, basic maps) with the LOAD side of compact_kernel:
+// a producer warp keeps a shared-memory ring of S tiles full with 1-D bulk copies (TMA unit, one per coordinate the run
+// reads, completion counted in bytes on the stage's mbarrier), the compute warps take a tile out of its stage into
+// registers, release the stage at once, apply the run's maps and store with 128-bit st.global.  The load stream no
+// longer stops while a warp computes or stores (chain_kernel holds its in-flight loads in registers).  Same arithmetic,
+// same order, as chain_kernel; tiles are dealt round-robin to a persistent grid.  Measured at 1e8 particles
+// (profiles/r02d_variants.md): DRIFT + MATRIX 1.626 -> 1.584 ms (6.06 TB/s) with 2 stages and 3 blocks per SM; 3 - 5
+// stages at 2 blocks per SM are slower, and so is the moment epilogue on this structure (one block of 8 compute warps
+// per SM: 1.15 -> 1.27 ms), which therefore stays with chain_kernel.
+// ---------------------------------------------------------------------------------------------------
+#ifndef ELG_CR_BLOCKS
+#define ELG_CR_BLOCKS 3
+#endif
+#ifndef ELG_CR_S
+#define ELG_CR_S 2
+#endif
+constexpr int kCrNT = 256;                              // compute threads per block (+ one producer warp)
+constexpr int kCrTile = 2 * kCrNT;                      // thread t owns particles 2t, 2t + 1 of the tile
+constexpr int kCrS = ELG_CR_S;                          // ring stages
+constexpr int kCrThreads = kCrNT + 32;
+constexpr int chain_ring_smem_bytes() { return kCrS * 6 * kCrTile * 8; }
+
+template <int MAXOPS>
+__global__ void __launch_bounds__(kCrThreads, ELG_CR_BLOCKS) chain_ring_kernel(const __grid_constant__ ChainArgs<MAXOPS> a) {
+    pdl_begin();
+    constexpr int NT = kCrNT, TILE = kCrTile, S = kCrS, NW = NT / 32;
+    const ChainCommon& c = a.c;
+    const long long n_all = c.st->n_alive[c.cur];
+    const long long n = (c.range_hi >= 0 && c.range_hi < n_all) ? c.range_hi : n_all;       // end of my range
+    const long long n_tiles = (n > c.range_lo) ? (n - c.range_lo + TILE - 1) / TILE : 0;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    account_work(c.st, c.prof_kind, n - c.range_lo, c.bytes_pp, c.flops_pp);
+
+    extern __shared__ __align__(16) double cr_ring[];            // [S][6][TILE]
+    __shared__ unsigned long long s_full[S], s_empty[S];         // mbarriers: tile landed / stage read by all
+    const long long G = gridDim.x;
+    const long long n_it = (n_tiles > blockIdx.x) ? (n_tiles - blockIdx.x + G - 1) / G : 0;  // my tiles
+
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < S; k++) { mbar_init(&s_full[k], 1); mbar_init(&s_empty[k], NT); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (wid == NW) {                                             // producer warp: one lane feeds the ring
+        if (lane == 0) {
+            const unsigned int n_rd = (unsigned int)__popc(c.rmask & 0x3Fu);
+            for (long long it = 0; it < n_it; it++) {
+                const int stg = (int)(it % S);
+                const long long use = it / S;
+                if (use > 0) mbar_wait(&s_empty[stg], (unsigned int)((use - 1) & 1));
+                const long long i0 = c.range_lo + (blockIdx.x + it * G) * TILE;
+                const long long left = n - i0;
+                // whole 16-byte units; an odd tail reads one element past n, inside the array's 256-byte padding
+                const unsigned int bytes = (unsigned int)(((left < TILE ? left : TILE) + 1) / 2) * 16u;
+                double* stage = cr_ring + (size_t)stg * 6 * TILE;
+                mbar_expect_tx(&s_full[stg], n_rd * bytes);
+#pragma unroll
+                for (int cc = 0; cc < 6; cc++)
+                    if (c.rmask & (1u << cc)) bulk_g2s(stage + cc * TILE, c.src[cc] + i0, bytes, &s_full[stg]);
+            }
+        }
+        return;
+    }
+
+    double mn = INFINITY, mx = -INFINITY;
+
+    for (long long it = 0; it < n_it; it++) {
+        const int stg = (int)(it % S);
+        const long long i0 = c.range_lo + (blockIdx.x + it * G) * TILE + (long long)threadIdx.x * 2;
+        const double* stage = cr_ring + (size_t)stg * 6 * TILE + threadIdx.x * 2;
+        mbar_wait(&s_full[stg], (unsigned int)((it / S) & 1));
+        double v[2][6];
+#pragma unroll
+        for (int cc = 0; cc < 6; cc++) {
+            double2 t = make_double2(0.0, 0.0);
+            if (c.rmask & (1u << cc)) t = *reinterpret_cast<const double2*>(stage + cc * TILE);
+            v[0][cc] = t.x; v[1][cc] = t.y;
+        }
+        fence_proxy_async();                                     // my generic-proxy reads before the next bulk write
+        mbar_arrive(&s_empty[stg]);                              // stage released (NT arrivals complete the phase)
+        const bool full = (i0 + 2 <= n), one = (i0 < n);         // slots past n hold stale bytes: mapped, never used
+
+        apply_ops<MAXOPS, 2, false, (ELG_TKICK_BASE != 0)>(a, v);
+
+#pragma unroll
+        for (int cc = 0; cc < 6; cc++) {
+            if (c.wmask & (1u << cc)) {
+                if (full) *reinterpret_cast<double2*>(c.dst[cc] + i0) = make_double2(v[0][cc], v[1][cc]);
+                else if (one) c.dst[cc][i0] = v[0][cc];
+            }
+        }
+        if (c.want_minmax) {
+            if (one) { mn = fmin(mn, v[0][4]); mx = fmax(mx, v[0][4]); }
+            if (full) { mn = fmin(mn, v[1][4]); mx = fmax(mx, v[1][4]); }
+        }
+    }
+
+    if (c.want_minmax) {                                         // exact min/max of s (a8): order-independent
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, d));
+            mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+        }
+        __shared__ double s_mn[NW], s_mx[NW];
+        if (lane == 0) { s_mn[wid] = mn; s_mx[wid] = mx; }
+        named_barrier<1, NT>();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < NW; w++) { mn = fmin(mn, s_mn[w]); mx = fmax(mx, s_mx[w]); }
+            c.mm_partial[2 * blockIdx.x] = mn;
+            c.mm_partial[2 * blockIdx.x + 1] = mx;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // window_kernel (a8 -> G10): reduce the per-block min/max partials (exact in any order), derive the
 // histogram window with the same fp64 operations as the definition, the occupied bin range used for
 // shared-memory privatisation, and zero the counts (every block zeroes a slice, block 0 does the rest).

@@ -265,3 +265,31 @@ def test_wake_and_trwake_own_bin_kicks_end_to_end(elg, elgo, n):
         wi = make_workload("p5-trwake", n=n)
         oi = elgo.Bunch(v0, w.p0c_eV, w.charge_C); oi.track(elgo.Beamline(wi.elements), 1, n_threads=8)
         assert np.max(np.abs(oi.read()[0][1] - ov[1])) > 0
+
+
+def test_rfcw_pair_with_different_interpolation_flags(elg, elgo):
+    """A WAKE + TRWAKE pair that shares its histogram pass but not its interpolation rule: the planner must keep two
+    kick ops (the fused OP_KICK3 holds one rule for both)."""
+    n = 50_003
+    w = make_workload("p5-trwake", n=n)
+    pair = [{"type": "WAKE", "nb": 300, "window": "AUTO_MINMAX", "wake": "RESONATOR", "f": 1.3e9, "Q": 5.0, "Rs": 1e3,
+             "interp": True},
+            {"type": "TRWAKE", "nb": 300, "window": "AUTO_MINMAX", "wake": "RESONATOR_T", "f": 2.4e9, "Q": 10.0,
+             "Rs": 1e6, "interp": False},
+            {"type": "DRIFT", "L": 0.1}]
+    same = [dict(e, interp=True) for e in pair[:2]] + [pair[2]]
+    v0 = w.particles()
+    v0[0] += 2e-4; v0[2] -= 1e-4
+    res = {}
+    for name, elems in (("mixed", pair), ("both", same)):
+        ob = elgo.Bunch(v0, w.p0c_eV, w.charge_C)
+        ob.track(elgo.Beamline(elems), 1, n_threads=8)
+        gbl = elg.Beamline(elems); gb = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=gbl)
+        gb.track(gbl, 1)
+        ov, oid = ob.read(); gv, gid = gb.read()
+        assert np.array_equal(gid, oid)
+        sig = ov.std(axis=1, keepdims=True)
+        assert np.max(np.abs(gv - ov) / np.maximum(np.abs(ov), sig)) <= 1e-12
+        res[name] = gv
+    assert np.array_equal(res["mixed"][5], res["both"][5])          # same longitudinal kick
+    assert np.max(np.abs(res["mixed"][1] - res["both"][1])) > 0      # different transverse rule
