@@ -594,6 +594,16 @@ struct Tracker {
         return (int)g;
     }
 
+    // chain_ring_kernel takes the short runs that are nothing but DRIFT / MATRIX maps (the purely HBM-bound ones: 1.626 ->
+    // 1.584 ms at 1e8 particles); with a wake or RF kick in the run the register-held form measured as fast or faster
+    // (cfg2's KICK + DRIFT at 1e7 particles: 0.163 vs 0.174 ms per pass)
+    bool use_ring() const {
+        if (!ring_enabled()) return false;
+        for (const HostOp& op : pending)
+            if (op.type != OP_DRIFT && op.type != OP_MATRIX) return false;
+        return !pending.empty();
+    }
+
     // EXT: 0 basic maps, 1 + MATRIX2 / TKICK, 2 + MATRIX3, 3 pattern matrices.  MOM: moment epilogue (record slot rec_count)
     template <int MAXOPS, bool COMPACT, int P, int EXT, bool MOM = false>
     void launch_chain(int ap_type, double ap_x, double ap_y, long long te_code, bool want_mm, unsigned rmask, unsigned wmask) {
@@ -655,7 +665,7 @@ struct Tracker {
             grid = cached_grid((const void*)compact_kernel<MAXOPS, (EXT != 0), MOM>, compact_smem_bytes(), kC2Threads);
             if (grid > kCompactMaxGrid) grid = kCompactMaxGrid;      // kPoll status words per thread
         } else if constexpr (P == 2 && EXT == 0 && !MOM) {
-            if (ring_enabled()) grid = cached_grid((const void*)chain_ring_kernel<MAXOPS>, chain_ring_smem_bytes(), kCrThreads);
+            if (use_ring()) grid = cached_grid((const void*)chain_ring_kernel<MAXOPS>, chain_ring_smem_bytes(), kCrThreads);
             else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, false, MOM>, 0);
         } else grid = cached_grid((const void*)chain_kernel<MAXOPS, P, (EXT != 0), MOM>, 0);
         if (!ok()) return;
@@ -677,7 +687,7 @@ struct Tracker {
                 check(cudaLaunchKernelEx(&cfg, compact_kernel<MAXOPS, (EXT != 0), MOM>, a), "compact_kernel cooperative launch");
             }
             else if constexpr (P == 2 && EXT == 0 && !MOM) {
-                if (ring_enabled()) launch_k(chain_ring_kernel<MAXOPS>, grid, kCrThreads, chain_ring_smem_bytes(), b->stream, a);
+                if (use_ring()) launch_k(chain_ring_kernel<MAXOPS>, grid, kCrThreads, chain_ring_smem_bytes(), b->stream, a);
                 else launch_k(chain_kernel<MAXOPS, P, false, MOM>, grid, kBlock, 0, b->stream, a);
             }
             else

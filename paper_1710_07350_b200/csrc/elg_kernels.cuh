@@ -632,12 +632,12 @@ __device__ __forceinline__ void moments_finish(const double (&acc)[kNMom], const
 // one-pass formula: s is an absolute path length), it need not be a survivor.
 template <int MAXOPS, bool EXT, bool TK = false>
 __device__ __forceinline__ void moment_shift(const ChainArgs<MAXOPS>& a, long long n, double (&K)[6]) {
-    double k2[2][6];
+    double k1[1][6];
 #pragma unroll
-    for (int cc = 0; cc < 6; cc++) { k2[0][cc] = (n > 0) ? __ldg(a.c.src[cc]) : 0.0; k2[1][cc] = k2[0][cc]; }
-    apply_ops<MAXOPS, 2, EXT, TK>(a, k2);
+    for (int cc = 0; cc < 6; cc++) k1[0][cc] = (n > 0) ? __ldg(a.c.src[cc]) : 0.0;
+    apply_ops<MAXOPS, 1, EXT, TK>(a, k1);
 #pragma unroll
-    for (int cc = 0; cc < 6; cc++) K[cc] = (fabs(k2[0][cc]) < INFINITY) ? k2[0][cc] : 0.0;
+    for (int cc = 0; cc < 6; cc++) K[cc] = (fabs(k1[0][cc]) < INFINITY) ? k1[0][cc] : 0.0;
 }
 
 // MOM: the run is followed by a moments record (G26): the 27 shifted sums are accumulated on the mapped particles
