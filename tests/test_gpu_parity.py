@@ -790,3 +790,45 @@ def test_fp64_peak_hook(elg):
     148 SMs x 64 DFMA/clk x 2 x clock."""
     tf, ms = elg.dbg_fp64_peak(5000)
     assert ms > 0 and 25.0 < tf < 45.0
+
+
+# ------------------------------------------------------------------------------------ launch options change no bit
+_SWITCH_SCRIPT = r"""
+import hashlib, sys
+import numpy as np
+sys.path.insert(0, {root!r})
+from elg_inputs import make_workload
+from paper_1710_07350_b200 import elg
+h = hashlib.sha256()
+for name, n, turns in (("cfg4", 300_007, 1), ("cfg0", 100_000, 1), ("cfg2", 200_003, 3), ("p6-rfcw", 150_001, 1), ("cfg1", 120_011, 1)):
+    w = make_workload(name, n=n)
+    bl = elg.Beamline(w.elements, ring=w.ring)
+    for rep in range(3):                                  # repeated: a launch-order race would not hit every time
+        b = elg.Bunch(w.particles(), w.p0c_eV, w.charge_C, beamline=bl, lost_capacity=n)
+        o = b.track(bl, turns, moments_every=w.moments_every, want_stage_outputs=True)
+        v, ids = b.read()
+        lost = b.lost()
+        for arr in (v, ids, o["hist"], o["V"], o["window"], o.get("records", np.zeros(0)), lost[0], lost[3]):
+            h.update(np.ascontiguousarray(arr).tobytes())
+print(h.hexdigest())
+"""
+
+
+@pytest.mark.gpu
+def test_launch_switches_change_no_bit(elg):
+    """Programmatic dependent launch (every kernel starts with griddepcontrol.wait) and the bulk-copy ring of the short
+    runs are launch mechanics: coordinates, IDs, histograms, voltages, windows, records and the lost log of five
+    workloads (61-launch cfg4, the compacting runs of cfg0 / cfg1 with records, multi-turn cfg2, RFCW cavities) must be
+    bit-identical with each of them switched off (ELG_PDL=0, ELG_CHAIN_RING=0), run three times each."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = _SWITCH_SCRIPT.format(root=root)
+    digests = {}
+    for tag, env in (("default", {}), ("no-pdl", {"ELG_PDL": "0"}), ("no-ring", {"ELG_CHAIN_RING": "0"})):
+        e = dict(os.environ); e.update(env)
+        out = subprocess.run([sys.executable, "-c", script], env=e, capture_output=True, text=True, check=True, timeout=600)
+        digests[tag] = out.stdout.strip().splitlines()[-1]
+    assert len(digests["default"]) == 64
+    assert digests["no-pdl"] == digests["default"] and digests["no-ring"] == digests["default"], digests
