@@ -39,6 +39,12 @@ constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
 #define ELG_L1_PL 6
 #define ELG_L1_REGS 200
 #endif
+#ifndef ELG_MM_ROWS
+#define ELG_MM_ROWS 2            // rows of a MATRIX formed together in the long-run kernel (levels 0, 2, 3)
+#endif
+#ifndef ELG_MM_ROWS_L1
+#define ELG_MM_ROWS_L1 1         // ... at level 1 (second-order maps)
+#endif
 #ifndef ELG_TKICK_BASE
 #define ELG_TKICK_BASE 1         // 1: the base (fully unrolled) chain_kernel instantiations also hold the transverse wake kick
 #endif
@@ -755,24 +761,39 @@ constexpr int chain_long_smem_bytes() { return 6 * LongCfg<LEVEL>::NT * LongCfg<
 // `zero` is a 0 loaded from the device state (opaque to the compiler, and a per-thread value to it): OR-ing it into the
 // bits of C[r] makes C[r] a vector value once per ROW without changing a bit of it, so that every DFMA of the row has
 // exactly one uniform operand.
-template <int P>
+// R rows are formed together, coefficient by coefficient: R x P accumulator chains in flight in SOURCE order.  ptxas
+// reschedules, but the order it is given matters: chain after chain (round 1 to mid round 2) ran cfg3 at 0.924 of the
+// fp64 peak, one row of P chains at 0.947, two rows at 0.949 (three: 0.943, six: 0.949; profiles/r02d_variants.md); the
+// second-order level is best with one row (p4 0.860 against 0.846).  Per chain the FMAs keep their order (G3).
+template <int P, int R>
 __device__ __forceinline__ void matrix_map_uniform(const double* __restrict__ c, long long zero, const double (&v)[P][6], double (&w)[P][6]) {
+    static_assert(6 % R == 0, "rows per group divide 6");
 #pragma unroll
-    for (int r = 0; r < 6; r++) {
-        const double cv = __longlong_as_double(__double_as_longlong(c[36 + r]) | zero);
+    for (int r0 = 0; r0 < 6; r0 += R) {
+        double acc[R][P];
 #pragma unroll
-        for (int p = 0; p < P; p++) {
-            double acc = cv;
+        for (int rr = 0; rr < R; rr++) {
+            const double cv = __longlong_as_double(__double_as_longlong(c[36 + r0 + rr]) | zero);
 #pragma unroll
-            for (int cc = 0; cc < 6; cc++) acc = fma(c[6 * r + cc], v[p][cc], acc);
-            w[p][r] = acc;
+            for (int p = 0; p < P; p++) acc[rr][p] = cv;
         }
+#pragma unroll
+        for (int cc = 0; cc < 6; cc++)
+#pragma unroll
+            for (int rr = 0; rr < R; rr++)
+#pragma unroll
+                for (int p = 0; p < P; p++) acc[rr][p] = fma(c[6 * (r0 + rr) + cc], v[p][cc], acc[rr][p]);
+#pragma unroll
+        for (int rr = 0; rr < R; rr++)
+#pragma unroll
+            for (int p = 0; p < P; p++) w[p][r0 + rr] = acc[rr][p];
     }
 }
 
 template <int MAXOPS, int P, int LEVEL>
 __device__ __forceinline__ void apply_ops_uniform(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
     const long long zero = a.c.st->zero_bits;                    // 0, but loaded: opaque to the compiler, and a vector value
+    constexpr int MMR = (LEVEL == 1) ? ELG_MM_ROWS_L1 : ELG_MM_ROWS;
     const int n_ops = a.c.n_ops;
     int op = 0;
     while (op < n_ops) {
@@ -782,12 +803,12 @@ __device__ __forceinline__ void apply_ops_uniform(const ChainArgs<MAXOPS>& a, do
 #pragma unroll 1
             for (; op + 1 < end; op += 2) {                      // pairs: v -> w -> v, no copy-back; nothing else in this loop
                 double w[P][6];
-                matrix_map_uniform<P>(a.coef[op], zero, v, w);
-                matrix_map_uniform<P>(a.coef[op + 1], zero, w, v);
+                matrix_map_uniform<P, MMR>(a.coef[op], zero, v, w);
+                matrix_map_uniform<P, MMR>(a.coef[op + 1], zero, w, v);
             }
             if (op < end) {
                 double w[P][6];
-                matrix_map_uniform<P>(a.coef[op], zero, v, w);
+                matrix_map_uniform<P, MMR>(a.coef[op], zero, v, w);
 #pragma unroll
                 for (int p = 0; p < P; p++)
 #pragma unroll
@@ -813,7 +834,7 @@ __device__ __forceinline__ void apply_ops_uniform(const ChainArgs<MAXOPS>& a, do
             }
         } else if ((LEVEL == 1 || LEVEL == 2) && (ty == OP_MATRIX2 || (LEVEL == 2 && ty == OP_MATRIX3))) {
             double w[P][6];
-            matrix_map_uniform<P>(a.coef[op], zero, v, w);
+            matrix_map_uniform<P, MMR>(a.coef[op], zero, v, w);
             matrix2_terms<P>(a.coef[op + 1], v, w);              // slots op + 1 .. op + 3: Tt[21][6]
             if (LEVEL == 2 && ty == OP_MATRIX3) matrix3_terms<P>(a.coef[op + 4], zero, v, w);     // op + 4 .. op + 11: Ut[56][6]
 #pragma unroll
