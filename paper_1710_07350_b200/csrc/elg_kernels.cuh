@@ -42,6 +42,9 @@ constexpr int kNMom = 27;              // 6 first + 21 second shifted sums
 #ifndef ELG_MM_ROWS
 #define ELG_MM_ROWS 2            // rows of a MATRIX formed together in the long-run kernel (levels 0, 2, 3)
 #endif
+#ifndef ELG_MM_ROWS_L3
+#define ELG_MM_ROWS_L3 0         // ... at level 3 (dense matrices between the zero-pattern ones of the flagged option); 0: chain after chain
+#endif
 #ifndef ELG_MM_ROWS_L1
 #define ELG_MM_ROWS_L1 1         // ... at level 1 (second-order maps)
 #endif
@@ -767,12 +770,27 @@ constexpr int chain_long_smem_bytes() { return 6 * LongCfg<LEVEL>::NT * LongCfg<
 // second-order level is best with one row (p4 0.860 against 0.846).  Per chain the FMAs keep their order (G3).
 template <int P, int R>
 __device__ __forceinline__ void matrix_map_uniform(const double* __restrict__ c, long long zero, const double (&v)[P][6], double (&w)[P][6]) {
-    static_assert(6 % R == 0, "rows per group divide 6");
+    if constexpr (R == 0) {                                      // chain after chain (the order level 3 is fastest with)
 #pragma unroll
-    for (int r0 = 0; r0 < 6; r0 += R) {
-        double acc[R][P];
+        for (int r = 0; r < 6; r++) {
+            const double cv = __longlong_as_double(__double_as_longlong(c[36 + r]) | zero);
 #pragma unroll
-        for (int rr = 0; rr < R; rr++) {
+            for (int p = 0; p < P; p++) {
+                double acc = cv;
+#pragma unroll
+                for (int cc = 0; cc < 6; cc++) acc = fma(c[6 * r + cc], v[p][cc], acc);
+                w[p][r] = acc;
+            }
+        }
+        return;
+    }
+    constexpr int RR = (R == 0) ? 1 : R;
+    static_assert(6 % RR == 0, "rows per group divide 6");
+#pragma unroll
+    for (int r0 = 0; r0 < 6; r0 += RR) {
+        double acc[RR][P];
+#pragma unroll
+        for (int rr = 0; rr < RR; rr++) {
             const double cv = __longlong_as_double(__double_as_longlong(c[36 + r0 + rr]) | zero);
 #pragma unroll
             for (int p = 0; p < P; p++) acc[rr][p] = cv;
@@ -780,11 +798,11 @@ __device__ __forceinline__ void matrix_map_uniform(const double* __restrict__ c,
 #pragma unroll
         for (int cc = 0; cc < 6; cc++)
 #pragma unroll
-            for (int rr = 0; rr < R; rr++)
+            for (int rr = 0; rr < RR; rr++)
 #pragma unroll
                 for (int p = 0; p < P; p++) acc[rr][p] = fma(c[6 * (r0 + rr) + cc], v[p][cc], acc[rr][p]);
 #pragma unroll
-        for (int rr = 0; rr < R; rr++)
+        for (int rr = 0; rr < RR; rr++)
 #pragma unroll
             for (int p = 0; p < P; p++) w[p][r0 + rr] = acc[rr][p];
     }
@@ -793,7 +811,7 @@ __device__ __forceinline__ void matrix_map_uniform(const double* __restrict__ c,
 template <int MAXOPS, int P, int LEVEL>
 __device__ __forceinline__ void apply_ops_uniform(const ChainArgs<MAXOPS>& a, double (&v)[P][6]) {
     const long long zero = a.c.st->zero_bits;                    // 0, but loaded: opaque to the compiler, and a vector value
-    constexpr int MMR = (LEVEL == 1) ? ELG_MM_ROWS_L1 : ELG_MM_ROWS;
+    constexpr int MMR = (LEVEL == 1) ? ELG_MM_ROWS_L1 : (LEVEL == 3) ? ELG_MM_ROWS_L3 : ELG_MM_ROWS;
     const int n_ops = a.c.n_ops;
     int op = 0;
     while (op < n_ops) {
