@@ -722,7 +722,7 @@ struct Tracker {
             }
         }
         if (want_mm) rmask |= 0x10;
-        // the long-run kernel (coefficients in shared memory, 6 particles per thread) also takes the short runs that
+        // the long-run kernel (coefficients as uniform operands, 6 particles per thread) also takes the short runs that
         // are already fp64-bound: from 5 matrices on it beats the parameter-bank kernel (bench.py p3 sweep)
         int n_mat_run = 0;
         for (const HostOp& op : pending) n_mat_run += (op.type == OP_MATRIX || op.type == OP_MATRIX_UNC) + 4 * (op.type == OP_MATRIX2);

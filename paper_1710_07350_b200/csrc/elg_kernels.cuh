@@ -242,7 +242,7 @@ __device__ __forceinline__ int bin_of(double s, double inv_bc, double t_lo, doub
 // Element maps on P particles held in registers.  Coefficients come straight from the kernel parameter
 // constant bank (uniform operands of DFMA), so a MATRIX costs 42 DFMA per particle and no LSU traffic.
 // One coefficient fetch (LDCU) feeds P DFMAs: P = 4 keeps the fp64 pipe, not the constant path, the
-// limiter of long runs (profiles/r01a_first_path.md).
+// limiter of long runs (profiles/r01a_first_path.md, round 1).
 // ---------------------------------------------------------------------------------------------------
 // v -> w through one MATRIX (G3): row r accumulates from C[r] over c = 0..5 with FMAs, in that order.
 template <int P>
@@ -747,7 +747,8 @@ __global__ void __launch_bounds__(kBlock, ((P >= 4 || MOM) ? 2 : 3)) chain_kerne
 // LEVEL 0: MATRIX, DRIFT, RFKICK, KICK; 1: + MATRIX2, TKICK; 2: + MATRIX3; 3: level 0 + MATRIX_UNC (flagged option).
 // The planner picks the lowest level a run needs; particles per thread, block size and register cap per level below.
 // Level 0: 6 particles per thread, one block of 384 threads per SM (152 registers): a register-only loop of 80
-// matrices runs at 61.5 DFMA/clk/SM = 96 % of the pipe (50.0 with shared-memory coefficients; profiles/r02_long.md).
+// matrices ran at 61.5 DFMA/clk/SM = 96 % of the pipe in a microbenchmark (50.0 with shared-memory coefficients); the
+// kernel as it is: fp64 pipe 96.2 % active in ncu (profiles/r02f_final_round2.md, capture G).
 // The next tile is prefetched into shared memory with cp.async while the current one is in the pipe, every thread
 // copying exactly the 16-byte chunks it will read itself (no block-wide barrier in the tile loop).
 // Same arithmetic, in the same order, as chain_kernel.
@@ -989,7 +990,7 @@ __global__ void __maxnreg__(LongCfg<LEVEL>::REGS) chain_long_kernel(const __grid
 //       slots t + m NT of that stage to dst[base + slot]: dense 256-byte warp stores; slots past the survivors
 //       go to the lost log at n_lost + (index - survivors before); then the stage is released.
 // Measured variants (tile sizes, ring depths, per-thread cp.async instead of bulk copies, round 1's
-// register-held tile): profiles/r02_compact.md.
+// register-held tile of round 1): profiles/r02_compact.md.
 // ---------------------------------------------------------------------------------------------------
 #ifndef ELG_C2_NT
 #define ELG_C2_NT 256
@@ -1511,7 +1512,7 @@ __global__ void __launch_bounds__(kBlock, 6) hist_kernel(const HistArgs a) {
 // PLANES of 32-bit words (count | low and high words of the four 64-bit sums): the word of bin b in a plane sits in
 // bank b mod 32, so the 32 lanes of an atomic spread over all banks (round 1 kept the four 64-bit sums of a bin side by
 // side: every atomic of a warp fell into 4 of the 32 banks, 85 % of the shared-memory wavefront peak, 0.74 ms per
-// 1e8 particles; profiles/r02_dipole.md).  The split point 2^36 (round 1: 2^32) leaves both integers of a
+// 1e8 particles; profiles/r02c_dipole.md).  The split point 2^36 (round 1: 2^32) leaves both integers of a
 // millimetre-sized offset below 2^28, so the low word of a sum rarely wraps and an add is ONE native 32-bit atomic
 // (the carry into the high word follows in 1-3 % of the adds): 5.1 shared atomics per particle instead of 9.
 // ---------------------------------------------------------------------------------------------------
