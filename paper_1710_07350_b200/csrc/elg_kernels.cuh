@@ -744,9 +744,9 @@ __global__ void __launch_bounds__(kBlock, ((P >= 4 || MOM) ? 2 : 3)) chain_kerne
 // (LDCU.64 UR, c[0x0][UR+imm]; DFMA R, R, UR, R).  A DFMA takes one uniform operand, so the row constant C[r] is made
 // a vector value once per row (matrix_map_uniform); with two uniform operands in the first term ptxas falls back to
 // per-thread LDC for everything.  tests/test_abi.py checks the SASS for the uniform form.
-// LEVEL 0: MATRIX, DRIFT, RFKICK, KICK; 1: + MATRIX2, TKICK; 2: + MATRIX3; 3: level 0 + MATRIX_UNC (flagged option).
+// LEVEL 0: MATRIX, DRIFT, RFKICK, KICK; 1: + MATRIX2, TKICK, KICK3; 2: + MATRIX3; 3: level 0 + MATRIX_UNC (flagged option).
 // The planner picks the lowest level a run needs; particles per thread, block size and register cap per level below.
-// Level 0: 6 particles per thread, one block of 384 threads per SM (152 registers): a register-only loop of 80
+// Level 0: 6 particles per thread, one block of 384 threads per SM (168 registers): a register-only loop of 80
 // matrices ran at 61.5 DFMA/clk/SM = 96 % of the pipe in a microbenchmark (50.0 with shared-memory coefficients); the
 // kernel as it is: fp64 pipe 96.2 % active in ncu (profiles/r02f_final_round2.md, capture G).
 // The next tile is prefetched into shared memory with cp.async while the current one is in the pipe, every thread
