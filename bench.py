@@ -640,7 +640,7 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="particles per GPU (default: the workload's own count)")
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="particles of the oracle's bounded sample")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--e2e-chunks", type=int, default=16, help="particle ranges of the pipelined upload (1: no overlap)")
+    ap.add_argument("--e2e-chunks", type=int, default=32, help="particle ranges of the pipelined upload (1: no overlap)")
     ap.add_argument("--probe-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

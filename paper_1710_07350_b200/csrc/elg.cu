@@ -1221,7 +1221,7 @@ extern "C" int32_t elg_upload_and_track(elg_bunch* b, const elg_beamline* bl, co
         ELG_CK(cudaStreamCreateWithFlags(&b->copy_stream, cudaStreamNonBlocking));
         ELG_CK(cudaEventCreateWithFlags(&b->entry_ev, cudaEventDisableTiming));
     }
-    if (n_chunks > 24) n_chunks = 24;                               // min/max partial slots (kMmPartials)
+    if (n_chunks > 32) n_chunks = 32;                               // min/max partial slots: 32 chunks x 444 blocks <= kMmPartials
     while ((int)b->chunk_ev.size() < n_chunks) {
         cudaEvent_t e = nullptr;
         ELG_CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
