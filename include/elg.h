@@ -182,11 +182,15 @@ int32_t elg_bunch_upload(elg_bunch*, const double* const h_coords[6], const int6
 /* The caller has rewritten d_soa with n0 fresh particles: n_alive = n0, turn = 0, lost log empty. */
 int32_t elg_bunch_rewind(elg_bunch*);
 
-/* Track n_turns passes through the beamline.  opts nullable. */
+/* Track n_turns passes through the beamline.  opts nullable.  Asynchronous on the bunch's stream unless
+ * opts asks for host outputs.  Every kernel is launched with the programmatic-stream-serialization attribute and begins
+ * with griddepcontrol.wait, so the order is the stream's.  Environment switches for A/B measurements (read once per
+ * process; the defaults are the measured best): ELG_PDL=0 (plain launches), ELG_CHAIN_RING=0 (short DRIFT / MATRIX runs
+ * through chain_kernel instead of the bulk-copy ring), ELG_HIST_AGGREGATE=1, ELG_CHAIN_P=2|4. */
 int32_t elg_track(elg_bunch*, const elg_beamline*, int64_t n_turns, elg_track_opts* opts);
 
 /* elg_bunch_upload followed by elg_track in ONE call with the upload pipelined against the tracking: the bunch is
- * cut into n_chunks particle ranges (n_chunks <= 1: no pipelining); each range is copied from the HOST arrays on a
+ * cut into n_chunks particle ranges (n_chunks <= 1: no pipelining; at most 32 are used); each range is copied from the HOST arrays on a
  * copy stream owned by the bunch and, as soon as it has landed, the leading per-particle maps of the first turn
  * (everything in front of the first WAKE / HISTO / TRWAKE, aperture, bunch-fiducial RFKICK or per-element record)
  * run on that range while the following ranges are still being copied.  Results are identical to
