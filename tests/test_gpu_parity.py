@@ -832,3 +832,42 @@ def test_launch_switches_change_no_bit(elg):
         digests[tag] = out.stdout.strip().splitlines()[-1]
     assert len(digests["default"]) == 64
     assert digests["no-pdl"] == digests["default"] and digests["no-ring"] == digests["default"], digests
+
+
+# ------------------------------------------------------------------------------------ the roofline's numerator
+@pytest.mark.gpu
+def test_work_accounting_matches_the_algorithmic_counts(elg):
+    """bench.py's roofline divides the ALGORITHMIC bytes / flops the launches report (elg_profile_read) by their device
+    time.  The reported work must be DESIGN.md section 5's per-particle figures times the live particles of each launch:
+    96 B and 11 + 72 flops for DRIFT + MATRIX, 112 B for a compacting run (live count BEFORE the aperture), 8 B per
+    histogram, 24 B for a wake kick (+ the record's coordinates), 72 flops per matrix of a long run."""
+    n = 100_003
+    # p1: DRIFT + MATRIX, one launch
+    w = make_workload("p1-chain", n=n)
+    bl = elg.Beamline(w.elements); b = elg.Bunch(w.particles(), w.p0c_eV, w.charge_C, beamline=bl)
+    b.profile(True); b.profile_read()
+    b.track(bl, 1, moments_every="none", records=False)
+    p = b.profile_read(work=True)
+    assert p["chain"][0] == 1 and p["chain"][2] == 96.0 * n and p["chain"][3] == (11 + 72) * float(n)
+    assert sum(v[0] for k, v in p.items() if k != "chain") == 0
+    # cfg0 with the turn record: compacting run (112 B x n0), histogram (8 B x survivors), kick + record (56 B x survivors)
+    w = make_workload("cfg0", n=n)
+    bl = elg.Beamline(w.elements); b = elg.Bunch(w.particles(), w.p0c_eV, w.charge_C, beamline=bl, lost_capacity=n)
+    b.profile(True); b.profile_read()
+    b.track(bl, 1, moments_every="turn", records=False)
+    p = b.profile_read(work=True)
+    alive = b.n_alive
+    assert 0 < alive < n
+    assert p["chain_compact"][0] == 1 and p["chain_compact"][2] == 112.0 * n and p["chain_compact"][3] == (11 + 72) * float(n)
+    assert p["hist"][0] == 1 and p["hist"][2] == 8.0 * alive
+    assert p["chain"][0] == 1 and p["chain"][2] == 56.0 * alive and p["chain"][3] == (10 + 60) * float(alive)
+    assert p["moments"][0] == 0                                        # the record rode in the kick run's epilogue
+    # cfg3, one turn: 200 matrices + RF kick in three long-run launches
+    w = make_workload("cfg3", n=n, n_turns=1)
+    bl = elg.Beamline(w.elements, ring=True); b = elg.Bunch(w.particles(), w.p0c_eV, w.charge_C, beamline=bl)
+    b.profile(True); b.profile_read()
+    b.track(bl, 1, moments_every="turn", records=False)
+    p = b.profile_read(work=True)
+    assert p["chain_long"][0] == 3 and p["chain_long"][2] == 3 * 96.0 * n and p["chain_long"][3] == (200 * 72 + 6) * float(n)
+    assert p["chain"][0] == 1 and p["chain"][2] == 56.0 * n
+    b.profile(False)
