@@ -450,38 +450,54 @@ def line_passes(gb, w):
 def run_other_configs(elg, stream, dev, steps=10, warmup=3):
     """BASELINE.json's configs 0, 1, 2 and 4 at their own sizes (1e5 ... 1e7 particles: launch-latency-sized and
     largely L2-resident): one step = the whole job of the config (cfg2: its 10 passes), median of `steps`
-    CUDA-event timings, inputs resident.  Parity at these sizes: tests/test_gpu_parity.py, tests/test_gpu_fullsize.py."""
+    CUDA-event timings, inputs resident, fresh particles restored before every step (not timed).  `ms_per_step`: the
+    elg_track call as a user makes it; `graph_ms_per_step`: the same call captured once into a CUDA graph (elg.h, "CUDA
+    graphs") and replayed.  Parity at these sizes: tests/test_gpu_parity.py, tests/test_gpu_fullsize.py."""
     import torch
     from elg_inputs import make_workload
     out = {}
+    side = torch.cuda.Stream(device=dev)                             # (a capture needs a stream of its own)
     for name in ("cfg0", "cfg1", "cfg2", "cfg4"):
         w = make_workload(name)
         n0 = w.n0
         hp = torch.empty((6, n0), dtype=torch.float64, pin_memory=True)
         w.particles(n0, out=hp.numpy())
-        gb = elg.Bunch(None, w.p0c_eV, w.charge_C, beamline=None, n0=n0, device=str(dev), lost_capacity=n0)
-        bl = elg.Beamline(w.elements, ring=w.ring)
-        gb.upload(hp); gb.synchronize()
-        keep = gb.soa.clone()
-        times = []
-        launches = 0
-        for rep in range(warmup + steps):
-            gb.soa.copy_(keep); gb.rewind(); gb.synchronize()
-            l0 = elg.launch_count()
-            ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
-            ev0.record(stream)
-            gb.track(bl, w.n_turns, moments_every=w.moments_every, records=False)
-            ev1.record(stream)
-            torch.cuda.synchronize(dev)
-            launches = elg.launch_count() - l0
-            if rep >= warmup:
-                times.append(ev0.elapsed_time(ev1))
-        ms = float(np.median(times))
-        passes = line_passes(gb, w) if not w.ring else float(n0) * w.n_pass_elements * w.n_turns
+        with torch.cuda.stream(side):
+            gb = elg.Bunch(None, w.p0c_eV, w.charge_C, beamline=None, n0=n0, device=str(dev), lost_capacity=n0, stream=side)
+            bl = elg.Beamline(w.elements, ring=w.ring)
+            gb.upload(hp); gb.synchronize()
+            keep = gb.soa.clone()
+            times = []
+            launches = 0
+            for rep in range(warmup + steps):
+                gb.soa.copy_(keep); gb.rewind(); gb.synchronize()
+                l0 = elg.launch_count()
+                ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+                ev0.record(side)
+                gb.track(bl, w.n_turns, moments_every=w.moments_every, records=False)
+                ev1.record(side)
+                side.synchronize()
+                launches = elg.launch_count() - l0
+                if rep >= warmup:
+                    times.append(ev0.elapsed_time(ev1))
+            ms = float(np.median(times))
+            passes = line_passes(gb, w) if not w.ring else float(n0) * w.n_pass_elements * w.n_turns
+            n_alive = int(gb.n_alive)
+            graph = gb.capture_track(bl, w.n_turns, moments_every=w.moments_every)     # [rewind, track]
+            gtimes = []
+            for rep in range(warmup + steps):
+                gb.soa.copy_(keep); gb.synchronize()
+                ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+                ev0.record(side); graph.replay(); ev1.record(side)
+                side.synchronize()
+                if rep >= warmup:
+                    gtimes.append(ev0.elapsed_time(ev1))
+            assert int(gb.n_alive) == n_alive
         out[name] = {"particles": n0, "elements_per_pass": w.n_pass_elements, "passes_per_step": w.n_turns,
                      "moments_every": w.moments_every, "ms_per_step": ms, "launches_per_step": int(launches),
-                     "value": passes / (ms * 1e-3) / 1e6, "unit": UNIT, "n_alive_after": int(gb.n_alive)}
-        del gb, keep, hp
+                     "graph_ms_per_step": float(np.median(gtimes)),
+                     "value": passes / (ms * 1e-3) / 1e6, "unit": UNIT, "n_alive_after": n_alive}
+        del graph, gb, keep, hp
     return out
 
 

@@ -189,6 +189,19 @@ int32_t elg_bunch_rewind(elg_bunch*);
  * through chain_kernel instead of the bulk-copy ring), ELG_HIST_AGGREGATE=1, ELG_CHAIN_P=2|4. */
 int32_t elg_track(elg_bunch*, const elg_beamline*, int64_t n_turns, elg_track_opts* opts);
 
+/* CUDA graphs.  elg_track (and elg_bunch_rewind) may be CAPTURED by the caller (cudaStreamBeginCapture on the bunch's
+ * stream; the stream must not be the legacy default stream) when opts asks for no host output, profiling is off and
+ * the beamline has been tracked once before (wake tables are uploaded on first use): nothing in the call synchronises
+ * or reads the device; inside a capture elg_track clears the compaction's tile status and restarts its epoch first.
+ * A replay repeats the captured launches with the parameters of the capture (buffers, turn numbers, RF phase
+ * references, record slots), so it is valid whenever the bunch is in the state the capture started from -- normally the
+ * capture begins with the caller's copy of fresh particles into d_soa and elg_bunch_rewind.  The library's HOST mirror of
+ * the device state (current store, count slot, epoch, turn, records in the device ring) is advanced by the capture, not
+ * by a replay: save it after the capture and restore it after every replay before calling anything else on the bunch.
+ * Records of a captured run stay in the device ring (the host copy needs opts->records, which cannot be captured). */
+int32_t elg_bunch_host_state_save(const elg_bunch*, int64_t state[8]);
+int32_t elg_bunch_host_state_restore(elg_bunch*, const int64_t state[8]);
+
 /* elg_bunch_upload followed by elg_track in ONE call with the upload pipelined against the tracking: the bunch is
  * cut into n_chunks particle ranges (n_chunks <= 1: no pipelining; at most 32 are used); each range is copied from the HOST arrays on a
  * copy stream owned by the bunch and, as soon as it has landed, the leading per-particle maps of the first turn

@@ -1185,6 +1185,24 @@ extern "C" int64_t elg_beamline_launches_per_turn(const elg_beamline* bl, int32_
 extern "C" int32_t elg_track(elg_bunch* b, const elg_beamline* bl, int64_t n_turns, elg_track_opts* o) {
     if (!b || !bl || n_turns < 0) return fail(ELG_EINVAL, "elg_track: bad arguments");
     if (o) { o->n_records = 0; o->hist_written = 0; o->V_written = 0; o->window_written = 0; }
+    // The caller may CAPTURE this call into a CUDA graph (cudaStreamBeginCapture on the bunch's stream): nothing in it
+    // synchronises or reads the device when no host output is asked for.  A replay repeats the launches with the
+    // parameters of the capture, so it is valid from the bunch state the capture started from (typically a captured
+    // copy of the particles + elg_bunch_rewind in front of it).  The compaction's tile status is cleared at the head of
+    // the captured work and its epoch restarted, so that the words of an earlier replay never look current.
+    {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        ELG_CK(cudaStreamIsCapturing(b->stream, &cs));
+        if (cs != cudaStreamCaptureStatusNone) {
+            if (o && (o->records || o->hist_out || o->V_out || o->window_out))
+                return fail(ELG_ESTATE, "elg_track: host outputs cannot be captured into a CUDA graph");
+            if (b->prof_on) return fail(ELG_ESTATE, "elg_track: per-kernel profiling cannot be captured into a CUDA graph");
+            if (b->table_serial != bl->serial && bl->table_total > 0)
+                return fail(ELG_ESTATE, "elg_track: run this beamline once before capturing it (wake tables are uploaded on first use)");
+            ELG_CK(cudaMemsetAsync(b->tile_status, 0, (b->stride / kStatusTile + 2) * 8, b->stream));
+            b->epoch = 0;
+        }
+    }
     { int32_t rc = upload_tables(b, bl); if (rc != ELG_OK) return rc; }
     Tracker t{b, bl, o};
     b->rec_count = 0;
@@ -1264,6 +1282,24 @@ extern "C" int32_t elg_upload_and_track(elg_bunch* b, const elg_beamline* bl, co
         if (e != cudaSuccess) return fail(ELG_ECUDA, std::string("cudaStreamSynchronize: ") + cudaGetErrorString(e));
     }
     return t.rc;
+}
+
+// ------------------------------------------------------------------------------------- CUDA-graph support
+// The host keeps a mirror of what it needs to know about the device state without ever reading it (which store holds
+// the live particles, which count slot is current, the compaction epoch, the turn number, the records in the device
+// ring).  A graph replay advances the device exactly as the captured call did but not this mirror: the caller saves
+// it after the capture and puts it back after every replay.
+extern "C" int32_t elg_bunch_host_state_save(const elg_bunch* b, int64_t out[8]) {
+    if (!b || !out) return fail(ELG_EINVAL, "elg_bunch_host_state_save: bad arguments");
+    out[0] = b->cur_buf; out[1] = b->cur_slot; out[2] = (int64_t)b->epoch; out[3] = b->turn; out[4] = b->rec_count;
+    out[5] = 0; out[6] = 0; out[7] = 0x656c67;                    // tag
+    return ELG_OK;
+}
+extern "C" int32_t elg_bunch_host_state_restore(elg_bunch* b, const int64_t in[8]) {
+    if (!b || !in || in[7] != 0x656c67 || (in[0] | 1) != 1 || (in[1] | 1) != 1 || in[2] < 0 || in[2] > 0x3fffffff || in[4] < 0 || in[4] > kRecCap)
+        return fail(ELG_EINVAL, "elg_bunch_host_state_restore: not a state written by elg_bunch_host_state_save");
+    b->cur_buf = (int)in[0]; b->cur_slot = (int)in[1]; b->epoch = (unsigned int)in[2]; b->turn = in[3]; b->rec_count = in[4];
+    return ELG_OK;
 }
 
 // ------------------------------------------------------------------------------------- host readbacks

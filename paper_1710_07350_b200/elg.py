@@ -31,7 +31,7 @@ EXPORTS = (
     "elg_beamline_load", "elg_beamline_destroy", "elg_beamline_n_elements", "elg_beamline_length",
     "elg_beamline_s_design", "elg_beamline_launches_per_turn", "elg_workspace_bytes",
     "elg_bunch_create", "elg_bunch_destroy", "elg_bunch_upload", "elg_bunch_rewind", "elg_track",
-    "elg_upload_and_track",
+    "elg_upload_and_track", "elg_bunch_host_state_save", "elg_bunch_host_state_restore",
     "elg_moments", "elg_lost", "elg_n_alive", "elg_bunch_read", "elg_bunch_device_array",
     "elg_profile_enable", "elg_profile_read",
     "elg_dbg_histogram", "elg_dbg_dipole_histogram", "elg_dbg_kick", "elg_dbg_tkick", "elg_dbg_compact",
@@ -107,6 +107,8 @@ def lib():
     L.elg_bunch_upload.argtypes = [vp, v6, _i64p]; L.elg_bunch_upload.restype = C.c_int32
     L.elg_bunch_rewind.argtypes = [vp]; L.elg_bunch_rewind.restype = C.c_int32
     L.elg_track.argtypes = [vp, vp, C.c_int64, C.POINTER(TrackOpts)]; L.elg_track.restype = C.c_int32
+    L.elg_bunch_host_state_save.argtypes = [vp, C.POINTER(C.c_int64)]; L.elg_bunch_host_state_save.restype = C.c_int32
+    L.elg_bunch_host_state_restore.argtypes = [vp, C.POINTER(C.c_int64)]; L.elg_bunch_host_state_restore.restype = C.c_int32
     L.elg_upload_and_track.argtypes = [vp, vp, v6, _i64p, C.c_int64, C.POINTER(TrackOpts), C.c_int32]
     L.elg_upload_and_track.restype = C.c_int32
     L.elg_moments.argtypes = [vp, _i64p, _dp, _dp]; L.elg_moments.restype = C.c_int32
@@ -355,6 +357,13 @@ class Bunch:
         _ck(lib().elg_track(self._h, bl._h, n_turns, C.byref(o)))
         return self._outputs(o, rec, hist, V, win, want_stage_outputs)
 
+    def capture_track(self, bl: Beamline, n_turns: int = 1, moments_every: str = "none", prologue=None) -> "TrackGraph":
+        """Capture [prologue(), elg_bunch_rewind, elg_track] into a CUDA graph on the bunch's stream (which must not be the
+        default stream) and return it; .replay() launches the graph and puts the host mirror of the device state back to
+        what it was after the capture (include/elg.h, "CUDA graphs").  prologue: e.g. the copy of fresh particles into
+        bunch.soa.  The beamline must have been tracked once before (wake tables)."""
+        return TrackGraph(self, bl, n_turns, moments_every, prologue)
+
     def upload_and_track(self, coords, bl: Beamline, n_turns: int = 1, moments_every: str = "none",
                          want_stage_outputs: bool = False, records: bool = True, n_chunks: int = 8, ids=None):
         """elg_upload_and_track: upload from host memory pipelined against the first turn's leading maps."""
@@ -434,6 +443,29 @@ class Bunch:
                 t = base[off // 8: off // 8 + self.stride]
                 return t.view(torch.int64) if c == 6 else t
         raise ElgError(ESTATE, "device array outside the lent buffers")
+
+
+class TrackGraph:
+    """A captured [prologue, rewind, track] (Bunch.capture_track).  Argument marshalling and torch.cuda.CUDAGraph only."""
+
+    def __init__(self, bunch: Bunch, bl: Beamline, n_turns: int, moments_every: str, prologue):
+        torch = _torch()
+        self.bunch = bunch
+        self.graph = torch.cuda.CUDAGraph()
+        o = TrackOpts()
+        o.moments_every = MOM[moments_every]
+        o.flags = 1 if getattr(bunch, "sparse_matrices", False) else 0
+        with torch.cuda.graph(self.graph, stream=bunch._stream):
+            if prologue is not None:
+                prologue()
+            _ck(lib().elg_bunch_rewind(bunch._h))
+            _ck(lib().elg_track(bunch._h, bl._h, n_turns, C.byref(o)))
+        self.state = (C.c_int64 * 8)()
+        _ck(lib().elg_bunch_host_state_save(bunch._h, self.state))
+
+    def replay(self) -> None:
+        self.graph.replay()
+        _ck(lib().elg_bunch_host_state_restore(self.bunch._h, self.state))
 
 
 # ------------------------------------------------------------------------------- single-stage hooks

@@ -871,3 +871,41 @@ def test_work_accounting_matches_the_algorithmic_counts(elg):
     assert p["chain_long"][0] == 3 and p["chain_long"][2] == 3 * 96.0 * n and p["chain_long"][3] == (200 * 72 + 6) * float(n)
     assert p["chain"][0] == 1 and p["chain"][2] == 56.0 * n
     b.profile(False)
+
+
+# ------------------------------------------------------------------------------------ CUDA-graph replay of elg_track
+@pytest.mark.gpu
+@pytest.mark.parametrize("name,n,turns", [("cfg0", 100_000, 1), ("cfg4", 200_003, 1), ("cfg1", 150_001, 1), ("p6-rfcw", 120_007, 1),
+                                         ("cfg2", 150_000, 3), ("cfg3", 30_011, 2)])
+def test_cuda_graph_replay_equals_direct_tracking(elg, name, n, turns):
+    """[copy of fresh particles, rewind, elg_track] captured into a CUDA graph on the bunch's own stream (cooperative
+    compaction launches and the programmatic-dependent-launch attribute included) and replayed three times gives, bit
+    for bit, the coordinates, IDs, lost log and moments of a direct call -- whatever the parity of the compactions
+    (the host mirror of the device state is restored after each replay, include/elg.h "CUDA graphs")."""
+    import torch
+    kw = {"n_turns": turns} if name == "cfg3" else {}
+    w = make_workload(name, n=n, **kw)
+    v0 = w.particles()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        bl = elg.Beamline(w.elements, ring=w.ring)
+        b = elg.Bunch(v0, w.p0c_eV, w.charge_C, beamline=bl, lost_capacity=n, stream=s)
+        keep = b.soa.clone()
+        b.track(bl, turns, moments_every=w.moments_every, records=False)      # direct (also uploads the wake tables)
+        rv, rid = b.read(); rlost = b.lost(); rmom = b.moments() if rv.shape[1] else None
+        g = b.capture_track(bl, turns, moments_every=w.moments_every, prologue=lambda: b.soa.copy_(keep))
+        for rep in range(3):
+            if rep == 1:
+                b.rewind()                                            # host state knocked out of step on purpose
+            g.replay()
+            gv, gid = b.read(); glost = b.lost()
+            assert np.array_equal(gid, rid) and np.array_equal(gv, rv)
+            for x, y in zip(glost, rlost):
+                assert np.array_equal(x, y)
+            if rmom is not None:
+                gm = b.moments()
+                assert gm[0] == rmom[0] and np.array_equal(gm[1], rmom[1]) and np.array_equal(gm[2], rmom[2])
+        # a direct call afterwards continues from the replayed state like from a direct one
+        b.soa.copy_(keep); b.rewind()
+        b.track(bl, turns, moments_every=w.moments_every, records=False)
+        assert np.array_equal(b.read()[0], rv)
