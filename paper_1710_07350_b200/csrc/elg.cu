@@ -269,7 +269,7 @@ int32_t hist_setup_once() {
 }  // namespace
 
 // =====================================================================================================
-extern "C" const char* elg_version(void) { return "elg 0.1 (sm_100a)"; }
+extern "C" const char* elg_version(void) { return "elg 0.2 (sm_100a)"; }
 extern "C" const char* elg_last_error(void) { return g_err.c_str(); }
 extern "C" int64_t elg_launch_count(void) { return g_launches.load(); }
 extern "C" int64_t elg_soa_stride(int64_t n0) { return n0 <= 0 ? 32 : align_up(n0, 32); }
