@@ -228,14 +228,15 @@ __device__ __forceinline__ int bin_of(double s, double inv_bc, double t_lo, doub
     const double t = s * inv_bc;
     const double u = (t - t_lo) * inv_dt;
     *u_out = u;
-    if (!(u >= 0.0) || !(u < (double)nb)) return -1;
+    const bool in_range = (u >= 0.0) && (u < (double)nb);        // NaN: false
 #if !ELG_BIN_MAGIC
-    return (int)floor(u);
+    return in_range ? (int)floor(u) : -1;
 #endif
     constexpr double kMagic = 6755399441055744.0;                // 1.5 x 2^52
-    const double m = u + kMagic;
+    const double m = u + kMagic;                                 // (evaluated for every u, used only in range: no branch)
     const double r = m - kMagic;
-    return __double2loint(m) - ((r > u) ? 1 : 0);
+    const int k = __double2loint(m) - ((r > u) ? 1 : 0);
+    return in_range ? k : -1;
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -1473,6 +1474,30 @@ __global__ void __launch_bounds__(kBlock, 6) hist_kernel(const HistArgs a) {
                 if (have[2 * k + 1]) { const double2 t = ld_stream2(a.s + i); sv[2 * k] = t.x; sv[2 * k + 1] = t.y; }
                 else if (have[2 * k]) sv[2 * k] = ld_stream1(a.s + i);
             }
+        }
+        if constexpr (!AGG) {
+            // branch-free common path: one predicated shared-memory reduction per particle (the kernel is bound by
+            // instruction issue, not by memory: 8 bytes per particle); bins outside the privatised range are rare and
+            // take the global atomics in a second pass over the registers
+            const unsigned int mine32 = smem_u32(mine);
+            int bb[kPer];
+            bool fallback = false;
+#pragma unroll
+            for (int p = 0; p < kPer; p++) {
+                double u;
+                const int b = bin_of(sv[p], a.inv_bc, t_lo, inv_dt, a.nb, &u);
+                bb[p] = have[p] ? b : -1;
+                const unsigned int rel = (unsigned int)(bb[p] - lo32);       // (wraps past S when b < bin_lo or b = -1)
+                const bool in_s = bb[p] >= 0 && rel < (unsigned int)S;
+                asm volatile("{\n.reg .pred q;\nsetp.ne.s32 q, %1, 0;\n@q red.shared.add.u32 [%0], 1;\n}" ::"r"(mine32 + rel * 4u), "r"((int)in_s) : "memory");
+                fallback |= bb[p] >= 0 && !in_s;
+            }
+            if (fallback) {
+#pragma unroll
+                for (int p = 0; p < kPer; p++)
+                    if (bb[p] >= 0 && (unsigned int)(bb[p] - lo32) >= (unsigned int)S) atomicAdd(a.counts + bb[p], 1u);
+            }
+            continue;
         }
 #pragma unroll
         for (int p = 0; p < kPer; p++) {
