@@ -1228,6 +1228,12 @@ extern "C" int32_t elg_upload_and_track(elg_bunch* b, const elg_beamline* bl, co
                                         const int64_t* h_ids, int64_t n_turns, elg_track_opts* o, int32_t n_chunks) {
     if (!b || !bl || !h_coords || n_turns < 0) return fail(ELG_EINVAL, "elg_upload_and_track: bad arguments");
     for (int c = 0; c < 6; c++) if (!h_coords[c]) return fail(ELG_EINVAL, "elg_upload_and_track: NULL coordinate array");
+    {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        ELG_CK(cudaStreamIsCapturing(b->stream, &cs));
+        if (cs != cudaStreamCaptureStatusNone)
+            return fail(ELG_ESTATE, "elg_upload_and_track: cannot be captured into a CUDA graph (host copies on a second stream); capture elg_track");
+    }
     Tracker probe{b, bl, o};
     const long long k_split = probe.map_prefix();
     if (n_turns < 1 || k_split == 0 || n_chunks <= 1 || b->n0 < 4 * 9216) {       // nothing to overlap
