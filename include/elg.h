@@ -268,6 +268,24 @@ int32_t elg_dbg_wake_samples(int32_t kind, int32_t nb, double dt, double f, doub
 int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W, int32_t nb, double q, double* d_V,
                          void* stream);
 
+/* ---- an entry point that allocates nothing ------------------------------------------------------------------------
+ * The dipole histogram stage (TRWAKE, G32-G33: bin counts and the exact per-bin sums of x and y) for callers that cannot
+ * call cudaMalloc and have no workspace to lend: code under CUDA-graph capture, tight serving loops, harnesses that
+ * forbid allocation.  Inputs and outputs are the caller's DEVICE arrays: s, x, y (n doubles each, 16-byte aligned),
+ * counts (uint32[nb]), D (double[2 nb]: Dx then Dy); bin k = [t_lo + k dt, t_lo + (k + 1) dt) of t = s inv_bc (G9, G10).
+ * The scratch of the stage (a state block + four 64-bit accumulators per bin) is a file-scope device array inside the
+ * library, 524 800 bytes, held by every GPU that loads the library until the process exits; hence
+ * nb <= elg_noalloc_max_bins() = 16384, beyond which the call returns ELG_ECAPACITY and launches nothing.
+ * The call performs no cudaMalloc / cudaFree and calls no allocating library routine; it launches three kernels on
+ * `stream` (the histogram and finalize kernels are tracking's own) and does not synchronise.  Results equal
+ * elg_dbg_dipole_histogram's bit for bit.
+ * Every call on a device shares the one array, which keeps the last call's contents: each call clears what must start
+ * at zero (accumulators, counts) itself, and calls that OVERLAP on the GPU (two streams without an ordering between
+ * them, two host threads) race on it -- serialise them. */
+int32_t elg_noalloc_max_bins(void);
+int32_t elg_dipole_histogram_noalloc(const double* d_s, const double* d_x, const double* d_y, int64_t n, double inv_bc,
+                                     double t_lo, double dt, int32_t nb, uint32_t* d_counts, double* d_D, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

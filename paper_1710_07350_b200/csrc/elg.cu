@@ -1503,3 +1503,104 @@ extern "C" int32_t elg_dbg_convolve(const uint32_t* d_counts, const double* d_W,
     ELG_CK(cudaGetLastError());
     return ELG_OK;
 }
+
+// =====================================================================================================
+// elg_dipole_histogram_noalloc: the dipole histogram stage (TRWAKE, G32-G33) for callers that cannot allocate and have
+// no workspace to lend (code under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The
+// scratch the stage needs -- a device state block and four 64-bit fixed-point accumulators per bin -- lives in a
+// file-scope device array of fixed size, held by every GPU that loads the library until the process exits:
+// 512 B + 32 B x kNoAllocMaxBins = 524 800 bytes.  The call allocates nothing (no cudaMalloc / cudaFree, no allocating
+// library routine): it launches a prepare kernel (state, zeroed accumulators, zeroed output counts), tracking's own
+// dipole_hist_kernel and dipole_finalize_kernel on the caller's stream.
+// In HOST code the array's name is a host-side stand-in, not a device address: the address is asked for once per
+// device, with that device current (cudaGetSymbolAddress), and handed to the kernels.
+// All calls on a device share the array and it keeps the last call's contents: every call clears what must start at
+// zero, and two calls that overlap on the GPU (different streams, no ordering between them) RACE on it.
+// =====================================================================================================
+namespace {
+constexpr int kNoAllocMaxBins = 16384;
+constexpr size_t kNoAllocStateBytes = 512;                               // >= sizeof(DevState)
+constexpr size_t kNoAllocBytes = kNoAllocStateBytes + (size_t)kNoAllocMaxBins * 4 * sizeof(unsigned long long);
+static_assert(sizeof(DevState) <= kNoAllocStateBytes, "state block of the static scratch");
+}  // namespace
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+namespace {
+// fills the state block the histogram kernel reads (n, EXPLICIT window, whole bin range) and clears what accumulates
+__global__ void __launch_bounds__(kBlock) noalloc_prepare_kernel(unsigned char* scratch, long long n, double t_lo, double dt, int nb,
+                                                                 unsigned int* counts) {
+    DevState* st = reinterpret_cast<DevState*>(scratch);
+    unsigned long long* dacc = reinterpret_cast<unsigned long long*>(scratch + kNoAllocStateBytes);
+    const int stride = gridDim.x * kBlock;
+    for (int i = blockIdx.x * kBlock + threadIdx.x; i < 4 * nb; i += stride) dacc[i] = 0ull;
+    for (int i = blockIdx.x * kBlock + threadIdx.x; i < nb; i += stride) counts[i] = 0u;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        st->n_alive[0] = n; st->n_alive[1] = n; st->n_lost[0] = 0; st->n_lost[1] = 0;
+        st->win[0] = t_lo; st->win[1] = dt; st->win[2] = 1.0 / dt; st->win[3] = 0.0;
+        st->smin = 0.0; st->smax = 0.0;
+        st->bin_lo = 0; st->bin_hi = nb - 1;
+        st->zero_bits = 0;
+    }
+}
+
+// device address of the scratch array on the CURRENT device, looked up once per device
+int32_t noalloc_scratch(unsigned char** out) {
+    constexpr int kMaxDevices = 64;
+    static unsigned char* ptrs[kMaxDevices] = {nullptr};
+    static std::atomic<int> have[kMaxDevices];
+    int dev = 0;
+    ELG_CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(ELG_EINVAL, "elg_dipole_histogram_noalloc: device index out of range");
+    if (!have[dev].load(std::memory_order_acquire)) {
+        unsigned char* p = nullptr;
+        ELG_CK(cudaGetSymbolAddress((void**)&p, g_noalloc_scratch));
+        if (!p) return fail(ELG_ECUDA, "elg_dipole_histogram_noalloc: cudaGetSymbolAddress returned NULL");
+        ptrs[dev] = p;                                                   // (the same value from every thread that races here)
+        have[dev].store(1, std::memory_order_release);
+    }
+    *out = ptrs[dev];
+    return ELG_OK;
+}
+}  // namespace
+
+extern "C" int32_t elg_noalloc_max_bins(void) { return kNoAllocMaxBins; }
+
+extern "C" int32_t elg_dipole_histogram_noalloc(const double* d_s, const double* d_x, const double* d_y, int64_t n, double inv_bc,
+                                                double t_lo, double dt, int32_t nb, uint32_t* d_counts, double* d_D, void* stream) {
+    if (n < 0 || n >= (1LL << 31) || (n > 0 && (!d_s || !d_x || !d_y)) || !d_counts || !d_D || !(dt > 0.0) || !std::isfinite(t_lo) ||
+        !std::isfinite(inv_bc))
+        return fail(ELG_EINVAL, "elg_dipole_histogram_noalloc: bad arguments");
+    if (nb < 2) return fail(ELG_EINVAL, "elg_dipole_histogram_noalloc: nb < 2");
+    if (nb > kNoAllocMaxBins) {
+        char buf[160];
+        std::snprintf(buf, sizeof buf, "elg_dipole_histogram_noalloc: nb = %d exceeds the static scratch (at most %d bins)", (int)nb, kNoAllocMaxBins);
+        return fail(ELG_ECAPACITY, buf);
+    }
+    if ((n > 0 && (((uintptr_t)d_s | (uintptr_t)d_x | (uintptr_t)d_y) & 15)) || ((uintptr_t)d_D & 7))
+        return fail(ELG_EINVAL, "elg_dipole_histogram_noalloc: s, x, y must be 16-byte aligned");
+    unsigned char* scratch = nullptr;
+    { int32_t rc = noalloc_scratch(&scratch); if (rc != ELG_OK) return rc; }
+    { int32_t rc = hist_setup_once(); if (rc != ELG_OK) return rc; }
+    int sms = 0;
+    { int32_t rc = device_sms(&sms); if (rc != ELG_OK) return rc; }
+    cudaStream_t st = (cudaStream_t)stream;
+    noalloc_prepare_kernel<<<(4 * nb + kBlock - 1) / kBlock, kBlock, 0, st>>>(scratch, (long long)n, t_lo, dt, nb, d_counts);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    DipoleArgs d;
+    d.s = d_s; d.x = d_x; d.y = d_y;
+    d.st = reinterpret_cast<DevState*>(scratch); d.prof_kind = -1; d.cur = 0; d.inv_bc = inv_bc; d.nb = nb;
+    d.smem_bins = nb < kDipoleSmemBins ? (nb + 31) / 32 * 32 : kDipoleSmemBins;
+    d.counts = d_counts;
+    d.dacc = reinterpret_cast<unsigned long long*>(scratch + kNoAllocStateBytes);
+    int occ = 0;
+    ELG_CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dipole_hist_kernel, kBlock, (size_t)d.smem_bins * 36));
+    if (occ < 1) occ = 1;
+    dipole_hist_kernel<<<occ * sms, kBlock, (size_t)d.smem_bins * 36, st>>>(d);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    dipole_finalize_kernel<<<(nb + kBlock - 1) / kBlock, kBlock, 0, st>>>(d.dacc, nb, d_D);
+    g_launches++;
+    ELG_CK(cudaGetLastError());
+    return ELG_OK;
+}

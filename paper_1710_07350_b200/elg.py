@@ -36,6 +36,7 @@ EXPORTS = (
     "elg_profile_enable", "elg_profile_read",
     "elg_dbg_histogram", "elg_dbg_dipole_histogram", "elg_dbg_kick", "elg_dbg_tkick", "elg_dbg_compact",
     "elg_dbg_wake_samples", "elg_dbg_convolve", "elg_dbg_fp64_peak",
+    "elg_noalloc_max_bins", "elg_dipole_histogram_noalloc",
 )
 KERNEL_KINDS = ("chain", "chain_compact", "window", "hist", "wake_samples", "conv", "moments", "chain_long")
 
@@ -503,6 +504,23 @@ def dbg_dipole_histogram(s, x, y, p0c_eV: float, t_lo: float, dt: float, nb: int
     b.synchronize()
     D = d_D.cpu().numpy()
     return d_c.cpu().numpy().view(np.uint32), D[:nb], D[nb:]
+
+
+def dipole_histogram_noalloc(d_s, d_x, d_y, inv_bc: float, t_lo: float, dt: float, nb: int, d_counts, d_D, stream=None) -> None:
+    """elg_dipole_histogram_noalloc: every array is the CALLER's torch CUDA tensor (s, x, y float64[n]; counts int32[nb];
+    D float64[2 nb]); the library allocates nothing and does not synchronise.  Argument marshalling only."""
+    torch = _torch()
+    L = lib()
+    L.elg_dipole_histogram_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_double,
+                                               C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.elg_dipole_histogram_noalloc.restype = C.c_int32
+    st = stream if stream is not None else torch.cuda.current_stream(d_s.device)
+    _ck(L.elg_dipole_histogram_noalloc(d_s.data_ptr(), d_x.data_ptr(), d_y.data_ptr(), int(d_s.numel()), float(inv_bc), float(t_lo),
+                                       float(dt), int(nb), d_counts.data_ptr(), d_D.data_ptr(), st.cuda_stream))
+
+
+def noalloc_max_bins() -> int:
+    return int(lib().elg_noalloc_max_bins())
 
 
 def dbg_kick(s, delta, p0c_eV: float, t_lo: float, dt: float, nb: int, V, interp=True) -> np.ndarray:
